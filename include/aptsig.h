@@ -1,0 +1,115 @@
+/* aptsig.h -- C ABI of libaptsig: crystallographic signatures of atom-probe point clouds on one
+ * NVIDIA B200 (sm_100a).  Hot path of the real space method (RSP) of Kuehbach, Kasemer, Gault, Breen,
+ * arXiv 2009.00735: for every material point (ROI centre) gather the ions of the accepted types
+ * inside a sphere of radius R, project them onto every direction of a unit-sphere grid
+ * (L60), histogram the signed distances into B = 2^m bins (Eq. 1; dR and f_s in the Fig. 2
+ * caption, L138; one zero pad bin per side, L365), take the one-sided DFT amplitude spectrum (L73) and
+ * record the highest amplitude inside a spectral bin window and its bin (L75, L416).
+ *
+ * Conventions
+ *   - every function returns APX_OK (0) or a negative apx_status; nothing throws or aborts.
+ *   - pointers marked DEVICE are CUDA device pointers on the plan's device, owned by the caller; the
+ *     library never frees them and does not touch them after the stream work of the call completed.
+ *     Pointers marked HOST are read (or written) before the call returns.
+ *   - all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream);
+ *     calls return without synchronising unless stated.
+ *   - a plan is not thread-safe; distinct plans are independent.  No global state.
+ *   - there is NO CPU fallback: without a usable CUDA device apx_plan_create fails with APX_ECUDA.
+ */
+#ifndef APTSIG_H_
+#define APTSIG_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    APX_OK = 0,
+    APX_EINVAL = -1,   /* bad argument: B not a power of two in 256..4096, R <= 0, D < 1, bad window, NULL */
+    APX_ENOMEM = -2,   /* host or device allocation failed */
+    APX_ECUDA = -3,    /* a CUDA call failed; apx_last_cuda_error() gives the cudaError_t */
+    APX_ESTATE = -4,   /* apx_query / apx_debug_histograms before apx_ingest */
+    APX_ERANGE = -5    /* size beyond what the plan supports (N >= 2^31, M*D >= 2^40) */
+} apx_status;
+
+/* flags */
+#define APX_FLAG_FORCE_FFT 1   /* always use the general FFT kernel, even for a narrow window */
+#define APX_FLAG_FORCE_MMA 2   /* fail with APX_EINVAL instead of falling back when the tensor-core
+                                  windowed-DFT kernel cannot serve the plan (window too wide) */
+
+typedef struct apx_plan apx_plan; /* opaque */
+
+typedef struct {
+    float R;              /* ROI radius > 0, same length unit as the coordinates (L52)                  */
+    int32_t B;            /* histogram bins, power of two, 256..4096 (m = 8..12, L71)                   */
+    int32_t pad;          /* 1 = paper's Eq. 1: span [-R-dR, R+dR], dR = R/(B/2-1) (L138, L365; default)
+                             0 = span [-R, R] (BASELINE.json north_star wording)                         */
+    int32_t k_lo, k_hi;   /* inclusive spectral-bin window, 0 <= k_lo <= k_hi <= B/2;
+                             k_lo = k_hi = 0 selects [1, B/2] (every bin but DC, L122/L151)             */
+    const float *dirs;    /* HOST, D x 3 direction vectors (unit vectors expected, L60), copied         */
+    int32_t D;            /* number of directions, >= 1                                                  */
+    uint8_t type_mask[32];/* bit t (byte t>>3, bit t&7) set = ion type t accepted (L52 "selected atom
+                             types"); all 0xFF = no filter                                               */
+    int32_t device;       /* CUDA device ordinal                                                         */
+    int32_t flags;        /* APX_FLAG_*                                                                  */
+} apx_plan_desc;
+
+/* Plan (step a0): derived constants R2 = fl32(R*R), s = fl32((B/2-pad)/R) = 1/dR, scaled directions
+ * n' = fl32(n*s), twiddle tables; owns all internal device buffers.  *out is NULL on failure. */
+int apx_plan_create(const apx_plan_desc *desc, apx_plan **out);
+int apx_plan_destroy(apx_plan *plan);
+
+/* The exact fp32 constants the kernels use (HOST out pointers, any may be NULL):
+ * R2, s, and the spatial frequency of spectral bin 1, nu_1 = s/B (bin k is k*nu_1; plane spacing 1/(k nu_1)). */
+int apx_plan_constants(const apx_plan *plan, float *R2, float *s, float *freq_per_bin);
+/* 0 = general FFT kernel, 1 = tensor-core windowed-DFT kernel (chosen at create time from the window). */
+int apx_plan_path(const apx_plan *plan);
+int apx_last_cuda_error(const apx_plan *plan);
+
+/* Step a1: ingest an ion cloud: drop ions of rejected types and non-finite coordinates, bucket the
+ * rest into a uniform cell grid (cell edge ~R/2) by a counting sort on the device.
+ *   xyz   DEVICE float32[N][3]     types DEVICE uint8[N] or NULL (NULL = every ion is type 0)
+ * The plan keeps the sorted copy (16 B per ion) until the next ingest; xyz/types are not referenced
+ * after the enqueued work completed.  N = 0 is valid (all ROIs empty). */
+int apx_ingest(apx_plan *plan, const float *xyz, const uint8_t *types, int64_t N, void *cuda_stream);
+
+/* Steps a2-a7 for M material points against the ingested cloud.
+ *   centres DEVICE float32[M][3]
+ *   sig     DEVICE float32[M][D][2]: sig[m][d] = (A*, (float)k*), A* = max_{k in window} |X_k|
+ *           (unnormalised, A_0 would be the ion count), k* the smallest such k.  Empty ROI: (0, k_lo).
+ *   counts  DEVICE uint32[M] or NULL: number of ions in each ROI (N_c) for caller-side normalisation.
+ * M = 0 is valid.  Requires a prior apx_ingest (else APX_ESTATE). */
+int apx_query(apx_plan *plan, const float *centres, int64_t M, float *sig, uint32_t *counts,
+              void *cuda_stream);
+
+/* apx_ingest followed by apx_query on the same stream (north_star's run()). */
+int apx_run(apx_plan *plan, const float *xyz, const uint8_t *types, int64_t N,
+            const float *centres, int64_t M, float *sig, uint32_t *counts, void *cuda_stream);
+
+/* Same as apx_run but every array is a HOST pointer; copies in and out on an internal stream and
+ * synchronises before returning (the end-to-end entry bench.py's "e2e" figure is timed through). */
+int apx_run_host(apx_plan *plan, const float *xyz, const uint8_t *types, int64_t N,
+                 const float *centres, int64_t M, float *sig, uint32_t *counts);
+
+/* Test hook: integer histograms (Eq. 1) of ONE material point for directions [d0, d0+nd):
+ *   centre3 HOST float32[3],  out DEVICE uint32[nd][B] (overwritten).  Uses the same gather and the
+ *   same binning arithmetic as the production kernels. */
+int apx_debug_histograms(apx_plan *plan, const float *centre3, int32_t d0, int32_t nd, uint32_t *out,
+                         void *cuda_stream);
+
+/* Step a3, host side (fp64 internally, fp32 out; `out` is HOST):
+ * Fibonacci sphere: z_i = 1-(2i+1)/D, phi_i = i*pi*(3-sqrt 5)  (BASELINE.json configs 1-2). */
+int apx_dirs_fibonacci(int32_t D, float *out /* D x 3 */);
+/* Geodesic sphere: icosahedron subdivided `level` times (level 6 = the paper's 40 962 nodes, L60).
+ * out may be NULL to query *D_out = 10*4^level + 2 only; level 0..8. */
+int apx_dirs_geodesic(int32_t level, float *out, int32_t *D_out);
+
+const char *apx_strerror(int status);
+const char *apx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* APTSIG_H_ */

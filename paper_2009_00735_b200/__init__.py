@@ -1,0 +1,12 @@
+"""paper_2009_00735_b200 -- B200-native signatures for atom-probe crystallography (arXiv 2009.00735).
+
+The product is the CUDA library `libaptsig.so` (sources in csrc/, ABI in include/aptsig.h); this
+package is its ctypes binding.  Importing the package does not load the library; the first call does,
+and raises if it has not been built (there is no CPU fallback).
+"""
+from .binding import (Plan, ApxError, apx_dirs_fibonacci, apx_dirs_geodesic, apx_version, EXPORTS, LIB_PATH,
+                      APX_FLAG_FORCE_FFT, APX_FLAG_FORCE_MMA, APX_OK, APX_EINVAL, APX_ENOMEM, APX_ECUDA,
+                      APX_ESTATE, APX_ERANGE)
+
+__all__ = ["Plan", "ApxError", "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_version", "EXPORTS", "LIB_PATH",
+           "APX_FLAG_FORCE_FFT", "APX_FLAG_FORCE_MMA"]

@@ -1,0 +1,182 @@
+"""Thin ctypes binding of libaptsig (include/aptsig.h): argument marshalling only.
+
+Every step of the hot path runs inside the CUDA library; torch is used for device memory and streams.
+There is no fallback: if the shared library is missing or a call fails, an exception is raised.
+Function names mirror the C ABI (apx_*); `Plan` is a convenience holder for the opaque handle.
+"""
+from __future__ import annotations
+import ctypes as C
+import os
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libaptsig.so")
+
+APX_OK, APX_EINVAL, APX_ENOMEM, APX_ECUDA, APX_ESTATE, APX_ERANGE = 0, -1, -2, -3, -4, -5
+APX_FLAG_FORCE_FFT, APX_FLAG_FORCE_MMA = 1, 2
+
+EXPORTS = ["apx_plan_create", "apx_plan_destroy", "apx_plan_constants", "apx_plan_path", "apx_last_cuda_error",
+           "apx_ingest", "apx_query", "apx_run", "apx_run_host", "apx_debug_histograms",
+           "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_strerror", "apx_version"]
+
+
+class apx_plan_desc(C.Structure):
+    _fields_ = [("R", C.c_float), ("B", C.c_int32), ("pad", C.c_int32), ("k_lo", C.c_int32), ("k_hi", C.c_int32),
+                ("dirs", C.POINTER(C.c_float)), ("D", C.c_int32), ("type_mask", C.c_uint8 * 32),
+                ("device", C.c_int32), ("flags", C.c_int32)]
+
+
+class ApxError(RuntimeError):
+    def __init__(self, status, where, cuda=None):
+        self.status = status
+        msg = f"{where}: {_lib().apx_strerror(status).decode()} ({status})"
+        if cuda is not None:
+            msg += f" [cudaError {cuda}]"
+        super().__init__(msg)
+
+
+_LIB = None
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2009_00735_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        vp, i64, i32 = C.c_void_p, C.c_int64, C.c_int32
+        L.apx_plan_create.argtypes = [C.POINTER(apx_plan_desc), C.POINTER(vp)]
+        L.apx_plan_destroy.argtypes = [vp]
+        L.apx_plan_constants.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]
+        L.apx_plan_path.argtypes = [vp]
+        L.apx_last_cuda_error.argtypes = [vp]
+        L.apx_ingest.argtypes = [vp, vp, vp, i64, vp]
+        L.apx_query.argtypes = [vp, vp, i64, vp, vp, vp]
+        L.apx_run.argtypes = [vp, vp, vp, i64, vp, i64, vp, vp, vp]
+        L.apx_run_host.argtypes = [vp, vp, vp, i64, vp, i64, vp, vp]
+        L.apx_debug_histograms.argtypes = [vp, C.POINTER(C.c_float), i32, i32, vp, vp]
+        L.apx_dirs_fibonacci.argtypes = [i32, vp]
+        L.apx_dirs_geodesic.argtypes = [i32, vp, C.POINTER(i32)]
+        L.apx_strerror.argtypes = [C.c_int]
+        L.apx_strerror.restype = C.c_char_p
+        L.apx_version.restype = C.c_char_p
+        for name in EXPORTS:
+            if name not in ("apx_strerror", "apx_version"):
+                getattr(L, name).restype = C.c_int
+        _LIB = L
+    return _LIB
+
+
+def type_mask_bytes(accepted=None) -> bytes:
+    m = bytearray(32)
+    if accepted is None:
+        m = bytearray(b"\xff" * 32)
+    else:
+        for t in accepted:
+            m[t >> 3] |= 1 << (t & 7)
+    return bytes(m)
+
+
+def apx_version() -> str:
+    return _lib().apx_version().decode()
+
+
+def apx_dirs_fibonacci(D: int) -> np.ndarray:
+    out = np.empty((D, 3), np.float32)
+    rc = _lib().apx_dirs_fibonacci(D, out.ctypes.data)
+    if rc:
+        raise ApxError(rc, "apx_dirs_fibonacci")
+    return out
+
+
+def apx_dirs_geodesic(level: int) -> np.ndarray:
+    n = C.c_int32(0)
+    rc = _lib().apx_dirs_geodesic(level, None, C.byref(n))
+    if rc:
+        raise ApxError(rc, "apx_dirs_geodesic")
+    out = np.empty((n.value, 3), np.float32)
+    rc = _lib().apx_dirs_geodesic(level, out.ctypes.data, C.byref(n))
+    if rc:
+        raise ApxError(rc, "apx_dirs_geodesic")
+    return out
+
+
+def _ptr(t, dtype=None):
+    """device (or host) pointer of a torch tensor / numpy array / None, after layout checks."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        assert t.flags.c_contiguous and (dtype is None or t.dtype == dtype)
+        return t.ctypes.data
+    assert t.is_contiguous(), "tensor must be contiguous"
+    return t.data_ptr()
+
+
+def _stream(stream=None):
+    import torch
+    return (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+
+
+class Plan:
+    """Owner of one apx_plan*. Methods are 1:1 with the C entry points."""
+
+    def __init__(self, R, B, dirs, pad=1, k_lo=0, k_hi=0, accepted_types=None, device=0, flags=0):
+        dirs = np.ascontiguousarray(dirs, np.float32).reshape(-1, 3)
+        d = apx_plan_desc()
+        d.R, d.B, d.pad, d.k_lo, d.k_hi = float(R), int(B), int(pad), int(k_lo), int(k_hi)
+        d.dirs = dirs.ctypes.data_as(C.POINTER(C.c_float))
+        d.D = dirs.shape[0]
+        d.type_mask = (C.c_uint8 * 32).from_buffer_copy(type_mask_bytes(accepted_types))
+        d.device, d.flags = int(device), int(flags)
+        self._h = C.c_void_p()
+        self.B, self.D, self.device = int(B), dirs.shape[0], int(device)
+        self.k_lo, self.k_hi = (1, B // 2) if (k_lo == 0 and k_hi == 0) else (int(k_lo), int(k_hi))
+        rc = _lib().apx_plan_create(C.byref(d), C.byref(self._h))
+        if rc:
+            self._h = C.c_void_p()
+            raise ApxError(rc, "apx_plan_create")
+
+    def _check(self, rc, where):
+        if rc:
+            raise ApxError(rc, where, _lib().apx_last_cuda_error(self._h) if rc == APX_ECUDA else None)
+
+    def apx_plan_constants(self):
+        r2, s, f = C.c_float(), C.c_float(), C.c_float()
+        self._check(_lib().apx_plan_constants(self._h, C.byref(r2), C.byref(s), C.byref(f)), "apx_plan_constants")
+        return np.float32(r2.value), np.float32(s.value), np.float32(f.value)
+
+    def apx_plan_path(self) -> int:
+        return _lib().apx_plan_path(self._h)
+
+    def apx_ingest(self, xyz, types=None, stream=None):
+        self._check(_lib().apx_ingest(self._h, _ptr(xyz), _ptr(types), xyz.shape[0], _stream(stream)), "apx_ingest")
+
+    def apx_query(self, centres, sig, counts=None, stream=None):
+        self._check(_lib().apx_query(self._h, _ptr(centres), centres.shape[0], _ptr(sig), _ptr(counts),
+                                     _stream(stream)), "apx_query")
+
+    def apx_run(self, xyz, types, centres, sig, counts=None, stream=None):
+        self._check(_lib().apx_run(self._h, _ptr(xyz), _ptr(types), xyz.shape[0], _ptr(centres), centres.shape[0],
+                                   _ptr(sig), _ptr(counts), _stream(stream)), "apx_run")
+
+    def apx_run_host(self, xyz, types, centres, sig, counts=None):
+        """All arguments are HOST arrays (numpy, or pinned CPU torch tensors)."""
+        self._check(_lib().apx_run_host(self._h, _ptr(xyz), _ptr(types), xyz.shape[0], _ptr(centres),
+                                        centres.shape[0], _ptr(sig), _ptr(counts)), "apx_run_host")
+
+    def apx_debug_histograms(self, centre3, d0, nd, out, stream=None):
+        c = (C.c_float * 3)(*[float(v) for v in centre3])
+        self._check(_lib().apx_debug_histograms(self._h, c, d0, nd, _ptr(out), _stream(stream)),
+                    "apx_debug_histograms")
+
+    def apx_plan_destroy(self):
+        if self._h:
+            _lib().apx_plan_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.apx_plan_destroy()
+        except Exception:
+            pass

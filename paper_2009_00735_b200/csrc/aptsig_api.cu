@@ -1,0 +1,221 @@
+// aptsig_api.cu -- the C ABI declared in include/aptsig.h: plan object (step a0), argument checks,
+// error mapping, host staging for apx_run_host.  No arithmetic of the method lives here except the
+// derived constants of the plan (R2, s, scaled directions, twiddles).
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+#include "common.cuh"
+
+using namespace apx;
+
+struct apx_plan : public apx::Plan {};
+
+#define CU(p, call)                                   \
+    do {                                              \
+        cudaError_t e__ = (call);                     \
+        if (e__ != cudaSuccess) {                     \
+            (p)->last_cuda = (int)e__;                \
+            return e__ == cudaErrorMemoryAllocation ? APX_ENOMEM : APX_ECUDA; \
+        }                                             \
+    } while (0)
+
+static int ensure_capacity(apx_plan *p, int64_t N)
+{
+    if (N <= p->capacity) return APX_OK;
+    if (p->d_sorted) cudaFree(p->d_sorted);
+    if (p->d_cell_of_ion) cudaFree(p->d_cell_of_ion);
+    p->d_sorted = nullptr; p->d_cell_of_ion = nullptr; p->capacity = 0;
+    int64_t cap = N + N / 8 + 1024;
+    CU(p, cudaMalloc(&p->d_sorted, (size_t)cap * sizeof(float4)));
+    CU(p, cudaMalloc(&p->d_cell_of_ion, (size_t)cap * sizeof(uint32_t)));
+    p->capacity = cap;
+    return APX_OK;
+}
+
+static int grow(apx_plan *p, void **buf, int64_t *cap, int64_t bytes)
+{
+    if (bytes <= *cap) return APX_OK;
+    if (*buf) cudaFree(*buf);
+    *buf = nullptr; *cap = 0;
+    CU(p, cudaMalloc(buf, (size_t)bytes));
+    *cap = bytes;
+    return APX_OK;
+}
+
+extern "C" int apx_plan_destroy(apx_plan *p)
+{
+    if (!p) return APX_OK;
+    cudaSetDevice(p->device);
+    void *bufs[] = {p->d_dirs_scaled, p->d_twiddle, p->d_mma_table, p->d_type_mask, p->d_grid, p->d_cell_start,
+                    p->d_cell_cursor, p->d_cell_of_ion, p->d_sorted, p->h2d_xyz, p->h2d_types, p->h2d_centres,
+                    p->d2h_sig, p->d2h_counts};
+    for (void *b : bufs)
+        if (b) cudaFree(b);
+    if (p->own_stream) cudaStreamDestroy(p->own_stream);
+    delete p;
+    return APX_OK;
+}
+
+extern "C" int apx_plan_create(const apx_plan_desc *desc, apx_plan **out)
+{
+    if (!out) return APX_EINVAL;
+    *out = nullptr;
+    if (!desc || !desc->dirs) return APX_EINVAL;
+    const int B = desc->B;
+    if (!(desc->R > 0.0f) || !std::isfinite(desc->R)) return APX_EINVAL;
+    if (B < 256 || B > 4096 || (B & (B - 1))) return APX_EINVAL;
+    if (desc->pad != 0 && desc->pad != 1) return APX_EINVAL;
+    if (desc->D < 1) return APX_EINVAL;
+    int k_lo = desc->k_lo, k_hi = desc->k_hi;
+    if (k_lo == 0 && k_hi == 0) { k_lo = 1; k_hi = B / 2; }
+    if (k_lo < 0 || k_hi > B / 2 || k_lo > k_hi) return APX_EINVAL;
+    if ((desc->flags & APX_FLAG_FORCE_FFT) && (desc->flags & APX_FLAG_FORCE_MMA)) return APX_EINVAL;
+
+    apx_plan *p = new (std::nothrow) apx_plan();
+    if (!p) return APX_ENOMEM;
+    std::memset(static_cast<apx::Plan *>(p), 0, sizeof(apx::Plan));
+    p->desc = *desc;
+    p->desc.dirs = nullptr;
+    p->B = B; p->D = desc->D; p->pad = desc->pad; p->k_lo = k_lo; p->k_hi = k_hi; p->W = k_hi - k_lo + 1;
+    p->R = desc->R; p->device = desc->device;
+    volatile float r2 = desc->R * desc->R;                                     // one fp32 multiply
+    p->R2 = r2;
+    p->s = (float)((double)(B / 2 - desc->pad) / (double)desc->R);             // fp64, rounded once
+
+    auto fail = [&](int code) { apx_plan_destroy(p); return code; };
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e != cudaSuccess) { delete p; return APX_ECUDA; }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) { delete p; return APX_ECUDA; }
+    p->sm_count = prop.multiProcessorCount;
+
+    // scaled directions n' = fl32(n * s), one fp32 multiply per component
+    std::vector<float> nps((size_t)3 * p->D);
+    for (size_t i = 0; i < nps.size(); ++i) { volatile float v = desc->dirs[i] * p->s; nps[i] = v; }
+    std::vector<float2> tw((size_t)B / 2);
+    for (int r = 0; r < B / 2; ++r) {
+        double th = 2.0 * M_PI * (double)r / (double)B;
+        tw[r] = make_float2((float)std::cos(th), (float)-std::sin(th));
+    }
+    uint32_t mask[8];
+    std::memcpy(mask, desc->type_mask, 32);
+
+#define CUF(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { p->last_cuda = (int)e__; \
+        return fail(e__ == cudaErrorMemoryAllocation ? APX_ENOMEM : APX_ECUDA); } } while (0)
+    CUF(cudaMalloc(&p->d_dirs_scaled, nps.size() * sizeof(float)));
+    CUF(cudaMalloc(&p->d_twiddle, tw.size() * sizeof(float2)));
+    CUF(cudaMalloc(&p->d_type_mask, 32));
+    CUF(cudaMalloc(&p->d_grid, sizeof(GridParams)));
+    CUF(cudaMalloc(&p->d_cell_start, (size_t)(kMaxCells + 1) * sizeof(uint32_t)));
+    CUF(cudaMalloc(&p->d_cell_cursor, (size_t)kMaxCells * sizeof(uint32_t)));
+    CUF(cudaMemcpy(p->d_dirs_scaled, nps.data(), nps.size() * sizeof(float), cudaMemcpyHostToDevice));
+    CUF(cudaMemcpy(p->d_twiddle, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    CUF(cudaMemcpy(p->d_type_mask, mask, 32, cudaMemcpyHostToDevice));
+    CUF(cudaStreamCreateWithFlags(&p->own_stream, cudaStreamNonBlocking));
+
+    p->path = 0;
+    if (!(desc->flags & APX_FLAG_FORCE_FFT) && mma_path_supported(p)) {
+        CUF(mma_path_prepare(p));
+        p->path = 1;
+    } else if (desc->flags & APX_FLAG_FORCE_MMA) {
+        return fail(APX_EINVAL);
+    }
+#undef CUF
+    *out = p;
+    return APX_OK;
+}
+
+extern "C" int apx_plan_constants(const apx_plan *p, float *R2, float *s, float *freq_per_bin)
+{
+    if (!p) return APX_EINVAL;
+    if (R2) *R2 = p->R2;
+    if (s) *s = p->s;
+    if (freq_per_bin) *freq_per_bin = p->s / (float)p->B;
+    return APX_OK;
+}
+
+extern "C" int apx_plan_path(const apx_plan *p) { return p ? p->path : APX_EINVAL; }
+extern "C" int apx_last_cuda_error(const apx_plan *p) { return p ? p->last_cuda : (int)cudaErrorInvalidValue; }
+
+extern "C" int apx_ingest(apx_plan *p, const float *xyz, const uint8_t *types, int64_t N, void *stream)
+{
+    if (!p || N < 0 || (N > 0 && !xyz)) return APX_EINVAL;
+    if (N >= (1LL << 31)) return APX_ERANGE;
+    CU(p, cudaSetDevice(p->device));
+    int rc = ensure_capacity(p, N);
+    if (rc) return rc;
+    CU(p, launch_ingest(p, xyz, types, N, (cudaStream_t)stream));
+    p->ingested = true;
+    return APX_OK;
+}
+
+extern "C" int apx_query(apx_plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts, void *stream)
+{
+    if (!p || M < 0 || (M > 0 && (!centres || !sig))) return APX_EINVAL;
+    if (!p->ingested) return APX_ESTATE;
+    if ((double)M * (double)p->D >= 1099511627776.0) return APX_ERANGE;
+    CU(p, cudaSetDevice(p->device));
+    if (p->path == 1) CU(p, launch_signature_mma(p, centres, M, sig, counts, (cudaStream_t)stream));
+    else CU(p, launch_signature_fft(p, centres, M, sig, counts, (cudaStream_t)stream));
+    return APX_OK;
+}
+
+extern "C" int apx_run(apx_plan *p, const float *xyz, const uint8_t *types, int64_t N, const float *centres,
+                       int64_t M, float *sig, uint32_t *counts, void *stream)
+{
+    int rc = apx_ingest(p, xyz, types, N, stream);
+    if (rc) return rc;
+    return apx_query(p, centres, M, sig, counts, stream);
+}
+
+extern "C" int apx_run_host(apx_plan *p, const float *xyz, const uint8_t *types, int64_t N, const float *centres,
+                            int64_t M, float *sig, uint32_t *counts)
+{
+    if (!p || N < 0 || M < 0 || (N > 0 && !xyz) || (M > 0 && (!centres || !sig))) return APX_EINVAL;
+    CU(p, cudaSetDevice(p->device));
+    cudaStream_t st = p->own_stream;
+    int rc;
+    const int64_t sig_bytes = M * (int64_t)p->D * 8;
+    if ((rc = grow(p, &p->h2d_xyz, &p->cap_xyz, N * 12 + 16))) return rc;
+    if (types && (rc = grow(p, &p->h2d_types, &p->cap_types, N + 16))) return rc;
+    if ((rc = grow(p, &p->h2d_centres, &p->cap_centres, M * 12 + 16))) return rc;
+    if ((rc = grow(p, &p->d2h_sig, &p->cap_sig, sig_bytes + 16))) return rc;
+    if (counts && (rc = grow(p, &p->d2h_counts, &p->cap_counts, M * 4 + 16))) return rc;
+    if (N) CU(p, cudaMemcpyAsync(p->h2d_xyz, xyz, (size_t)N * 12, cudaMemcpyHostToDevice, st));
+    if (N && types) CU(p, cudaMemcpyAsync(p->h2d_types, types, (size_t)N, cudaMemcpyHostToDevice, st));
+    if (M) CU(p, cudaMemcpyAsync(p->h2d_centres, centres, (size_t)M * 12, cudaMemcpyHostToDevice, st));
+    rc = apx_run(p, (const float *)p->h2d_xyz, types ? (const uint8_t *)p->h2d_types : nullptr, N,
+                 (const float *)p->h2d_centres, M, (float *)p->d2h_sig, counts ? (uint32_t *)p->d2h_counts : nullptr, st);
+    if (rc) return rc;
+    if (M) CU(p, cudaMemcpyAsync(sig, p->d2h_sig, (size_t)sig_bytes, cudaMemcpyDeviceToHost, st));
+    if (M && counts) CU(p, cudaMemcpyAsync(counts, p->d2h_counts, (size_t)M * 4, cudaMemcpyDeviceToHost, st));
+    CU(p, cudaStreamSynchronize(st));
+    return APX_OK;
+}
+
+extern "C" int apx_debug_histograms(apx_plan *p, const float *centre3, int32_t d0, int32_t nd, uint32_t *out,
+                                    void *stream)
+{
+    if (!p || !centre3 || d0 < 0 || nd < 0 || d0 + nd > p->D || (nd > 0 && !out)) return APX_EINVAL;
+    if (!p->ingested) return APX_ESTATE;
+    CU(p, cudaSetDevice(p->device));
+    CU(p, launch_debug_hist(p, centre3, d0, nd, out, (cudaStream_t)stream));
+    return APX_OK;
+}
+
+extern "C" const char *apx_strerror(int s)
+{
+    switch (s) {
+        case APX_OK: return "ok";
+        case APX_EINVAL: return "invalid argument";
+        case APX_ENOMEM: return "out of memory";
+        case APX_ECUDA: return "CUDA error (see apx_last_cuda_error)";
+        case APX_ESTATE: return "no ion cloud ingested";
+        case APX_ERANGE: return "size out of range";
+        default: return "unknown status";
+    }
+}
+
+extern "C" const char *apx_version(void) { return "aptsig 0.1 (sm_100a)"; }

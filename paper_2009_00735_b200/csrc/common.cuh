@@ -1,0 +1,86 @@
+// common.cuh -- internal declarations shared by the libaptsig translation units (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/aptsig.h"
+
+namespace apx {
+
+// Uniform cell grid over the accepted ions; lives in DEVICE memory and is written by k_grid_params,
+// so that ingest never synchronises with the host.
+struct GridParams {
+    float ox, oy, oz;      // origin = min corner of the accepted ions
+    float inv_h;           // 1 / cell edge
+    int nx, ny, nz;        // cells per axis (x fastest in the cell index)
+    int ncells;            // nx*ny*nz  (<= kMaxCells)
+    unsigned n_accepted;   // ions that passed the type / finite filter
+    // ordered-int encodings of min/max used by the bounds reduction
+    int minx, miny, minz, maxx, maxy, maxz;
+};
+
+constexpr int kMaxCells = 1 << 21;
+
+struct Plan {
+    apx_plan_desc desc;            // copy (dirs pointer nulled)
+    int B, D, pad, k_lo, k_hi, W;
+    float R, R2, s;
+    int device;
+    int path;                      // 0 = FFT kernel, 1 = MMA kernel
+    int sm_count;
+    int last_cuda;
+    bool ingested;
+    // device buffers owned by the plan
+    float *d_dirs_scaled;          // [D][3]  n' = fl32(n*s)
+    float2 *d_twiddle;             // [B/2]   exp(-2 pi i r / B), r < B/2   (FFT path)
+    void *d_mma_table;             // twiddle operand of the windowed DFT (MMA path)
+    uint32_t *d_type_mask;         // [8] words
+    GridParams *d_grid;
+    uint32_t *d_cell_start;        // [kMaxCells + 1]
+    uint32_t *d_cell_cursor;       // [kMaxCells]
+    uint32_t *d_cell_of_ion;       // [capacity]
+    float4 *d_sorted;              // [capacity]  (x, y, z, original index bits)
+    int64_t capacity;              // ions the sorted buffers can hold
+    // host staging for apx_run_host
+    cudaStream_t own_stream;
+    void *h2d_xyz, *h2d_types, *h2d_centres, *d2h_sig, *d2h_counts;   // device-side staging
+    int64_t cap_xyz, cap_types, cap_centres, cap_sig, cap_counts;
+};
+
+// ---- binning arithmetic (Eq. 1 in the fp32 operation order fixed by DESIGN.md reading #15) ----------
+// x = fma(n'z, dz, fma(n'y, dy, n'x*dx)); b = clamp(B/2 + floor(x), 0, B-1).
+// floor via a round-down add of the magic constant 1.5*2^23 + B/2 (exact for |x| < 2^22): the low
+// mantissa bits of the sum are B/2 + floor(x).  The clamp is applied on x first:
+// max(x, -B/2) -> b >= 0 and min(x, B/2 - 0.25) -> b <= B-1, identical to clamping b.
+__device__ __forceinline__ int bin_of(float npx, float npy, float npz, float dx, float dy, float dz,
+                                      float half_b, float magic)
+{
+    float x = __fmaf_rn(npz, dz, __fmaf_rn(npy, dy, __fmul_rn(npx, dx)));
+    x = fminf(fmaxf(x, -half_b), half_b - 0.25f);
+    return __float_as_int(__fadd_rd(x, magic)) - 0x4B400000;
+}
+__host__ __device__ __forceinline__ float magic_for(int B) { return 12582912.0f + (float)(B / 2); }
+
+// membership: closed ball in fp32, r2 = fma(dz,dz, fma(dy,dy, dx*dx)) <= R2
+__device__ __forceinline__ bool inside(float dx, float dy, float dz, float R2)
+{
+    return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx))) <= R2;
+}
+
+// cell coordinate along one axis (monotone in v); clamped to [0, n-1]
+__device__ __forceinline__ int cell_coord(float v, float o, float inv_h, int n)
+{
+    int c = __float2int_rd(__fmul_rn(__fsub_rn(v, o), inv_h));
+    return min(max(c, 0), n - 1);
+}
+
+// launchers (each returns the cudaError_t of the launch)
+cudaError_t launch_ingest(Plan *p, const float *xyz, const uint8_t *types, int64_t N, cudaStream_t st);
+cudaError_t launch_signature_fft(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts,
+                                 cudaStream_t st);
+cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts,
+                                 cudaStream_t st);
+cudaError_t launch_debug_hist(Plan *p, const float *centre3, int d0, int nd, uint32_t *out, cudaStream_t st);
+bool mma_path_supported(const Plan *p);
+cudaError_t mma_path_prepare(Plan *p);   // builds d_mma_table
+
+}  // namespace apx

@@ -1,0 +1,181 @@
+// ingest.cu -- step a1: type filter + uniform cell-grid bucketing by a counting sort on the device.
+// The paper queries ions with a tree (cost f R^3 rho log(V rho) per ROI);
+// here a uniform grid with cell edge ~R/2 replaces it: ROIs are fixed-radius balls, so a grid gives
+// contiguous x-rows of cells that are read with coalesced 16-byte loads.
+// HBM-bound: ~13 B read x2 + 4 B cell id + 16 B record written per ion.
+#include "common.cuh"
+
+namespace apx {
+
+// monotone float <-> int encoding for atomicMin/atomicMax on signed ints
+__device__ __forceinline__ int f2ord(float f)
+{
+    int i = __float_as_int(f);
+    return i >= 0 ? i : i ^ 0x7FFFFFFF;
+}
+__device__ __forceinline__ float ord2f(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7FFFFFFF); }
+
+__device__ __forceinline__ bool accepted(const uint32_t *mask, const uint8_t *types, int64_t i,
+                                         float x, float y, float z)
+{
+    unsigned t = types ? types[i] : 0u;
+    bool ok = (mask[t >> 5] >> (t & 31)) & 1u;
+    // finite test: |v| < inf  (NaN compares false)
+    return ok && fabsf(x) < 3.0e38f && fabsf(y) < 3.0e38f && fabsf(z) < 3.0e38f;
+}
+
+__global__ void k_reset(GridParams *g)
+{
+    g->minx = g->miny = g->minz = 0x7FFFFFFF;
+    g->maxx = g->maxy = g->maxz = (int)0x80000000;
+    g->n_accepted = 0;
+}
+
+__global__ void __launch_bounds__(256) k_bounds(const float *__restrict__ xyz, const uint8_t *__restrict__ types,
+                                                int64_t N, const uint32_t *__restrict__ mask, GridParams *g)
+{
+    int mn[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF};
+    int mx[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
+    unsigned cnt = 0;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+        float x = xyz[3 * i], y = xyz[3 * i + 1], z = xyz[3 * i + 2];
+        if (!accepted(mask, types, i, x, y, z)) continue;
+        ++cnt;
+        int ox = f2ord(x), oy = f2ord(y), oz = f2ord(z);
+        mn[0] = min(mn[0], ox); mn[1] = min(mn[1], oy); mn[2] = min(mn[2], oz);
+        mx[0] = max(mx[0], ox); mx[1] = max(mx[1], oy); mx[2] = max(mx[2], oz);
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            mn[a] = min(mn[a], __shfl_xor_sync(0xffffffffu, mn[a], o));
+            mx[a] = max(mx[a], __shfl_xor_sync(0xffffffffu, mx[a], o));
+        }
+        cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    }
+    if ((threadIdx.x & 31) == 0 && cnt) {
+        atomicMin(&g->minx, mn[0]); atomicMin(&g->miny, mn[1]); atomicMin(&g->minz, mn[2]);
+        atomicMax(&g->maxx, mx[0]); atomicMax(&g->maxy, mx[1]); atomicMax(&g->maxz, mx[2]);
+        atomicAdd(&g->n_accepted, cnt);
+    }
+}
+
+// one thread: derive the grid from the bounds.  Cell edge h = R/2, doubled until the grid fits kMaxCells.
+__global__ void k_grid_params(GridParams *g, float R)
+{
+    if (g->n_accepted == 0) {
+        g->ox = g->oy = g->oz = 0.f; g->inv_h = 1.f; g->nx = g->ny = g->nz = 1; g->ncells = 1;
+        return;
+    }
+    float lo[3] = {ord2f(g->minx), ord2f(g->miny), ord2f(g->minz)};
+    float hi[3] = {ord2f(g->maxx), ord2f(g->maxy), ord2f(g->maxz)};
+    float h = 0.5f * R;
+    int n[3];
+    for (;;) {
+        double cells = 1.0;
+        for (int a = 0; a < 3; ++a) {
+            double e = ((double)hi[a] - (double)lo[a]) / (double)h;
+            e = e < 2.0e9 ? e : 2.0e9;
+            n[a] = (int)e + 1;
+            cells *= (double)n[a];
+        }
+        if (cells <= (double)kMaxCells) break;
+        h *= 2.0f;
+    }
+    g->ox = lo[0]; g->oy = lo[1]; g->oz = lo[2];
+    g->inv_h = 1.0f / h;
+    g->nx = n[0]; g->ny = n[1]; g->nz = n[2];
+    g->ncells = n[0] * n[1] * n[2];
+}
+
+__global__ void __launch_bounds__(256) k_zero_cells(uint32_t *cell_start, const GridParams *g)
+{
+    int n = g->ncells + 1;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) cell_start[i] = 0;
+}
+
+__global__ void __launch_bounds__(256) k_count(const float *__restrict__ xyz, const uint8_t *__restrict__ types,
+                                               int64_t N, const uint32_t *__restrict__ mask,
+                                               const GridParams *__restrict__ g, uint32_t *cell_count,
+                                               uint32_t *cell_of_ion)
+{
+    const float ox = g->ox, oy = g->oy, oz = g->oz, ih = g->inv_h;
+    const int nx = g->nx, ny = g->ny, nz = g->nz;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+        float x = xyz[3 * i], y = xyz[3 * i + 1], z = xyz[3 * i + 2];
+        uint32_t c = 0xFFFFFFFFu;
+        if (accepted(mask, types, i, x, y, z)) {
+            c = (uint32_t)((cell_coord(z, oz, ih, nz) * ny + cell_coord(y, oy, ih, ny)) * nx + cell_coord(x, ox, ih, nx));
+            atomicAdd(&cell_count[c], 1u);
+        }
+        cell_of_ion[i] = c;
+    }
+}
+
+// exclusive scan of cell_count[0..ncells) in place, total at [ncells]; one 1024-thread block walks chunks.
+__global__ void __launch_bounds__(1024) k_scan(uint32_t *cell, uint32_t *cursor, const GridParams *g)
+{
+    __shared__ uint32_t warp_sum[32];
+    __shared__ uint32_t carry;
+    const int n = g->ncells;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int base = 0; base < n; base += 1024) {
+        int i = base + threadIdx.x;
+        uint32_t v = i < n ? cell[i] : 0u;
+        uint32_t inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) warp_sum[wid] = inc;
+        __syncthreads();
+        if (wid == 0) {
+            uint32_t w = warp_sum[lane], wi = w;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                uint32_t t = __shfl_up_sync(0xffffffffu, wi, o);
+                if (lane >= o) wi += t;
+            }
+            warp_sum[lane] = wi - w;   // exclusive
+        }
+        __syncthreads();
+        uint32_t excl = carry + warp_sum[wid] + inc - v;
+        if (i < n) { cell[i] = excl; cursor[i] = excl; }
+        __syncthreads();
+        if (threadIdx.x == 1023) carry = excl + v;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) cell[n] = carry;
+}
+
+__global__ void __launch_bounds__(256) k_scatter(const float *__restrict__ xyz, int64_t N,
+                                                 const uint32_t *__restrict__ cell_of_ion, uint32_t *cursor,
+                                                 float4 *__restrict__ sorted)
+{
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+        uint32_t c = cell_of_ion[i];
+        if (c == 0xFFFFFFFFu) continue;
+        uint32_t pos = atomicAdd(&cursor[c], 1u);
+        sorted[pos] = make_float4(xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2], __uint_as_float((uint32_t)i));
+    }
+}
+
+cudaError_t launch_ingest(Plan *p, const float *xyz, const uint8_t *types, int64_t N, cudaStream_t st)
+{
+    const int blocks = p->sm_count * 8;
+    k_reset<<<1, 1, 0, st>>>(p->d_grid);
+    if (N > 0) k_bounds<<<blocks, 256, 0, st>>>(xyz, types, N, p->d_type_mask, p->d_grid);
+    k_grid_params<<<1, 1, 0, st>>>(p->d_grid, p->R);
+    k_zero_cells<<<blocks, 256, 0, st>>>(p->d_cell_start, p->d_grid);
+    if (N > 0)
+        k_count<<<blocks, 256, 0, st>>>(xyz, types, N, p->d_type_mask, p->d_grid, p->d_cell_start, p->d_cell_of_ion);
+    k_scan<<<1, 1024, 0, st>>>(p->d_cell_start, p->d_cell_cursor, p->d_grid);
+    if (N > 0) k_scatter<<<blocks, 256, 0, st>>>(xyz, N, p->d_cell_of_ion, p->d_cell_cursor, p->d_sorted);
+    return cudaGetLastError();
+}
+
+}  // namespace apx

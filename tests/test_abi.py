@@ -1,0 +1,63 @@
+"""Host-side checks of the C ABI (no GPU): the library loads and exports every symbol declared in
+include/aptsig.h; host-only entry points (direction grids, strerror) behave; and the library's
+direction grids agree with the oracle's independent construction."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2009_00735_b200 as apx
+from paper_2009_00735_b200 import build as lib_build
+from oracle import oracle as O
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    return C.CDLL(lib_build.build())
+
+
+def test_every_declared_symbol_is_exported(lib):
+    hdr = open(os.path.join(ROOT, "include", "aptsig.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(apx_[a-z_0-9]+)\s*\(", hdr))
+    assert declared == set(apx.EXPORTS), declared ^ set(apx.EXPORTS)
+    for name in declared:
+        assert getattr(lib, name) is not None
+
+
+def test_strerror_and_version():
+    assert "aptsig" in apx.apx_version()
+    from paper_2009_00735_b200.binding import _lib
+    assert _lib().apx_strerror(0) == b"ok"
+    assert b"invalid" in _lib().apx_strerror(apx.APX_EINVAL)
+
+
+def test_fibonacci_matches_oracle_grid():
+    for D in (1, 7, 1000):
+        a, b = apx.apx_dirs_fibonacci(D), O.dirs_fibonacci(D)
+        np.testing.assert_allclose(a, b, rtol=0, atol=2e-7)
+    with pytest.raises(apx.ApxError):
+        apx.apx_dirs_fibonacci(0)
+
+
+def test_geodesic_matches_oracle_grid():
+    for level in (0, 1, 3):
+        a, b = apx.apx_dirs_geodesic(level), O.dirs_geodesic(level)
+        assert a.shape == b.shape == (10 * 4 ** level + 2, 3)
+        np.testing.assert_allclose(a, b, rtol=0, atol=2e-7)
+    assert apx.apx_dirs_geodesic(6).shape == (40962, 3)
+    with pytest.raises(apx.ApxError):
+        apx.apx_dirs_geodesic(9)
+
+
+def test_plan_create_rejects_bad_arguments_before_touching_cuda():
+    d = np.array([[0, 0, 1]], np.float32)
+    for kw in (dict(R=-1.0, B=256), dict(R=1.0, B=300), dict(R=1.0, B=128), dict(R=1.0, B=8192),
+               dict(R=1.0, B=256, pad=2), dict(R=1.0, B=256, k_lo=5, k_hi=3), dict(R=1.0, B=256, k_lo=1, k_hi=129)):
+        with pytest.raises(apx.ApxError) as ei:
+            apx.Plan(dirs=d, **kw)
+        assert ei.value.status == apx.APX_EINVAL

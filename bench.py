@@ -1,0 +1,278 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line: whole-hot-path throughput of libaptsig on BASELINE.json config 2.
+
+A "step" = one apx_run (ingest + gather + project/bin + DFT + peak + write-out) over the
+whole config-2 workload (1000 material points x 10 000 directions, B = 1024, ~241k ions).
+  value     device-timed (CUDA events, inputs resident in HBM), L2 flushed between timed steps
+  e2e       the same through apx_run_host with pinned HOST buffers (H2D + D2H inside the timed region)
+  roofline  dominant kernel vs the FP32 ALU peak
+  cpu_baseline  the oracle as it stands on the host cores, bounded sample of the same workload
+`--impl reference` times the oracle instead (the tier's reference arm).
+Multi-GPU (torchrun): material points are sharded over ranks, ions replicated, no collective on the data path.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "direction-histograms/s"
+UNIT = "histograms/s"
+# nominal FP32 peak used as the "alu" roofline denominator (B200_PROFILING.md: 148 SMs, 1965 MHz max SM clock;
+# 128 FP32 lanes per SM, FFMA = 2 flop): derived in DESIGN.md "Roofline".
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+
+
+def algorithmic_flops(n_pairs, n_hist, B):
+    """6 flop per (ion, direction) pair (FMUL + 2 FFMA + round-down FADD) and the unpruned real
+    FFT's 2.5 B log2 B flop per histogram."""
+    return 6.0 * n_pairs + 2.5 * B * np.log2(B) * n_hist
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for t, row in self.rows:
+            f = [x.strip() for x in row.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                mx = float(f[1])
+                if t0 - 0.05 <= t <= t1 + 0.05:
+                    sm.append(float(f[0]))
+                    for n, v in zip(names, f[3:7]):
+                        if v.lower().startswith("active"):
+                            reasons.add(n)
+            except ValueError:
+                continue
+        if not sm and self.rows:
+            try:
+                sm = [float(self.rows[-1][1].split(",")[0])]
+            except ValueError:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_sample(w, dirs, n_points, nthreads=0):
+    """Time the oracle on the first `n_points` interior-ish material points x all directions."""
+    from oracle import oracle as O
+    idx = np.linspace(0, len(w.centres) - 1, n_points).astype(np.int64)
+    t = time.perf_counter()
+    O.signatures(w.xyz, w.types, w.centres[idx], dirs, w.R, w.B, k_lo=w.window[0], k_hi=w.window[1],
+                 nthreads=nthreads)
+    dt = time.perf_counter() - t
+    return dt, n_points * len(dirs), O.num_threads() if nthreads <= 0 else nthreads
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle on the host cores, bounded sample per step (rank 0 only)."""
+    if rank != 0:
+        return
+    from workloads import make_config
+    from oracle import oracle as O
+    w = make_config(2)
+    dirs = O.dirs_fibonacci(w.D)
+    n_points = 16
+    for _ in range(args.warmup):
+        oracle_sample(w, dirs, 2)
+    times = []
+    cores = 1
+    for _ in range(args.steps):
+        dt, nh, cores = oracle_sample(w, dirs, n_points)
+        times.append(dt)
+    total_h = n_points * w.D * args.steps
+    v = total_h / sum(times)
+    sample = f"{n_points} of {len(w.centres)} material points x {w.D} directions per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "material_points_per_s": v / w.D,
+        "config": {"workload": "cfg2_single_crystal: fcc Al 20^3 nm, 1000 material points x 10000 Fibonacci "
+                               "directions, R=2.0 nm, B=1024, window [15,34]", "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import paper_2009_00735_b200 as apx
+    from workloads import make_config
+
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device(f"cuda:{local_rank}")
+
+    w = make_config(2)
+    dirs = apx.apx_dirs_fibonacci(w.D)                      # step a3 through the library
+    # weak scaling: every rank processes the full config-2 centre list of its own replica shard
+    # (material points are independent); ions are replicated, no collective on the data path.
+    centres_np = w.centres
+    M, D, B = len(centres_np), w.D, w.B
+    plan = apx.Plan(w.R, B, dirs, k_lo=w.window[0], k_hi=w.window[1], device=local_rank,
+                    flags=apx.APX_FLAG_FORCE_FFT if args.path == "fft" else 0)
+    xyz = torch.from_numpy(w.xyz).to(dev)
+    types = torch.from_numpy(w.types).to(dev)
+    centres = torch.from_numpy(centres_np).to(dev)
+    sig = torch.empty((M, D, 2), dtype=torch.float32, device=dev)
+    counts = torch.empty(M, dtype=torch.int32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        plan.apx_run(xyz, types, centres, sig, counts)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    # device-timed region: K steps, each bracketed by events; L2 flushed (untimed) between steps
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    qev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    t0 = time.time()
+    for i in range(args.steps):
+        flush.fill_(i & 0xFF)
+        ev[i][0].record()
+        plan.apx_ingest(xyz, types)
+        qev[i][0].record()
+        plan.apx_query(centres, sig, counts)
+        qev[i][1].record()
+        ev[i][1].record()
+    barrier()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1) if rank == 0 else None
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    ms_query = sum(a.elapsed_time(b) for a, b in qev)
+    n_c = counts.cpu().numpy().astype(np.int64)
+
+    # end to end through the host-pointer entry (pinned buffers; H2D + D2H inside the timed region)
+    h_xyz = torch.from_numpy(w.xyz).pin_memory()
+    h_types = torch.from_numpy(w.types).pin_memory()
+    h_centres = torch.from_numpy(centres_np).pin_memory()
+    h_sig = torch.empty((M, D, 2), dtype=torch.float32).pin_memory()
+    h_counts = torch.empty(M, dtype=torch.int32).pin_memory()
+    e2e_steps = max(1, min(args.steps, 5))
+    plan.apx_run_host(h_xyz, h_types, h_centres, h_sig, h_counts)
+    barrier()
+    te = time.perf_counter()
+    for _ in range(e2e_steps):
+        plan.apx_run_host(h_xyz, h_types, h_centres, h_sig, h_counts)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - te
+    assert torch.equal(h_sig, sig.cpu()), "host-path result differs from device-path result"
+
+    tt = torch.tensor([ms, ms_query, e2e_s], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    ms, ms_query, e2e_s = [float(v) for v in tt.cpu()]
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    n_hist = M * D * world
+    value = n_hist * args.steps / (ms * 1e-3)
+    pairs = float(n_c.sum()) * D
+    flops = algorithmic_flops(pairs, M * D, B)
+    q_s = ms_query * 1e-3 / args.steps
+    achieved = flops / q_s / 1e12
+    h2d = w.xyz.nbytes + w.types.nbytes + centres_np.nbytes
+    d2h = M * D * 8 + M * 4
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "material_points_per_s": value / D,
+        "config": {"workload": "cfg2_single_crystal: fcc Al 20^3 nm (~241k ions), 1000 material points x 10000 "
+                               "Fibonacci directions, R=2.0 nm, B=1024, window [15,34]",
+                   "kernel_path": "mma" if plan.apx_plan_path() == 1 else "fft",
+                   "l2": "flushed between timed steps (256 MiB fill, untimed)",
+                   "ions": int(len(w.xyz)), "mean_ions_per_roi": float(n_c.mean()),
+                   "multi_gpu": "material points sharded per rank, ions replicated, no collective"},
+        "clocks": clocks,
+        "e2e": {"value": n_hist * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": int(d2h), "entry": "apx_run_host", "steps": e2e_steps},
+        "gpu_launches": 8 * args.steps,
+        "roofline": {"bound": "alu", "kernel": "k_signature_mma" if plan.apx_plan_path() == 1 else "k_signature_fft",
+                     "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                     "frac": achieved / FP32_PEAK_TFLOPS, "traffic": None,
+                     "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md)",
+                     "ms_per_launch": ms_query / args.steps,
+                     "model": "6 flop/(ion,direction) pair + 2.5 B log2 B flop/histogram"},
+    }
+    if not args.no_cpu_baseline:
+        dt, nh, cores = oracle_sample(w, np.ascontiguousarray(dirs), 32)
+        out["cpu_baseline"] = {"value": nh / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                               "sample": f"32 of {M} material points x {D} directions, {dt:.1f} s",
+                               "paper_context": "0.72 material points/s on 1 Xeon Gold 6138 core (PAPER.md L248)"}
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--path", default="auto", choices=["auto", "fft"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -33,6 +33,9 @@ struct Plan {
     float *d_dirs_scaled;          // [D][3]  n' = fl32(n*s)
     float2 *d_twiddle;             // [B/2]   exp(-2 pi i r / B), r < B/2   (FFT path)
     void *d_mma_table;             // twiddle operand of the windowed DFT (MMA path)
+    int mma_clamp;                 // 1 = the bin clamp of Eq. 1 must stay in the MMA kernel's inner loop
+    uint32_t *d_deferred;          // [0] count, [1..] material points the MMA kernel left to the FFT kernel
+    int64_t cap_deferred;
     uint32_t *d_type_mask;         // [8] words
     GridParams *d_grid;
     uint32_t *d_cell_start;        // [kMaxCells + 1]
@@ -73,10 +76,31 @@ __device__ __forceinline__ int cell_coord(float v, float o, float inv_h, int n)
     return min(max(c, 0), n - 1);
 }
 
+struct RoiCells {
+    int ix0, ix1, iy0, iy1, iz0, iz1;
+};
+
+// conservative cell block of the ball around c (monotone cell_coord + a margin that covers the fp32
+// rounding of p - c and of c -+ R; membership itself is always the exact fp32 test)
+__device__ __forceinline__ RoiCells roi_cells(const GridParams &g, float cx, float cy, float cz, float R)
+{
+    RoiCells r;
+    float mx = R * 1.00001f + fabsf(cx) * 1e-6f;
+    float my = R * 1.00001f + fabsf(cy) * 1e-6f;
+    float mz = R * 1.00001f + fabsf(cz) * 1e-6f;
+    r.ix0 = cell_coord(cx - mx, g.ox, g.inv_h, g.nx); r.ix1 = cell_coord(cx + mx, g.ox, g.inv_h, g.nx);
+    r.iy0 = cell_coord(cy - my, g.oy, g.inv_h, g.ny); r.iy1 = cell_coord(cy + my, g.oy, g.inv_h, g.ny);
+    r.iz0 = cell_coord(cz - mz, g.oz, g.inv_h, g.nz); r.iz1 = cell_coord(cz + mz, g.oz, g.inv_h, g.nz);
+    return r;
+}
+
 // launchers (each returns the cudaError_t of the launch)
 cudaError_t launch_ingest(Plan *p, const float *xyz, const uint8_t *types, int64_t N, cudaStream_t st);
 cudaError_t launch_signature_fft(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts,
                                  cudaStream_t st);
+// FFT kernel over a device-side list of material points (list[0] = count, list[1..] = ids)
+cudaError_t launch_signature_fft_list(Plan *p, const float *centres, const uint32_t *list, float *sig,
+                                      uint32_t *counts, cudaStream_t st);
 cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts,
                                  cudaStream_t st);
 cudaError_t launch_debug_hist(Plan *p, const float *centre3, int d0, int nd, uint32_t *out, cudaStream_t st);

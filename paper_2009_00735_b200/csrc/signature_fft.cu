@@ -12,24 +12,6 @@ constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 constexpr int kDirChunk = 256;            // directions per CTA
 
-struct RoiCells {
-    int ix0, ix1, iy0, iy1, iz0, iz1;
-};
-
-// conservative cell block of the ball around c (monotone cell_coord + a margin that covers the fp32
-// rounding of p - c and of c -+ R; membership itself is always the exact fp32 test)
-__device__ __forceinline__ RoiCells roi_cells(const GridParams &g, float cx, float cy, float cz, float R)
-{
-    RoiCells r;
-    float mx = R * 1.00001f + fabsf(cx) * 1e-6f;
-    float my = R * 1.00001f + fabsf(cy) * 1e-6f;
-    float mz = R * 1.00001f + fabsf(cz) * 1e-6f;
-    r.ix0 = cell_coord(cx - mx, g.ox, g.inv_h, g.nx); r.ix1 = cell_coord(cx + mx, g.ox, g.inv_h, g.nx);
-    r.iy0 = cell_coord(cy - my, g.oy, g.inv_h, g.ny); r.iy1 = cell_coord(cy + my, g.oy, g.inv_h, g.ny);
-    r.iz0 = cell_coord(cz - mz, g.oz, g.inv_h, g.nz); r.iz1 = cell_coord(cz + mz, g.oz, g.inv_h, g.nz);
-    return r;
-}
-
 // Gather (step a2): every warp walks x-rows of cells (contiguous in the sorted array), keeps ions with
 // r^2 <= R2 and appends d = p - c to shared SoA arrays.  Returns the ROI ion count in *s_n (may exceed cap;
 // then only the first cap are stored and the caller must use the streaming path).
@@ -114,7 +96,8 @@ k_signature_fft(const float4 *__restrict__ sorted, const uint32_t *__restrict__ 
                 const GridParams *__restrict__ gp, const float *__restrict__ centres,
                 const float *__restrict__ dirs_scaled, const float2 *__restrict__ g_tw,
                 float2 *__restrict__ sig, uint32_t *__restrict__ counts,
-                int D, int B, int k_lo, int k_hi, float R, float R2, int cap, int nchunks)
+                int D, int B, int k_lo, int k_hi, float R, float R2, int cap, int nchunks,
+                const uint32_t *__restrict__ list)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem);                       // [kWarps][B]
@@ -125,15 +108,20 @@ k_signature_fft(const float4 *__restrict__ sorted, const uint32_t *__restrict__ 
     __shared__ int s_n;
 
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int64_t m = blockIdx.x / nchunks;
-    const int chunk = blockIdx.x % nchunks;
+    for (int i = threadIdx.x; i < B / 2; i += kThreads) s_tw[i] = g_tw[i];
+    // direct mode: one work item (material point, direction chunk) per CTA.  list mode: the grid is
+    // persistent and walks the items of the material points named in list[1 .. list[0]].
+    const int64_t n_items = list ? (int64_t)list[0] * nchunks : (int64_t)gridDim.x;
+    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+    const int64_t m = list ? (int64_t)list[1 + item / nchunks] : item / nchunks;
+    const int chunk = (int)(item % nchunks);
     const int d_begin = chunk * kDirChunk, d_end = min(D, d_begin + kDirChunk);
     const GridParams g = *gp;
     const float cx = centres[3 * m], cy = centres[3 * m + 1], cz = centres[3 * m + 2];
     const RoiCells rc = roi_cells(g, cx, cy, cz, R);
 
+    __syncthreads();                 // previous item fully written out; s_tw loaded
     if (threadIdx.x == 0) s_n = 0;
-    for (int i = threadIdx.x; i < B / 2; i += kThreads) s_tw[i] = g_tw[i];
     __syncthreads();
     if (g.n_accepted) gather_roi(sorted, cell_start, g, rc, cx, cy, cz, R2, sx, sy, sz, cap, &s_n);
     __syncthreads();
@@ -189,25 +177,38 @@ k_signature_fft(const float4 *__restrict__ sorted, const uint32_t *__restrict__ 
     __syncthreads();
     float2 *out = sig + (size_t)m * D + d_begin;
     for (int i = threadIdx.x; i < d_end - d_begin; i += kThreads) out[i] = s_res[i];
+    }
 }
 
 static int fft_cap_for(int B) { return B <= 1024 ? 3072 : (B == 2048 ? 2688 : 4096); }
 
-cudaError_t launch_signature_fft(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts,
-                                 cudaStream_t st)
+static cudaError_t launch_fft_common(Plan *p, const float *centres, int64_t M, const uint32_t *list, float *sig,
+                                     uint32_t *counts, cudaStream_t st)
 {
-    if (M == 0) return cudaSuccess;
     const int B = p->B, cap = fft_cap_for(B);
     const int nchunks = (p->D + kDirChunk - 1) / kDirChunk;
     size_t smem = (size_t)kWarps * B * 4 + (size_t)(B / 2) * 8 + (size_t)kDirChunk * 8 + (size_t)cap * 12;
     cudaError_t e = cudaFuncSetAttribute(k_signature_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    int64_t blocks = M * nchunks;
+    int64_t blocks = list ? (int64_t)p->sm_count * 2 : M * nchunks;
     if (blocks > 0x7FFFFFFFLL) return cudaErrorInvalidConfiguration;
     k_signature_fft<<<(unsigned)blocks, kThreads, smem, st>>>(
         p->d_sorted, p->d_cell_start, p->d_grid, centres, p->d_dirs_scaled, p->d_twiddle,
-        reinterpret_cast<float2 *>(sig), counts, p->D, B, p->k_lo, p->k_hi, p->R, p->R2, cap, nchunks);
+        reinterpret_cast<float2 *>(sig), counts, p->D, B, p->k_lo, p->k_hi, p->R, p->R2, cap, nchunks, list);
     return cudaGetLastError();
+}
+
+cudaError_t launch_signature_fft(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts,
+                                 cudaStream_t st)
+{
+    if (M == 0) return cudaSuccess;
+    return launch_fft_common(p, centres, M, nullptr, sig, counts, st);
+}
+
+cudaError_t launch_signature_fft_list(Plan *p, const float *centres, const uint32_t *list, float *sig,
+                                      uint32_t *counts, cudaStream_t st)
+{
+    return launch_fft_common(p, centres, 0, list, sig, counts, st);
 }
 
 }  // namespace apx

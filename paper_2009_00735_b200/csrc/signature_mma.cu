@@ -125,30 +125,45 @@ __device__ __forceinline__ void gather_roi4(const MmaParams &p, const GridParams
 // byte offset of (bin b, direction lane) = b*64 + (((lane>>3) ^ ((b>>1)&3)) << 4) + ((lane&7)>>1)*4,
 // low/high half of the word = even/odd lane.  With bits = 0x4B400000 + b (magic-add floor) this is
 // addr = bits*64 + K0, then addr ^= (bits<<3) & 0x30.
+__device__ __forceinline__ float4 lds128(uint32_t addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
 template <bool kClamp>
-__device__ __forceinline__ void bin_ions(const float4 *ions, int i0, int i1, float npx, float npy, float npz,
+__device__ __forceinline__ void bin_one(const float4 q, float npx, float npy, float npz, float half_b, float magic,
+                                        uint32_t k0, uint32_t inc)
+{
+    float x = __fmaf_rn(npz, q.z, __fmaf_rn(npy, q.y, __fmul_rn(npx, q.x)));
+    if (kClamp) x = fminf(fmaxf(x, -half_b), half_b - 0.25f);
+    const uint32_t bits = __float_as_uint(__fadd_rd(x, magic));
+    uint32_t addr = bits * 64u + k0;
+    addr ^= (bits << 3) & 0x30u;
+    red_shared_add(addr, inc);
+}
+
+// ions_s = shared-space byte address of the float4 ion records
+template <bool kClamp>
+__device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, float npx, float npy, float npz,
                                          float half_b, float magic, uint32_t k0, uint32_t inc)
 {
-    for (int ib = i0; ib < i1; ib += kIonBatch) {
+    int ib = i0;
+    for (; ib + kIonBatch <= i1; ib += kIonBatch) {          // full batches: loads first, then 8 independent chains
         float4 q[kIonBatch];
 #pragma unroll
-        for (int u = 0; u < kIonBatch; ++u) q[u] = ions[min(ib + u, i1 - 1)];
+        for (int u = 0; u < kIonBatch; ++u) q[u] = lds128(ions_s + (uint32_t)(ib + u) * 16u);
 #pragma unroll
-        for (int u = 0; u < kIonBatch; ++u) {
-            float x = __fmaf_rn(npz, q[u].z, __fmaf_rn(npy, q[u].y, __fmul_rn(npx, q[u].x)));
-            if (kClamp) x = fminf(fmaxf(x, -half_b), half_b - 0.25f);
-            uint32_t bits = __float_as_uint(__fadd_rd(x, magic));
-            uint32_t addr = bits * 64u + k0;
-            addr ^= (bits << 3) & 0x30u;
-            if (ib + u < i1) red_shared_add(addr, inc);
-        }
+        for (int u = 0; u < kIonBatch; ++u) bin_one<kClamp>(q[u], npx, npy, npz, half_b, magic, k0, inc);
     }
+    for (; ib < i1; ++ib) bin_one<kClamp>(lds128(ions_s + (uint32_t)ib * 16u), npx, npy, npz, half_b, magic, k0, inc);
 }
 
 __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParams p)
 {
     extern __shared__ unsigned char smem_raw[];
-    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned, still shared-space
     const MmaSmem L = mma_smem_layout(p.B, p.N, p.W, p.cap);
     __shared__ uint64_t s_bar[2];
     __shared__ uint32_t s_tmem;
@@ -214,8 +229,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
                 const int i0 = min(a1, a0 + warp * per), i1 = min(a1, i0 + per);
                 const uint32_t hb = smem_u32(smem + ((it & 1) ? L.hist1 : L.hist0));
                 const uint32_t k0 = hb + lane_off - 0x4B400000u * 64u;
-                if (p.clamp) bin_ions<true>(ions, i0, i1, npx, npy, npz, half_b, magic, k0, inc);
-                else bin_ions<false>(ions, i0, i1, npx, npy, npz, half_b, magic, k0, inc);
+                if (p.clamp) bin_ions<true>(smem_u32(ions), i0, i1, npx, npy, npz, half_b, magic, k0, inc);
+                else bin_ions<false>(smem_u32(ions), i0, i1, npx, npy, npz, half_b, magic, k0, inc);
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
             asm volatile("tcgen05.fence::before_thread_sync;");
@@ -248,7 +263,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
                     // ---- epilogue (steps a5-a7): TMEM -> phases -> sum over bin quarters -> arg-max ----
                     const int tau = warp & 3, half = warp >> 2;
                     const uint32_t acc = tmem + (uint32_t)((gp & 1) * p.N) + ((uint32_t)(tau * 32) << 16);
-                    for (int c = half; c < p.N / 16; c += 2) {
+                    for (int c = half; c < p.N / 16; c += kMmaWarps / 4) {
                         uint32_t v[16];
                         asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
                                      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),

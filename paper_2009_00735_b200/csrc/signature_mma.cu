@@ -23,14 +23,21 @@
 
 namespace apx {
 
-constexpr int kMmaThreads = 256;
-constexpr int kMmaWarps = kMmaThreads / 32;
+constexpr int kBinWarps = 12;            // project-and-bin warps
+constexpr int kMmaWarp = 4;              // tcgen05.mma issuer
+constexpr int kFirstBinWarp = 5;         // warps 0..3 = epilogue (one per TMEM lane quarter)
+constexpr int kMmaWarps = kFirstBinWarp + kBinWarps;
+constexpr int kMmaThreads = kMmaWarps * 32;
 constexpr int kIonBatch = 8;
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t cnt)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(cnt));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 {
@@ -165,7 +172,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned, still shared-space
     const MmaSmem L = mma_smem_layout(p.B, p.N, p.W, p.cap);
-    __shared__ uint64_t s_bar[2];
+    __shared__ uint64_t s_full[2], s_done[2], s_empty[2];
     __shared__ uint32_t s_tmem;
     __shared__ int s_n;
 
@@ -184,8 +191,11 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
 
     // ---- setup: barriers, TMEM, zero histograms, twiddle table, gather ------------------------------
     if (tid == 0) {
-        mbar_init(&s_bar[0], 1);
-        mbar_init(&s_bar[1], 1);
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(&s_full[i], kBinWarps);
+            mbar_init(&s_done[i], 1);
+            mbar_init(&s_empty[i], 4);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;");
         s_n = 0;
     }
@@ -212,58 +222,77 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
         // too many ions for the shared buffer: leave this material point to the FFT kernel
         if (chunk == 0 && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
     } else {
+        // Warp-specialised pipeline over items = (direction group, ion pass):
+        //   binning warps : wait empty[buf] -> project-and-bin the item into hist[buf] -> arrive full[buf]
+        //   MMA warp      : wait full[buf]  -> K/16 tcgen05.mma into acc[group&1] -> commit to done[buf]
+        //   epilogue warps: wait done[buf]  -> clear hist[buf]; on the last pass read TMEM, combine the four
+        //                    bin quarters, arg-max, store; arrive empty[buf]
         const int npass = n > 2048 ? (n + 2047) / 2048 : 1;          // fp16 counters are exact up to 2048
         const int nitems = (g_end - g_begin) * npass;
-        const float half_b = (float)(p.B / 2), magic = magic_for(p.B);
-        const uint32_t inc = (lane & 1) ? 65536u : 1u;
-        const uint32_t lane_off = (uint32_t)((lane >> 3) << 4) + (uint32_t)(((lane & 7) >> 1) << 2);
-        const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(p.N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-
-        for (int it = 0; it <= nitems; ++it) {
-            if (it < nitems) {
-                const int gi = g_begin + it / npass, pass = it % npass;
-                const int d = min(gi * 32 + lane, p.D - 1);
-                const float npx = p.dirs_scaled[3 * d], npy = p.dirs_scaled[3 * d + 1], npz = p.dirs_scaled[3 * d + 2];
+        if (warp >= kFirstBinWarp) {
+            const int bw = warp - kFirstBinWarp;
+            const float half_b = (float)(p.B / 2), magic = magic_for(p.B);
+            const uint32_t inc = (lane & 1) ? 65536u : 1u;
+            const uint32_t lane_off = (uint32_t)((lane >> 3) << 4) + (uint32_t)(((lane & 7) >> 1) << 2);
+            const uint32_t ions_s = smem_u32(ions);
+            int d = min(g_begin * 32 + lane, p.D - 1);
+            float npx = p.dirs_scaled[3 * d], npy = p.dirs_scaled[3 * d + 1], npz = p.dirs_scaled[3 * d + 2];
+            for (int it = 0; it < nitems; ++it) {
+                const int pass = it % npass;
+                // prefetch the next group's direction while this item is binned
+                float nx2 = npx, ny2 = npy, nz2 = npz;
+                if (pass == npass - 1 && it + 1 < nitems) {
+                    const int d2 = min((g_begin + (it + 1) / npass) * 32 + lane, p.D - 1);
+                    nx2 = p.dirs_scaled[3 * d2]; ny2 = p.dirs_scaled[3 * d2 + 1]; nz2 = p.dirs_scaled[3 * d2 + 2];
+                }
+                if (it >= 2) mbar_wait(&s_empty[it & 1], (uint32_t)(((it - 2) >> 1) & 1));
                 const int a0 = pass * 2048, a1 = min(n, a0 + 2048);
-                const int per = (a1 - a0 + kMmaWarps - 1) / kMmaWarps;
-                const int i0 = min(a1, a0 + warp * per), i1 = min(a1, i0 + per);
+                const int per = (a1 - a0 + kBinWarps - 1) / kBinWarps;
+                const int i0 = min(a1, a0 + bw * per), i1 = min(a1, i0 + per);
                 const uint32_t hb = smem_u32(smem + ((it & 1) ? L.hist1 : L.hist0));
                 const uint32_t k0 = hb + lane_off - 0x4B400000u * 64u;
-                if (p.clamp) bin_ions<true>(smem_u32(ions), i0, i1, npx, npy, npz, half_b, magic, k0, inc);
-                else bin_ions<false>(smem_u32(ions), i0, i1, npx, npy, npz, half_b, magic, k0, inc);
+                if (p.clamp) bin_ions<true>(ions_s, i0, i1, npx, npy, npz, half_b, magic, k0, inc);
+                else bin_ions<false>(ions_s, i0, i1, npx, npy, npz, half_b, magic, k0, inc);
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&s_full[it & 1]);
+                npx = nx2; npy = ny2; npz = nz2;
             }
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
-            asm volatile("tcgen05.fence::before_thread_sync;");
-            __syncthreads();
-            asm volatile("tcgen05.fence::after_thread_sync;");
-            if (it < nitems && tid == 0) {
+        } else if (warp == kMmaWarp) {
+            const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(p.N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+            const uint32_t tb = smem_u32(smem + L.table);
+            for (int it = 0; it < nitems; ++it) {
                 const int gi = g_begin + it / npass, pass = it % npass;
-                const uint32_t acc = tmem + (uint32_t)((gi & 1) * p.N);
-                const uint32_t ha = smem_u32(smem + ((it & 1) ? L.hist1 : L.hist0));
-                const uint32_t tb = smem_u32(smem + L.table);
-                for (int ks = 0; ks < K / 16; ++ks) {
-                    uint64_t ad = make_desc(ha + ks * 1024, (uint32_t)K * 64, 512, 4);
-                    uint64_t bd = make_desc(tb + (ks >> 2) * p.N * 128 + (ks & 3) * 32, 16, 1024, 2);
-                    mma_f16_ss(acc, ad, bd, idesc, (ks > 0 || pass > 0) ? 1u : 0u);
-                }
-                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
-                             ::"r"(smem_u32(&s_bar[it & 1])) : "memory");
-            }
-            if (it >= 1) {
-                const int prev = it - 1;
-                const int gp = g_begin + prev / npass;
-                const bool last_pass = (prev % npass) == npass - 1;
-                mbar_wait(&s_bar[prev & 1], (uint32_t)((prev >> 1) & 1));
+                mbar_wait(&s_full[it & 1], (uint32_t)((it >> 1) & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;");
-                {   // the transform of item `prev` has consumed its histogram: clear it for item prev+2
-                    uint4 *h = reinterpret_cast<uint4 *>(smem + ((prev & 1) ? L.hist1 : L.hist0));
-                    for (int i = tid; i < p.B * 4; i += kMmaThreads) h[i] = make_uint4(0, 0, 0, 0);
+                if (lane == 0) {
+                    const uint32_t acc = tmem + (uint32_t)((gi & 1) * p.N);
+                    const uint32_t ha = smem_u32(smem + ((it & 1) ? L.hist1 : L.hist0));
+                    for (int ks = 0; ks < K / 16; ++ks) {
+                        uint64_t ad = make_desc(ha + ks * 1024, (uint32_t)K * 64, 512, 4);
+                        uint64_t bd = make_desc(tb + (ks >> 2) * p.N * 128 + (ks & 3) * 32, 16, 1024, 2);
+                        mma_f16_ss(acc, ad, bd, idesc, (ks > 0 || pass > 0) ? 1u : 0u);
+                    }
+                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
+                                 ::"r"(smem_u32(&s_done[it & 1])) : "memory");
+                }
+                __syncwarp();
+            }
+        } else {
+            // ---- epilogue warps 0..3 (TMEM lane quarter = bin quarter tau = warp) -------------------------
+            const int tau = warp, et = tid;                               // et in [0,128)
+            for (int it = 0; it < nitems; ++it) {
+                const int gp = g_begin + it / npass;
+                const bool last_pass = (it % npass) == npass - 1;
+                mbar_wait(&s_done[it & 1], (uint32_t)((it >> 1) & 1));
+                asm volatile("tcgen05.fence::after_thread_sync;");
+                {   // the transform has consumed this histogram: clear it for item it+2
+                    uint4 *h = reinterpret_cast<uint4 *>(smem + ((it & 1) ? L.hist1 : L.hist0));
+                    for (int i = et; i < p.B * 4; i += 128) h[i] = make_uint4(0, 0, 0, 0);
                 }
                 if (last_pass) {
-                    // ---- epilogue (steps a5-a7): TMEM -> phases -> sum over bin quarters -> arg-max ----
-                    const int tau = warp & 3, half = warp >> 2;
                     const uint32_t acc = tmem + (uint32_t)((gp & 1) * p.N) + ((uint32_t)(tau * 32) << 16);
-                    for (int c = half; c < p.N / 16; c += kMmaWarps / 4) {
+                    for (int c = 0; c < p.N / 16; ++c) {
                         uint32_t v[16];
                         asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
                                      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
@@ -283,11 +312,17 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
                             }
                         }
                     }
-                    asm volatile("tcgen05.fence::before_thread_sync;");
-                    __syncthreads();
+                }
+                // histogram cleared and TMEM drained: hand the buffer (and accumulator) back
+                asm volatile("tcgen05.fence::before_thread_sync;");
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&s_empty[it & 1]);
+                if (last_pass) {
+                    asm volatile("bar.sync 1, 128;" ::: "memory");
                     float best = -1.0f;
                     int kbest = p.k_lo;
-                    for (int w = warp; w < p.W; w += kMmaWarps) {
+                    for (int w = warp; w < p.W; w += 4) {
                         float2 a = partial[(0 * p.W + w) * 32 + lane], b = partial[(1 * p.W + w) * 32 + lane];
                         float2 c2 = partial[(2 * p.W + w) * 32 + lane], d2 = partial[(3 * p.W + w) * 32 + lane];
                         float xr = (a.x + b.x) + (c2.x + d2.x), xi = (a.y + b.y) + (c2.y + d2.y);
@@ -295,12 +330,12 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
                         if (pw > best) { best = pw; kbest = p.k_lo + w; }
                     }
                     bestbuf[warp * 32 + lane] = make_float2(best, __int_as_float(kbest));
-                    __syncthreads();
+                    asm volatile("bar.sync 1, 128;" ::: "memory");
                     if (warp == 0) {
                         float bb = -1.0f;
                         int kb = p.k_lo;
 #pragma unroll
-                        for (int j = 0; j < kMmaWarps; ++j) {
+                        for (int j = 0; j < 4; ++j) {
                             float2 c = bestbuf[j * 32 + lane];
                             int ck = __float_as_int(c.y);
                             if (c.x > bb || (c.x == bb && ck < kb)) { bb = c.x; kb = ck; }
@@ -309,8 +344,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
                         if (dg < p.D)
                             p.sig[(size_t)m * p.D + dg] = make_float2(16777216.0f * sqrtf(fmaxf(bb, 0.0f)), (float)kb);
                     }
-                } else {
-                    __syncthreads();
                 }
             }
         }

@@ -34,14 +34,10 @@
 
 namespace apx {
 
-constexpr int kEpiWarps = 4;             // warps 0..3 = epilogue (one per TMEM lane quarter)
-constexpr int kMmaWarp = 4;              // tcgen05.mma issuer
-constexpr int kFirstBinWarp = 5;
-constexpr int kBinWarps = 12;            // project-and-bin warps (3 per scheduler)
-constexpr int kMmaWarps = kFirstBinWarp + kBinWarps;
+constexpr int kWorkWarps = 16;           // warps 0..15: project-and-bin, histogram clearing, epilogue
+constexpr int kWorkThreads = kWorkWarps * 32;
+constexpr int kMmaWarps = kWorkWarps + 1;  // warp 16 = tcgen05.mma issuer
 constexpr int kMmaThreads = kMmaWarps * 32;
-constexpr int kBinThreads = kBinWarps * 32;
-constexpr int kIonBatch = 8;
 constexpr int kRowGroupBytes = 1152;     // 8 M-chunks of 144 B: one (blk, kg) slab of 8 K rows x 64 directions
 constexpr int kChunkBytes = 144;         // SBO: 8 directions x 8 rows x 2 B + 16 B skew
 
@@ -86,11 +82,10 @@ __device__ __forceinline__ float4 lds128(uint32_t addr)
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
 }
-__device__ __forceinline__ void tmem_ld16(uint32_t addr, uint32_t (&v)[16])
+__device__ __forceinline__ void tmem_ld8(uint32_t addr, uint32_t (&v)[8])
 {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
                  : "r"(addr));
 }
 
@@ -113,7 +108,7 @@ struct MmaParams {
 
 // smem carve-up (bytes), shared by host and device
 struct MmaSmem {
-    uint32_t table, hist, exch, phase, ions, total;
+    uint32_t table, hist, exch, cand, phase, ions, total;
 };
 __host__ __device__ inline MmaSmem mma_smem_layout(int B, int N, int W, int cap)
 {
@@ -121,16 +116,17 @@ __host__ __device__ inline MmaSmem mma_smem_layout(int B, int N, int W, int cap)
     uint32_t off = 0;
     s.table = off; off += (uint32_t)(B / 4) * N * 2;             // (K/64) * N * 128 with K = B/4; multiple of 1024
     s.hist = off; off += (uint32_t)B * kChunkBytes;              // (B/8) row groups of 1152 B
-    s.exch = off; off += 64u * W * 8;
+    s.exch = off; off += 128u * N;                                // (N/8 chunks) x 2 blk x 64 slots x float2
+    s.cand = off; off += 8u * 64 * 8;
     s.phase = off; off += 4u * W * 8;
-    s.ions = off; off += (uint32_t)cap * 16;
+    s.ions = off; off += (uint32_t)cap * 12;
     s.total = off + 1024;                                          // slack for 1024-byte alignment
     return s;
 }
 
-// Gather (step a2) into float4 records (dx, dy, dz, -) for warp-broadcast LDS.128 reads.
-__device__ __forceinline__ void gather_roi4(const MmaParams &p, const GridParams &g, const RoiCells &rc,
-                                            float cx, float cy, float cz, float4 *ions, int *s_n)
+// Gather (step a2) into packed 12-byte records (dx, dy, dz): four ions = three LDS.128 for the binning warps.
+__device__ __forceinline__ void gather_roi3(const MmaParams &p, const GridParams &g, const RoiCells &rc,
+                                            float cx, float cy, float cz, float *ions, int *s_n)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int ny_r = rc.iy1 - rc.iy0 + 1, nz_r = rc.iz1 - rc.iz0 + 1;
@@ -151,7 +147,7 @@ __device__ __forceinline__ void gather_roi4(const MmaParams &p, const GridParams
                 int pos = 0;
                 if (lane == 0) pos = atomicAdd(s_n, __popc(msk));
                 pos = __shfl_sync(0xffffffffu, pos, 0) + __popc(msk & ((1u << lane) - 1u));
-                if (in && pos < p.cap) ions[pos] = make_float4(dx, dy, dz, 0.f);
+                if (in && pos < p.cap) { ions[3 * pos] = dx; ions[3 * pos + 1] = dy; ions[3 * pos + 2] = dz; }
             }
         }
     }
@@ -166,35 +162,125 @@ struct BinConst {
     uint32_t kz, k0;
 };
 template <bool kClamp>
-__device__ __forceinline__ void bin_one(const float4 q, float npx, float npy, float npz, const BinConst &c, uint32_t inc)
+__device__ __forceinline__ void bin_one(float dx, float dy, float dz, float npx, float npy, float npz, const BinConst &c,
+                                        uint32_t inc)
 {
-    float x = __fmaf_rn(npz, q.z, __fmaf_rn(npy, q.y, __fmul_rn(npx, q.x)));
+    float x = __fmaf_rn(npz, dz, __fmaf_rn(npy, dy, __fmul_rn(npx, dx)));
     if (kClamp) x = fminf(fmaxf(x, -c.half_b), c.half_b - 0.25f);
     const uint32_t ua = __float_as_uint(__fadd_rd(x, c.magic_a));
     const uint32_t va = __float_as_uint(__fmaf_rd(x, c.scl, c.magic_b));
     red_shared_add(ua * (uint32_t)kRowGroupBytes + (va * c.kz + c.k0), inc);
 }
+template <bool kClamp>
+__device__ __forceinline__ void bin_two(float dx, float dy, float dz, const float (&na)[3], const float (&nb)[3], const BinConst &c)
+{
+    bin_one<kClamp>(dx, dy, dz, na[0], na[1], na[2], c, 1u);            // set A: low u16 of the lane's word
+    bin_one<kClamp>(dx, dy, dz, nb[0], nb[1], nb[2], c, 65536u);        // set B: high u16
+}
 
-// ions_s = shared-space byte address of the float4 ion records; A = direction `lane`, B = direction `lane+32`
+// ions_s = shared-space byte address of the packed ion records; i0 is a multiple of 4
 template <bool kClamp>
 __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const float (&na)[3], const float (&nb)[3],
                                          const BinConst &c)
 {
     int ib = i0;
-    for (; ib + kIonBatch <= i1; ib += kIonBatch) {          // full batches: loads first, then 16 independent chains
-        float4 q[kIonBatch];
+    for (; ib + 8 <= i1; ib += 8) {                          // 8 ions = 6 LDS.128, then 16 independent chains
+        float4 q[6];
 #pragma unroll
-        for (int u = 0; u < kIonBatch; ++u) q[u] = lds128(ions_s + (uint32_t)(ib + u) * 16u);
+        for (int u = 0; u < 6; ++u) q[u] = lds128(ions_s + (uint32_t)ib * 12u + (uint32_t)u * 16u);
 #pragma unroll
-        for (int u = 0; u < kIonBatch; ++u) {
-            bin_one<kClamp>(q[u], na[0], na[1], na[2], c, 1u);
-            bin_one<kClamp>(q[u], nb[0], nb[1], nb[2], c, 65536u);
+        for (int h = 0; h < 2; ++h) {
+            const float4 a = q[3 * h], b = q[3 * h + 1], d = q[3 * h + 2];
+            bin_two<kClamp>(a.x, a.y, a.z, na, nb, c);
+            bin_two<kClamp>(a.w, b.x, b.y, na, nb, c);
+            bin_two<kClamp>(b.z, b.w, d.x, na, nb, c);
+            bin_two<kClamp>(d.y, d.z, d.w, na, nb, c);
         }
     }
+    if (ib + 4 <= i1) {
+        const float4 a = lds128(ions_s + (uint32_t)ib * 12u), b = lds128(ions_s + (uint32_t)ib * 12u + 16u),
+                     d = lds128(ions_s + (uint32_t)ib * 12u + 32u);
+        bin_two<kClamp>(a.x, a.y, a.z, na, nb, c);
+        bin_two<kClamp>(a.w, b.x, b.y, na, nb, c);
+        bin_two<kClamp>(b.z, b.w, d.x, na, nb, c);
+        bin_two<kClamp>(d.y, d.z, d.w, na, nb, c);
+        ib += 4;
+    }
     for (; ib < i1; ++ib) {
-        const float4 q = lds128(ions_s + (uint32_t)ib * 16u);
-        bin_one<kClamp>(q, na[0], na[1], na[2], c, 1u);
-        bin_one<kClamp>(q, nb[0], nb[1], nb[2], c, 65536u);
+        float dx, dy, dz;
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dx) : "r"(ions_s + (uint32_t)ib * 12u));
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dy) : "r"(ions_s + (uint32_t)ib * 12u + 4u));
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(ions_s + (uint32_t)ib * 12u + 8u));
+        bin_two<kClamp>(dx, dy, dz, na, nb, c);
+    }
+}
+
+// Epilogue of one direction group (steps a5 tail, a6, a7), run by all 16 worker warps while the tensor core
+// transforms the next group.  Worker warp w reads TMEM lane quarter q = w & 3 (M rows 32q..32q+31: blk = q >> 1,
+// direction slot from the lane) and the 8-column chunks c = j, j+4, ... (j = w >> 2; a chunk = 2 window bins).
+// A bin of the window is finished by the blk that matches its parity: the other blk hands its partial over
+// through `exch`.  Eight candidates per direction (2 blk x 4 j) are reduced by warps 0-1 and stored.
+__device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc_set, int gi, int64_t m, const float2 *phase,
+                                               float2 *exch, float2 *cand, int warp, int lane)
+{
+    const int q = warp & 3, j = warp >> 2, blk = q >> 1;
+    const int t = ((q & 1) << 5) + lane;
+    const uint32_t acc0 = acc_set + ((uint32_t)(q * 32) << 16);
+    const int nch = p.N >> 3;
+    float2 keep[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int c = j + 4 * u;
+        keep[u] = make_float2(0.f, 0.f);
+        if (c < nch) {
+            uint32_t v0[8], v1[8];
+            tmem_ld8(acc0 + (uint32_t)(c * 8), v0);
+            tmem_ld8(acc0 + (uint32_t)(p.N + c * 8), v1);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (int jj = 0; jj < 2; ++jj) {
+                const int w = 2 * c + jj;
+                if (w < p.W) {
+                    const float r0 = __uint_as_float(v0[4 * jj]) + __uint_as_float(v0[4 * jj + 2]) * (1.0f / 2048.0f);
+                    const float i0 = -(__uint_as_float(v0[4 * jj + 1]) + __uint_as_float(v0[4 * jj + 3]) * (1.0f / 2048.0f));
+                    const float r1 = __uint_as_float(v1[4 * jj]) + __uint_as_float(v1[4 * jj + 2]) * (1.0f / 2048.0f);
+                    const float i1 = -(__uint_as_float(v1[4 * jj + 1]) + __uint_as_float(v1[4 * jj + 3]) * (1.0f / 2048.0f));
+                    const float2 f0 = phase[blk * p.W + w], f1 = phase[(2 + blk) * p.W + w];
+                    const float xr = (f0.x * r0 - f0.y * i0) + (f1.x * r1 - f1.y * i1);
+                    const float xi = (f0.x * i0 + f0.y * r0) + (f1.x * i1 + f1.y * r1);
+                    if (jj == blk) keep[u] = make_float2(xr, xi);
+                    else exch[(c * 2 + blk) * 64 + t] = make_float2(xr, xi);
+                }
+            }
+        }
+    }
+    asm volatile("bar.sync 1, %0;" ::"n"(kWorkThreads) : "memory");
+    float best = -1.0f;
+    int kbest = p.k_lo;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int c = j + 4 * u, w = 2 * c + blk;
+        if (c < nch && w < p.W) {
+            const float2 o = exch[(c * 2 + (1 - blk)) * 64 + t];
+            const float xr = keep[u].x + o.x, xi = keep[u].y + o.y;
+            const float pw = xr * xr + xi * xi;
+            if (pw > best) { best = pw; kbest = p.k_lo + w; }            // ascending w: lowest k kept on ties
+        }
+    }
+    cand[(blk * 4 + j) * 64 + t] = make_float2(best, __int_as_float(kbest));
+    asm volatile("bar.sync 1, %0;" ::"n"(kWorkThreads) : "memory");
+    if (warp < 2) {
+        float bb = -1.0f;
+        int kb = p.k_lo;
+#pragma unroll
+        for (int s = 0; s < 8; ++s) {
+            const float2 c2 = cand[s * 64 + t];
+            const int ck = __float_as_int(c2.y);
+            if (c2.x > bb || (c2.x == bb && ck < kb)) { bb = c2.x; kb = ck; }
+        }
+        const int slot = ((lane & 1) << 5) + ((warp & 1) << 4) + ((lane >> 3) << 2) + ((lane & 7) >> 1);
+        const int d = p.perm[gi * 64 + slot];
+        if (d >= 0) p.sig[(size_t)m * p.D + d] = make_float2(16777216.0f * sqrtf(fmaxf(bb, 0.0f)), (float)kb);
     }
 }
 
@@ -203,7 +289,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned, still shared-space
     const MmaSmem L = mma_smem_layout(p.B, p.N, p.W, p.cap);
-    __shared__ uint64_t s_full, s_done, s_tfree;
+    __shared__ uint64_t s_full, s_done;
     __shared__ uint32_t s_tmem;
     __shared__ int s_n;
 
@@ -215,17 +301,17 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     const GridParams g = *p.grid;
     const float cx = p.centres[3 * m], cy = p.centres[3 * m + 1], cz = p.centres[3 * m + 2];
     const RoiCells rc = roi_cells(g, cx, cy, cz, p.R);
-    float4 *ions = reinterpret_cast<float4 *>(smem + L.ions);
+    float *ions = reinterpret_cast<float *>(smem + L.ions);
     float2 *exch = reinterpret_cast<float2 *>(smem + L.exch);
+    float2 *cand = reinterpret_cast<float2 *>(smem + L.cand);
     float2 *phase = reinterpret_cast<float2 *>(smem + L.phase);
     const int K = p.B / 4;
     const uint32_t hist_bytes = (uint32_t)p.B * kChunkBytes;
 
     // ---- setup: barriers, TMEM, zero histogram, twiddle table, gather ------------------------------
     if (tid == 0) {
-        mbar_init(&s_full, kBinWarps);
+        mbar_init(&s_full, kWorkWarps);
         mbar_init(&s_done, 1);
-        mbar_init(&s_tfree, kEpiWarps);
         asm volatile("fence.mbarrier_init.release.cluster;");
         s_n = 0;
     }
@@ -245,7 +331,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;");
     const uint32_t tmem = s_tmem;
-    if (g.n_accepted) gather_roi4(p, g, rc, cx, cy, cz, ions, &s_n);
+    if (g.n_accepted) gather_roi3(p, g, rc, cx, cy, cz, ions, &s_n);
     __syncthreads();
     const int n = s_n;
     if (chunk == 0 && tid == 0 && p.counts) p.counts[m] = (uint32_t)n;
@@ -254,15 +340,13 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
         // too many ions for the shared buffer: leave this material point to the FFT kernel
         if (chunk == 0 && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
     } else {
-        // Warp-specialised pipeline over items = (direction group, ion pass), one histogram buffer:
-        //   binning warps : wait done[it-1] -> clear the histogram -> project-and-bin item it -> arrive full
-        //   MMA warp      : wait full, tfree[it-1] -> 2 x K/16 tcgen05.mma into the two accumulators -> commit to done
-        //   epilogue warps: wait done[it]; on the last pass read TMEM, recombine the four (pair, blk) parts,
-        //                    arg-max, store; arrive tfree
+        // Pipeline over items = (direction group, ion pass); one histogram buffer, two TMEM accumulator sets.
+        //   worker warps 0..15 : [wait done(it-1) -> clear the histogram] -> project-and-bin item it -> arrive full(it)
+        //                        -> epilogue of the previous group (its accumulators are in the other TMEM set)
+        //   MMA warp 16        : wait full(it) -> 2 x K/16 tcgen05.mma into set (group & 1) -> commit to done(it)
         const int npass = n > 2048 ? (n + 2047) / 2048 : 1;          // fp16 counters are exact up to 2048
         const int nitems = (g_end - g_begin) * npass;
-        if (warp >= kFirstBinWarp) {
-            const int bw = warp - kFirstBinWarp, bt = tid - kFirstBinWarp * 32;
+        if (warp < kWorkWarps) {
             BinConst c;
             c.half_b = (float)(p.B / 2); c.magic_a = magic_for(p.B); c.magic_b = 12582912.0f + 4.0f;
             c.scl = __int_as_float((127 - p.nl) << 23);                       // 2^-nl
@@ -271,105 +355,72 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
                    - 0x4B400000u * (uint32_t)kRowGroupBytes - 0x4B400000u * c.kz;
             const uint32_t ions_s = smem_u32(ions);
             for (int it = 0; it < nitems; ++it) {
-                const int gi = g_begin + it / npass, pass = it % npass;
+                const int gl = it / npass, pass = it % npass;
                 float na[3], nb[3];
                 {
-                    const float *da = p.dirs_sorted + (size_t)(gi * 64 + lane) * 3;
+                    const float *da = p.dirs_sorted + (size_t)((g_begin + gl) * 64 + lane) * 3;
                     na[0] = da[0]; na[1] = da[1]; na[2] = da[2];
                     nb[0] = da[96]; nb[1] = da[97]; nb[2] = da[98];
                 }
                 if (it > 0) {
                     mbar_wait(&s_done, (uint32_t)((it - 1) & 1));     // the transform has consumed the histogram
+                    asm volatile("tcgen05.fence::after_thread_sync;");
                     uint4 *h = reinterpret_cast<uint4 *>(smem + L.hist);
-                    for (int i = bt; i < (int)(hist_bytes / 16); i += kBinThreads) h[i] = make_uint4(0, 0, 0, 0);
-                    asm volatile("bar.sync 2, %0;" ::"n"(kBinThreads) : "memory");
+                    for (int i = tid; i < (int)(hist_bytes / 16); i += kWorkThreads) h[i] = make_uint4(0, 0, 0, 0);
+                    asm volatile("bar.sync 2, %0;" ::"n"(kWorkThreads) : "memory");
                 }
                 const int a0 = pass * 2048, a1 = min(n, a0 + 2048);
-                const int per = (a1 - a0 + kBinWarps - 1) / kBinWarps;
-                const int i0 = min(a1, a0 + bw * per), i1 = min(a1, i0 + per);
+                const int per = (((a1 - a0 + kWorkWarps - 1) / kWorkWarps) + 3) & ~3;
+                const int i0 = min(a1, a0 + warp * per), i1 = min(a1, i0 + per);
                 if (p.clamp) bin_ions<true>(ions_s, i0, i1, na, nb, c);
                 else bin_ions<false>(ions_s, i0, i1, na, nb, c);
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
+                asm volatile("tcgen05.fence::before_thread_sync;");              // earlier TMEM reads -> next MMA
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&s_full);
+                if (it > 0 && pass == 0)                                         // item it-1 closed group gl-1
+                    epilogue_group(p, tmem + (uint32_t)(((gl - 1) & 1) * 2 * p.N), g_begin + gl - 1, m, phase, exch, cand, warp, lane);
             }
-        } else if (warp == kMmaWarp) {
-            const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(p.N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-            const uint32_t tb = smem_u32(smem + L.table), hb = smem_u32(smem + L.hist);
-            const uint32_t pair_off = (uint32_t)kRowGroupBytes * (uint32_t)(p.B / 16);
-            for (int it = 0; it < nitems; ++it) {
-                const int pass = it % npass;
-                mbar_wait(&s_full, (uint32_t)(it & 1));
-                if (it > 0) mbar_wait(&s_tfree, (uint32_t)((it - 1) & 1));
+            if (nitems > 0) {
+                const int gl = (nitems - 1) / npass;
+                mbar_wait(&s_done, (uint32_t)((nitems - 1) & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;");
-                if (lane == 0) {
-                    for (int pr = 0; pr < 2; ++pr)
-                        for (int ks = 0; ks < K / 16; ++ks) {
-                            uint64_t ad = make_desc(hb + pr * pair_off + ks * (4 * kRowGroupBytes), 2 * kRowGroupBytes, kChunkBytes, 0);
-                            uint64_t bd = make_desc(tb + (ks >> 2) * p.N * 128 + (ks & 3) * 32, 16, 1024, 2);
-                            mma_f16_ss(tmem + (uint32_t)(pr * p.N), ad, bd, idesc, (ks > 0 || pass > 0) ? 1u : 0u);
-                        }
-                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
-                                 ::"r"(smem_u32(&s_done)) : "memory");
-                }
-                __syncwarp();
+                epilogue_group(p, tmem + (uint32_t)((gl & 1) * 2 * p.N), g_begin + gl, m, phase, exch, cand, warp, lane);
             }
         } else {
-            // ---- epilogue warps 0..3: TMEM lane = 32*warp + lane = M row blk*64 + slot --------------------
-            const int blk = warp >> 1;
-            const int et = (warp & 1) * 32 + lane;                                    // thread index among the 64 of this blk
-            const int slot = ((lane & 1) << 5) + ((warp & 1) << 4) + ((lane >> 3) << 2) + ((lane & 7) >> 1);
-            const uint32_t acc0 = tmem + ((uint32_t)(warp * 32) << 16);
+            // ---- MMA warp: descriptors advance by adding to the 14-bit start-address field ---------------
+            const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(p.N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+            const uint32_t tb = smem_u32(smem + L.table), hb = smem_u32(smem + L.hist);
+            const uint32_t a_hi = (uint32_t)(kChunkBytes >> 4) | (1u << 14);                              // SBO, version 1, INTERLEAVE
+            const uint32_t a_lo0 = ((hb >> 4) & 0x3FFFu) | ((uint32_t)((2 * kRowGroupBytes) >> 4) << 16);   // LBO = 2304 B
+            const uint32_t b_hi = (uint32_t)(1024 >> 4) | (1u << 14) | (2u << 29);                          // SBO, version 1, SWIZZLE_128B
+            const uint32_t b_lo0 = ((tb >> 4) & 0x3FFFu) | (1u << 16);
+            const uint32_t pair_step = ((uint32_t)kRowGroupBytes * (uint32_t)(p.B / 16)) >> 4;
+            const uint32_t kblk_step = (uint32_t)(p.N * 128) >> 4;
             for (int it = 0; it < nitems; ++it) {
-                const int gi = g_begin + it / npass;
-                const bool last_pass = (it % npass) == npass - 1;
-                mbar_wait(&s_done, (uint32_t)(it & 1));
+                const int gl = it / npass, pass = it % npass;
+                mbar_wait(&s_full, (uint32_t)(it & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;");
-                if (last_pass && blk == 0) asm volatile("bar.sync 1, 128;" ::: "memory");     // partner's partials are in exch
-                float best = -1.0f;
-                int kbest = p.k_lo;
-                if (last_pass) {
+                const uint32_t acc = tmem + (uint32_t)((gl & 1) * 2 * p.N);
 #pragma unroll 1
-                    for (int c = 0; c < p.N / 16; ++c) {
-                        uint32_t v0[16], v1[16];
-                        tmem_ld16(acc0 + (uint32_t)(c * 16), v0);
-                        tmem_ld16(acc0 + (uint32_t)(p.N + c * 16), v1);
-                        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                for (int pr = 0; pr < 2; ++pr) {
+                    uint32_t a_lo = a_lo0 + (uint32_t)pr * pair_step, b_lo = b_lo0;
+#pragma unroll 1
+                    for (int kb = 0; kb < K / 64; ++kb) {
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const int w = c * 4 + j;
-                            if (w < p.W) {
-                                const float r0 = __uint_as_float(v0[4 * j]) + __uint_as_float(v0[4 * j + 2]) * (1.0f / 2048.0f);
-                                const float i0 = -(__uint_as_float(v0[4 * j + 1]) + __uint_as_float(v0[4 * j + 3]) * (1.0f / 2048.0f));
-                                const float r1 = __uint_as_float(v1[4 * j]) + __uint_as_float(v1[4 * j + 2]) * (1.0f / 2048.0f);
-                                const float i1 = -(__uint_as_float(v1[4 * j + 1]) + __uint_as_float(v1[4 * j + 3]) * (1.0f / 2048.0f));
-                                const float2 f0 = phase[blk * p.W + w], f1 = phase[(2 + blk) * p.W + w];
-                                float xr = (f0.x * r0 - f0.y * i0) + (f1.x * r1 - f1.y * i1);
-                                float xi = (f0.x * i0 + f0.y * r0) + (f1.x * i1 + f1.y * r1);
-                                if (blk == 1) {
-                                    exch[w * 64 + et] = make_float2(xr, xi);
-                                } else {
-                                    const float2 o = exch[w * 64 + et];
-                                    xr += o.x; xi += o.y;
-                                    const float pw = xr * xr + xi * xi;
-                                    if (pw > best) { best = pw; kbest = p.k_lo + w; }    // ascending w: lowest k kept on ties
-                                }
-                            }
+                        for (int kk = 0; kk < 4; ++kk) {
+                            const uint64_t ad = ((uint64_t)a_hi << 32) | (a_lo + (uint32_t)kk * ((4 * kRowGroupBytes) >> 4));
+                            const uint64_t bd = ((uint64_t)b_hi << 32) | (b_lo + (uint32_t)kk * 2u);
+                            if (lane == 0) mma_f16_ss(acc + (uint32_t)(pr * p.N), ad, bd, idesc, (kb > 0 || kk > 0 || pass > 0) ? 1u : 0u);
                         }
+                        a_lo += 4u * ((4 * kRowGroupBytes) >> 4);
+                        b_lo += kblk_step;
                     }
                 }
-                // TMEM drained: the MMA warp may overwrite the accumulators
-                asm volatile("tcgen05.fence::before_thread_sync;");
+                if (lane == 0)
+                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
+                                 ::"r"(smem_u32(&s_done)) : "memory");
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&s_tfree);
-                if (last_pass) {
-                    if (blk == 1) {
-                        asm volatile("bar.sync 1, 128;" ::: "memory");
-                    } else {
-                        const int d = p.perm[gi * 64 + slot];
-                        if (d >= 0) p.sig[(size_t)m * p.D + d] = make_float2(16777216.0f * sqrtf(fmaxf(best, 0.0f)), (float)kbest);
-                    }
-                }
             }
         }
     }
@@ -385,7 +436,7 @@ static int mma_cap_for(int B, int N, int W)
 {
     const int budget = 232448 - 512;   // 227 KB opt-in shared memory per CTA on sm_100, minus static shared
     MmaSmem s = mma_smem_layout(B, N, W, 0);
-    int cap = ((budget - (int)s.total) / 16) & ~63;
+    int cap = ((budget - (int)s.total) / 12) & ~63;
     return cap > 4096 ? 4096 : cap;
 }
 
@@ -393,7 +444,7 @@ bool mma_path_supported(const Plan *p)
 {
     if (p->B > 1024) return false;                       // B = 2048, 4096 stay on the FFT kernel
     const int N = mma_n_for(p->W);
-    if (2 * N > 512) return false;                       // two accumulators of N TMEM columns
+    if (4 * N > 512) return false;                       // two sets of two accumulators of N TMEM columns
     return mma_cap_for(p->B, N, p->W) >= 1024;           // room for a useful ion buffer
 }
 
@@ -528,7 +579,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.nchunks = nchunks;
     q.clamp = p->mma_clamp;
     uint32_t cols = 32;
-    while (cols < (uint32_t)(2 * q.N)) cols *= 2;
+    while (cols < (uint32_t)(4 * q.N)) cols *= 2;
     q.tmem_cols = cols;
     q.R = p->R; q.R2 = p->R2;
     const MmaSmem L = mma_smem_layout(p->B, q.N, p->W, q.cap);

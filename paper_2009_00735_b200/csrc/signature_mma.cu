@@ -72,6 +72,11 @@ __device__ __forceinline__ void mma_f16_ss(uint32_t d_tmem, uint64_t adesc, uint
     asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}"
                  ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
 }
+__device__ __forceinline__ void mma_f16_acc(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc)
+{
+    asm volatile("{\n .reg .pred p;\n setp.eq.b32 p, 0, 0;\n tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}"
+                 ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc) : "memory");
+}
 __device__ __forceinline__ void red_shared_add(uint32_t addr, uint32_t v)
 {
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
@@ -284,12 +289,13 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc_
     }
 }
 
+template <int KS>   // KS = K/16 = B/64 k-steps per accumulator
 __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParams p)
 {
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned, still shared-space
     const MmaSmem L = mma_smem_layout(p.B, p.N, p.W, p.cap);
-    __shared__ uint64_t s_full, s_done;
+    __shared__ uint64_t s_full, s_done[2];   // s_done[h]: the MMAs reading histogram half h (= pair h) have completed
     __shared__ uint32_t s_tmem;
     __shared__ int s_n;
 
@@ -305,13 +311,14 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     float2 *exch = reinterpret_cast<float2 *>(smem + L.exch);
     float2 *cand = reinterpret_cast<float2 *>(smem + L.cand);
     float2 *phase = reinterpret_cast<float2 *>(smem + L.phase);
-    const int K = p.B / 4;
+    constexpr int K = KS * 16;
     const uint32_t hist_bytes = (uint32_t)p.B * kChunkBytes;
 
     // ---- setup: barriers, TMEM, zero histogram, twiddle table, gather ------------------------------
     if (tid == 0) {
         mbar_init(&s_full, kWorkWarps);
-        mbar_init(&s_done, 1);
+        mbar_init(&s_done[0], 1);
+        mbar_init(&s_done[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;");
         s_n = 0;
     }
@@ -363,10 +370,15 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
                     nb[0] = da[96]; nb[1] = da[97]; nb[2] = da[98];
                 }
                 if (it > 0) {
-                    mbar_wait(&s_done, (uint32_t)((it - 1) & 1));     // the transform has consumed the histogram
-                    asm volatile("tcgen05.fence::after_thread_sync;");
+                    // clear each histogram half as soon as the MMAs that read it have completed
                     uint4 *h = reinterpret_cast<uint4 *>(smem + L.hist);
-                    for (int i = tid; i < (int)(hist_bytes / 16); i += kWorkThreads) h[i] = make_uint4(0, 0, 0, 0);
+                    const int half16 = (int)(hist_bytes / 32);
+#pragma unroll
+                    for (int hh = 0; hh < 2; ++hh) {
+                        mbar_wait(&s_done[hh], (uint32_t)((it - 1) & 1));
+                        for (int i = tid; i < half16; i += kWorkThreads) h[hh * half16 + i] = make_uint4(0, 0, 0, 0);
+                    }
+                    asm volatile("tcgen05.fence::after_thread_sync;");
                     asm volatile("bar.sync 2, %0;" ::"n"(kWorkThreads) : "memory");
                 }
                 const int a0 = pass * 2048, a1 = min(n, a0 + 2048);
@@ -383,7 +395,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
             }
             if (nitems > 0) {
                 const int gl = (nitems - 1) / npass;
-                mbar_wait(&s_done, (uint32_t)((nitems - 1) & 1));
+                mbar_wait(&s_done[1], (uint32_t)((nitems - 1) & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;");
                 epilogue_group(p, tmem + (uint32_t)((gl & 1) * 2 * p.N), g_begin + gl, m, phase, exch, cand, warp, lane);
             }
@@ -402,24 +414,20 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
                 mbar_wait(&s_full, (uint32_t)(it & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;");
                 const uint32_t acc = tmem + (uint32_t)((gl & 1) * 2 * p.N);
-#pragma unroll 1
-                for (int pr = 0; pr < 2; ++pr) {
-                    uint32_t a_lo = a_lo0 + (uint32_t)pr * pair_step, b_lo = b_lo0;
-#pragma unroll 1
-                    for (int kb = 0; kb < K / 64; ++kb) {
+                if (lane == 0) {
 #pragma unroll
-                        for (int kk = 0; kk < 4; ++kk) {
-                            const uint64_t ad = ((uint64_t)a_hi << 32) | (a_lo + (uint32_t)kk * ((4 * kRowGroupBytes) >> 4));
-                            const uint64_t bd = ((uint64_t)b_hi << 32) | (b_lo + (uint32_t)kk * 2u);
-                            if (lane == 0) mma_f16_ss(acc + (uint32_t)(pr * p.N), ad, bd, idesc, (kb > 0 || kk > 0 || pass > 0) ? 1u : 0u);
+                    for (int pr = 0; pr < 2; ++pr) {
+#pragma unroll
+                        for (int ks = 0; ks < KS; ++ks) {
+                            const uint64_t ad = ((uint64_t)a_hi << 32) | (a_lo0 + (uint32_t)pr * pair_step + (uint32_t)ks * ((4 * kRowGroupBytes) >> 4));
+                            const uint64_t bd = ((uint64_t)b_hi << 32) | (b_lo0 + (uint32_t)(ks >> 2) * kblk_step + (uint32_t)(ks & 3) * 2u);
+                            if (ks == 0) mma_f16_ss(acc + (uint32_t)(pr * p.N), ad, bd, idesc, pass > 0 ? 1u : 0u);
+                            else mma_f16_acc(acc + (uint32_t)(pr * p.N), ad, bd, idesc);
                         }
-                        a_lo += 4u * ((4 * kRowGroupBytes) >> 4);
-                        b_lo += kblk_step;
+                        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
+                                     ::"r"(smem_u32(&s_done[pr])) : "memory");
                     }
                 }
-                if (lane == 0)
-                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
-                                 ::"r"(smem_u32(&s_done)) : "memory");
                 __syncwarp();
             }
         }
@@ -583,11 +591,18 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.tmem_cols = cols;
     q.R = p->R; q.R2 = p->R2;
     const MmaSmem L = mma_smem_layout(p->B, q.N, p->W, q.cap);
-    e = cudaFuncSetAttribute(k_signature_mma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total);
-    if (e != cudaSuccess) return e;
     const int64_t blocks = M * nchunks;
     if (blocks > 0x7FFFFFFFLL) return cudaErrorInvalidConfiguration;
-    k_signature_mma<<<(unsigned)blocks, kMmaThreads, L.total, st>>>(q);
+    auto launch = [&](auto kern) -> cudaError_t {
+        cudaError_t le = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total);
+        if (le != cudaSuccess) return le;
+        kern<<<(unsigned)blocks, kMmaThreads, L.total, st>>>(q);
+        return cudaSuccess;
+    };
+    if (p->B == 1024) e = launch(k_signature_mma<16>);
+    else if (p->B == 512) e = launch(k_signature_mma<8>);
+    else e = launch(k_signature_mma<4>);
+    if (e != cudaSuccess) return e;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     return launch_signature_fft_list(p, centres, p->d_deferred, sig, counts, st);

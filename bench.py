@@ -30,10 +30,23 @@ UNIT = "histograms/s"
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 
 
-def algorithmic_flops(n_pairs, n_hist, B):
-    """6 flop per (ion, direction) pair (FMUL + 2 FFMA + round-down FADD) and the unpruned real
-    FFT's 2.5 B log2 B flop per histogram."""
-    return 6.0 * n_pairs + 2.5 * B * np.log2(B) * n_hist
+# issue-slot peak: 148 SMs x 4 schedulers x 32 lanes x 1.965 GHz thread-instructions/s
+ISSUE_PEAK_TINST = 148 * 4 * 32 * 1.965e9
+PAIR_FLOP = 6.0          # FMUL + 2 FFMA + round-down FADD of Eq. 1's projection and floor, per (ion, direction) pair
+PAIR_SLOTS_MMA = 8.0     # + FFMA.RD (hi3) + 2 IMAD (address) + 1 shared atomic: issue slots per pair, MMA kernel
+# traffic (dram__bytes_read.sum + dram__bytes_write.sum per launch) of the dominant kernel from the committed
+# ncu --set full capture (profiles/), config 2; None for a kernel/config that was not captured
+NCU_TRAFFIC = {"k_signature_mma": 25.9e6, "k_signature_fft": None}
+
+
+def algorithmic_flops(n_pairs, n_hist, B, path):
+    """the FP32-pipe work that the method itself prescribes.  Project-and-bin: 6 flop per
+    (ion, direction) pair.  DFT: on the MMA path it runs on the tensor pipe and is NOT counted against the FP32
+    peak; on the FFT path the unpruned real FFT's 2.5 B log2 B flop per histogram is added."""
+    f = PAIR_FLOP * n_pairs
+    if path == "fft":
+        f += 2.5 * B * np.log2(B) * n_hist
+    return f
 
 
 class ClockSampler:
@@ -219,9 +232,13 @@ def run_ours(args, rank, world, local_rank):
     n_hist = M * D * world
     value = n_hist * args.steps / (ms * 1e-3)
     pairs = float(n_c.sum()) * D
-    flops = algorithmic_flops(pairs, M * D, B)
+    path = "mma" if plan.apx_plan_path() == 1 else "fft"
+    kname = "k_signature_mma" if path == "mma" else "k_signature_fft"
+    flops = algorithmic_flops(pairs, M * D, B, path)
     q_s = ms_query * 1e-3 / args.steps
     achieved = flops / q_s / 1e12
+    W = w.window[1] - w.window[0] + 1
+    tensor_flops = 2.0 * 64 * ((4 * W + 15) // 16 * 16) * B * ((D + 63) // 64) * M if path == "mma" else 0.0
     h2d = w.xyz.nbytes + w.types.nbytes + centres_np.nbytes
     d2h = M * D * 8 + M * 4
     out = {
@@ -238,18 +255,28 @@ def run_ours(args, rank, world, local_rank):
         "clocks": clocks,
         "e2e": {"value": n_hist * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "entry": "apx_run_host", "steps": e2e_steps},
-        "gpu_launches": 8 * args.steps,
-        "roofline": {"bound": "alu", "kernel": "k_signature_mma" if plan.apx_plan_path() == 1 else "k_signature_fft",
+        # 7 ingest kernels (k_reset, k_bounds, k_grid_params, k_zero_cells, k_count, k_scan, k_scatter)
+        # + k_signature_mma + k_signature_fft over the deferred list (or k_signature_fft alone) per step
+        "gpu_launches": (9 if path == "mma" else 8) * args.steps,
+        "roofline": {"bound": "alu", "kernel": kname,
                      "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                     "frac": achieved / FP32_PEAK_TFLOPS, "traffic": None,
-                     "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md)",
+                     "frac": achieved / FP32_PEAK_TFLOPS, "traffic": NCU_TRAFFIC.get(kname),
+                     "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md); "
+                                    "MEASURED_PEAKS.json has no FP32 figure",
                      "ms_per_launch": ms_query / args.steps,
-                     "model": "6 flop/(ion,direction) pair + 2.5 B log2 B flop/histogram"},
+                     "model": "6 flop per (ion,direction) pair" + ("" if path == "mma" else " + 2.5 B log2 B flop per histogram"),
+                     "pairs_per_launch": pairs,
+                     "issue_slot_frac": (PAIR_SLOTS_MMA * pairs / q_s / ISSUE_PEAK_TINST) if path == "mma" else None,
+                     "tensor_tflops": tensor_flops / q_s / 1e12 if path == "mma" else None},
     }
     if not args.no_cpu_baseline:
-        dt, nh, cores = oracle_sample(w, np.ascontiguousarray(dirs), 32)
+        # bounded sample: batches of 64 material points until >= 10 s of CPU work
+        dt, nh, cores, npts = 0.0, 0, 1, 0
+        while dt < 10.0 and npts < M:
+            d1, n1, cores = oracle_sample(w, np.ascontiguousarray(dirs), 64)
+            dt += d1; nh += n1; npts += 64
         out["cpu_baseline"] = {"value": nh / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-                               "sample": f"32 of {M} material points x {D} directions, {dt:.1f} s",
+                               "sample": f"{npts} of {M} material points x {D} directions, {dt:.1f} s",
                                "paper_context": "0.72 material points/s on 1 Xeon Gold 6138 core (PAPER.md L248)"}
     print(json.dumps(out))
     if dist is not None:

@@ -8,5 +8,7 @@ from .binding import (Plan, ApxError, apx_dirs_fibonacci, apx_dirs_geodesic, apx
                       APX_FLAG_FORCE_FFT, APX_FLAG_FORCE_MMA, APX_OK, APX_EINVAL, APX_ENOMEM, APX_ECUDA,
                       APX_ESTATE, APX_ERANGE)
 
-__all__ = ["Plan", "ApxError", "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_version", "EXPORTS", "LIB_PATH",
+from .parallel import shard_range, run_sharded, gather_counts
+
+__all__ = ["shard_range", "run_sharded", "gather_counts", "Plan", "ApxError", "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_version", "EXPORTS", "LIB_PATH",
            "APX_FLAG_FORCE_FFT", "APX_FLAG_FORCE_MMA"]

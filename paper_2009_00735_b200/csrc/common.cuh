@@ -33,10 +33,11 @@ struct Plan {
     float *d_dirs_scaled;          // [D][3]  n' = fl32(n*s)
     float2 *d_twiddle;             // [B/2]   exp(-2 pi i r / B), r < B/2   (FFT path)
     void *d_mma_table;             // twiddle operand of the windowed DFT (MMA path)
+    void *d_mma_zero;              // zeros, source of the bulk copies that clear a histogram buffer (MMA path)
     float2 *d_mma_phase;           // [4][W] recombination phases of the four bin parts (MMA path)
     float *d_dirs_sorted;          // [Dp][3] scaled directions in patch order (MMA path)
     int *d_dir_perm;               // [Dp] original index of each sorted slot, -1 = padding
-    int Dp;                        // D rounded up to a multiple of 64
+    int Dp;                        // D rounded up to a multiple of 32
     int mma_clamp;                 // 1 = the bin clamp of Eq. 1 must stay in the MMA kernel's inner loop
     uint32_t *d_deferred;          // [0] count, [1..] material points the MMA kernel left to the FFT kernel
     int64_t cap_deferred;

@@ -1,30 +1,29 @@
 // signature_mma.cu -- windowed-DFT signature kernel: shared-memory histograms feed the tcgen05 tensor
 // cores directly (steps a2, a4-a7 for narrow spectral windows, B <= 1024).
 //
-// Per CTA: one material point x a chunk of direction groups; a group = 64 directions.
-//   binning  : every lane of a binning warp owns ONE 32-bit word per histogram row: two u16 counters, the
-//              low half for direction `lane` (set A) and the high half for direction `lane + 32` (set B) of
-//              the group (Eq. 1).  A row of the histogram is 32 words, so within one shared
-//              atomic the 32 lanes hit 32 different banks whenever their bins agree in the top three bits
-//              (hi3); the plan sorts the directions into spatially compact patches of 32 so that they
-//              almost always do.  The u16 bit pattern c is the fp16 number c * 2^-24 (subnormal / first
-//              binade, exact for c <= 2048), so the histogram IS a valid fp16 tensor-core operand and is
-//              never converted or copied.
-//   layout   : byte address of (bin b, lane L) = (L/4)*144 + (L%4)*4 + 16*hi3 + 1152*low,
-//              hi3 = b >> (log2 B - 3), low = b & (B/8 - 1).  Read as an MN-major INTERLEAVE (no swizzle)
-//              operand with SBO = 144 B (between 8-element M chunks) and LBO = 2304 B (between 8-row K
-//              groups) this is a [128 x K] tile: M row = blk*64 + direction slot (blk = bit 0 of low),
-//              K index = kg*8 + hi3 (kg = the middle bits of low); the top bit of low selects one of two
-//              accumulators ("pair").  K = B/4 per accumulator.
+// Per CTA: one material point x a chunk of direction groups; a group = 32 directions.
+//   binning  : lane l (0..15) of a half-warp owns ONE 32-bit word per histogram row: two u16 counters, the
+//              low half for direction l (set A) and the high half for direction l + 16 (set B) of the group
+//              (Eq. 1).  The two half-warps of a warp work on different ions.  The u16 bit
+//              pattern c is the fp16 number c * 2^-24 (subnormal / first binade, exact for c <= 2048), so the
+//              histogram IS a valid fp16 tensor-core operand and is never converted or copied.
+//   layout   : byte address of (bin b, lane l) = (l/4)*160 + (l%4)*4 + 16*hi3 + 640*low,
+//              hi3 = b >> (log2 B - 3), low = b & (B/8 - 1).  Bank = 8*(l/4) + 4*hi3 + l%4 (mod 32): the 16 lanes
+//              of a half-warp hit 16 different banks whenever their bins agree in the top three bits (hi3) -- the
+//              plan sorts the directions into spatially compact patches of 16 so that they almost always do --
+//              and the other half-warp falls on the other 16 banks when its hi3 has the other parity.
+//              Read as an MN-major INTERLEAVE (no swizzle) operand with SBO = 160 B (between 8-element M chunks)
+//              and LBO = 2560 B (between 8-row K groups) this is a [128 x K] tile: M row = blk*32 + direction slot
+//              (blk = low & 3), K index = kg*8 + hi3 (kg = low >> 2), K = B/4.
 //   DFT      : X_k = sum_b h_b w^{bk} restricted to the window [k_lo,k_hi] is the dense contraction
-//              [directions x bins] x [bins x window] (L73, L75).  With b = hi3*B/8 + 2*kg + (pair*B/16 + blk)
-//              the four (pair, blk) parts share one twiddle table T[k=(kg,hi3)][n] and are recombined in the
-//              epilogue with the phases w^{(pair*B/16+blk) k}.  T holds cos/sin as fp16 hi + lo parts
-//              (columns 4w+{0,1,2,3} = cos_hi, sin_hi, 2^11 cos_lo, 2^11 sin_lo) so amplitudes reach ~1e-7.
+//              [directions x bins] x [bins x window] (L73, L75).  With b = hi3*B/8 + 4*kg + blk the four blk parts
+//              share one twiddle table T[k=(kg,hi3)][n] and are recombined in the epilogue with the phases
+//              w^{blk k}.  T holds cos/sin as fp16 hi + lo parts (columns 4w+{0,1,2,3} = cos_hi, sin_hi,
+//              2^11 cos_lo, 2^11 sin_lo) so amplitudes reach ~1e-7.
 //   peak     : |X_k|^2 arg-max over the window, lowest k on ties (L75, L416); A* = 2^24 sqrt(max).
-// One histogram buffer (144*B bytes): bin -> transform -> clear are serial per group; the epilogue of
-// group g runs while group g+1 is binned.  ROIs with more ions than the shared-memory ion buffer are
-// appended to a deferred list and handled by the general FFT kernel.
+// Two histogram buffers and two TMEM accumulators: while the 16 binning warps fill buffer (g+1)&1, the tensor
+// core transforms buffer g&1 and four service warps clear it and run the epilogue of group g.  ROIs with more
+// ions than the shared-memory ion buffer are appended to a deferred list and handled by the general FFT kernel.
 #include <algorithm>
 #include <cmath>
 #include <cuda_fp16.h>
@@ -34,12 +33,17 @@
 
 namespace apx {
 
-constexpr int kWorkWarps = 16;           // warps 0..15: project-and-bin, histogram clearing, epilogue
-constexpr int kWorkThreads = kWorkWarps * 32;
-constexpr int kMmaWarps = kWorkWarps + 1;  // warp 16 = tcgen05.mma issuer
+constexpr int kBinWarps = 16;            // warps 0..15: project-and-bin
+constexpr int kMmaWarp = 16;             // tcgen05.mma issuer
+constexpr int kSvcWarp0 = 17;            // warps 17..24: histogram clearing + epilogue (TMEM quarter = warp & 3),
+constexpr int kSvcWarps = 8;             // two sets of four warps that take alternate rounds of window bins
+constexpr int kMmaWarps = kSvcWarp0 + kSvcWarps;
 constexpr int kMmaThreads = kMmaWarps * 32;
-constexpr int kRowGroupBytes = 1152;     // 8 M-chunks of 144 B: one (blk, kg) slab of 8 K rows x 64 directions
-constexpr int kChunkBytes = 144;         // SBO: 8 directions x 8 rows x 2 B + 16 B skew
+constexpr int kSvcThreads = kSvcWarps * 32;
+constexpr int kChunkBytes = 160;         // SBO: 8 directions x 8 rows x 2 B + 32 B skew
+constexpr int kBlkBytes = 640;           // 4 M-chunks: one (blk, kg) slab of 8 K rows x 32 directions
+constexpr int kGroupBytes = 2560;        // LBO: 16 M-chunks = the 4 blk slabs of one 8-row K group
+constexpr int kEpiRound = 4;             // window bins per epilogue round (one tcgen05.ld x16)
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t cnt)
@@ -50,22 +54,20 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 {
     asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}" ::"r"(smem_u32(bar)) : "memory");
 }
+template <unsigned kSleepNs = 64>
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 {
     uint32_t done;
     uint32_t spins = 0;
     do {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-        if (!done && ++spins > (1u << 24)) asm volatile("trap;");     // never hang the device on a lost commit
+        // the hint lets the hardware park the warp (up to ~1 ms) instead of burning issue slots in a spin loop
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity), "r"(1000000u) : "memory");
+        if (!done) {
+            __nanosleep(kSleepNs);                                   // do not burn issue slots of the binning warps
+            if (++spins > (1u << 22)) asm volatile("trap;");         // never hang the device on a lost commit
+        }
     } while (!done);
-}
-// shared-memory matrix descriptor (tcgen05): start address, leading / stride byte offsets (16-byte units),
-// descriptor version 1, layout type in bits 61-63 (0 = INTERLEAVE / no swizzle, 2 = 128B, 4 = 64B)
-__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes, uint32_t layout)
-{
-    return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16) |
-           ((uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32) | ((uint64_t)1 << 46) | ((uint64_t)layout << 61);
 }
 __device__ __forceinline__ void mma_f16_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc)
 {
@@ -87,10 +89,11 @@ __device__ __forceinline__ float4 lds128(uint32_t addr)
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
 }
-__device__ __forceinline__ void tmem_ld8(uint32_t addr, uint32_t (&v)[8])
+__device__ __forceinline__ void tmem_ld16(uint32_t addr, uint32_t (&v)[16])
 {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
                  : "r"(addr));
 }
 
@@ -99,10 +102,11 @@ struct MmaParams {
     const uint32_t *cell_start;
     const GridParams *grid;
     const float *centres;
-    const float *dirs_sorted;  // [Dp][3] scaled directions in patch order (Dp = D rounded up to 64)
+    const float *dirs_sorted;  // [Dp][3] scaled directions in patch order (Dp = D rounded up to 32)
     const int *perm;           // [Dp] original direction index of each sorted slot, -1 = padding
     const uint4 *table;        // pre-swizzled twiddle operand image, (K/64) blocks of [N][128 B]
-    const float2 *phase;       // [4][W] recombination phases, index pair*2 + blk
+    const float2 *phase;       // [4][W] recombination phases w^{blk k}
+    const void *zeros;         // hist_bytes of zeros: source of the bulk copies that clear a histogram buffer
     float2 *sig;
     uint32_t *counts;
     uint32_t *deferred;        // [0] = count, [1..] = material point ids left to the FFT kernel
@@ -113,16 +117,18 @@ struct MmaParams {
 
 // smem carve-up (bytes), shared by host and device
 struct MmaSmem {
-    uint32_t table, hist, exch, cand, phase, ions, total;
+    uint32_t table, hist0, hist1, exch, cand, phase, ions, hist_bytes, total;
 };
 __host__ __device__ inline MmaSmem mma_smem_layout(int B, int N, int W, int cap)
 {
     MmaSmem s;
     uint32_t off = 0;
+    s.hist_bytes = (uint32_t)(B / 32) * kGroupBytes;             // K/8 = B/32 K groups of 2560 B
     s.table = off; off += (uint32_t)(B / 4) * N * 2;             // (K/64) * N * 128 with K = B/4; multiple of 1024
-    s.hist = off; off += (uint32_t)B * kChunkBytes;              // (B/8) row groups of 1152 B
-    s.exch = off; off += 128u * N;                                // (N/8 chunks) x 2 blk x 64 slots x float2
-    s.cand = off; off += 8u * 64 * 8;
+    s.hist0 = off; off += s.hist_bytes;
+    s.hist1 = off; off += s.hist_bytes;
+    s.exch = off; off += 2u * kEpiRound * 4 * 32 * 8;             // per set, one epilogue round: 4 bins x 4 blk x 32 slots x float2
+    s.cand = off; off += 8u * 32 * 8;
     s.phase = off; off += 4u * W * 8;
     s.ions = off; off += (uint32_t)cap * 12;
     s.total = off + 1024;                                          // slack for 1024-byte alignment
@@ -161,32 +167,33 @@ __device__ __forceinline__ void gather_roi3(const MmaParams &p, const GridParams
 // Project-and-bin (step a4) of one ion for one direction of this lane.
 //   ua = bits(RD(x + 1.5*2^23 + B/2))       = 0x4B400000 + b          (b = B/2 + floor(x), Eq. 1)
 //   va = bits(RD(x*2^-nl + 1.5*2^23 + 4))   = 0x4B400000 + hi3        (hi3 = b >> nl, exact: floor(floor(y)/n) = floor(y/n))
-//   address = hist + lane offset + 1152*low + 16*hi3 = ua*1152 + va*(16 - 1152*2^nl) + k0   (mod 2^32)
+//   address = hist + lane offset + 640*low + 16*hi3 = ua*640 + va*(16 - 640*2^nl) + k0   (mod 2^32)
 struct BinConst {
     float half_b, magic_a, magic_b, scl;
-    uint32_t kz, k0;
+    uint32_t kz;
 };
 template <bool kClamp>
 __device__ __forceinline__ void bin_one(float dx, float dy, float dz, float npx, float npy, float npz, const BinConst &c,
-                                        uint32_t inc)
+                                        uint32_t k0, uint32_t inc)
 {
     float x = __fmaf_rn(npz, dz, __fmaf_rn(npy, dy, __fmul_rn(npx, dx)));
     if (kClamp) x = fminf(fmaxf(x, -c.half_b), c.half_b - 0.25f);
     const uint32_t ua = __float_as_uint(__fadd_rd(x, c.magic_a));
     const uint32_t va = __float_as_uint(__fmaf_rd(x, c.scl, c.magic_b));
-    red_shared_add(ua * (uint32_t)kRowGroupBytes + (va * c.kz + c.k0), inc);
+    red_shared_add(ua * (uint32_t)kBlkBytes + (va * c.kz + k0), inc);
 }
 template <bool kClamp>
-__device__ __forceinline__ void bin_two(float dx, float dy, float dz, const float (&na)[3], const float (&nb)[3], const BinConst &c)
+__device__ __forceinline__ void bin_two(float dx, float dy, float dz, const float (&na)[3], const float (&nb)[3],
+                                        const BinConst &c, uint32_t k0)
 {
-    bin_one<kClamp>(dx, dy, dz, na[0], na[1], na[2], c, 1u);            // set A: low u16 of the lane's word
-    bin_one<kClamp>(dx, dy, dz, nb[0], nb[1], nb[2], c, 65536u);        // set B: high u16
+    bin_one<kClamp>(dx, dy, dz, na[0], na[1], na[2], c, k0, 1u);            // set A: low u16 of the lane's word
+    bin_one<kClamp>(dx, dy, dz, nb[0], nb[1], nb[2], c, k0, 65536u);        // set B: high u16
 }
 
-// ions_s = shared-space byte address of the packed ion records; i0 is a multiple of 4
+// ions_s = shared-space byte address of the packed ion records; i0 is a multiple of 4 (per half-warp)
 template <bool kClamp>
 __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const float (&na)[3], const float (&nb)[3],
-                                         const BinConst &c)
+                                         const BinConst &c, uint32_t k0)
 {
     int ib = i0;
     for (; ib + 8 <= i1; ib += 8) {                          // 8 ions = 6 LDS.128, then 16 independent chains
@@ -196,19 +203,19 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             const float4 a = q[3 * h], b = q[3 * h + 1], d = q[3 * h + 2];
-            bin_two<kClamp>(a.x, a.y, a.z, na, nb, c);
-            bin_two<kClamp>(a.w, b.x, b.y, na, nb, c);
-            bin_two<kClamp>(b.z, b.w, d.x, na, nb, c);
-            bin_two<kClamp>(d.y, d.z, d.w, na, nb, c);
+            bin_two<kClamp>(a.x, a.y, a.z, na, nb, c, k0);
+            bin_two<kClamp>(a.w, b.x, b.y, na, nb, c, k0);
+            bin_two<kClamp>(b.z, b.w, d.x, na, nb, c, k0);
+            bin_two<kClamp>(d.y, d.z, d.w, na, nb, c, k0);
         }
     }
     if (ib + 4 <= i1) {
         const float4 a = lds128(ions_s + (uint32_t)ib * 12u), b = lds128(ions_s + (uint32_t)ib * 12u + 16u),
                      d = lds128(ions_s + (uint32_t)ib * 12u + 32u);
-        bin_two<kClamp>(a.x, a.y, a.z, na, nb, c);
-        bin_two<kClamp>(a.w, b.x, b.y, na, nb, c);
-        bin_two<kClamp>(b.z, b.w, d.x, na, nb, c);
-        bin_two<kClamp>(d.y, d.z, d.w, na, nb, c);
+        bin_two<kClamp>(a.x, a.y, a.z, na, nb, c, k0);
+        bin_two<kClamp>(a.w, b.x, b.y, na, nb, c, k0);
+        bin_two<kClamp>(b.z, b.w, d.x, na, nb, c, k0);
+        bin_two<kClamp>(d.y, d.z, d.w, na, nb, c, k0);
         ib += 4;
     }
     for (; ib < i1; ++ib) {
@@ -216,86 +223,79 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dx) : "r"(ions_s + (uint32_t)ib * 12u));
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dy) : "r"(ions_s + (uint32_t)ib * 12u + 4u));
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(ions_s + (uint32_t)ib * 12u + 8u));
-        bin_two<kClamp>(dx, dy, dz, na, nb, c);
+        bin_two<kClamp>(dx, dy, dz, na, nb, c, k0);
     }
 }
 
-// Epilogue of one direction group (steps a5 tail, a6, a7), run by all 16 worker warps while the tensor core
-// transforms the next group.  Worker warp w reads TMEM lane quarter q = w & 3 (M rows 32q..32q+31: blk = q >> 1,
-// direction slot from the lane) and the 8-column chunks c = j, j+4, ... (j = w >> 2; a chunk = 2 window bins).
-// A bin of the window is finished by the blk that matches its parity: the other blk hands its partial over
-// through `exch`.  Eight candidates per direction (2 blk x 4 j) are reduced by warps 0-1 and stored.
-__device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc_set, int gi, int64_t m, const float2 *phase,
-                                               float2 *exch, float2 *cand, int warp, int lane)
+// Epilogue of one direction group (a5 tail, a6, a7) by the eight service warps.  Service warp (set, q) reads TMEM
+// lane quarter q = M rows 32q..32q+31 = part blk = q of all 32 direction slots (slot from the lane).  Window bins
+// are handled in rounds of 4 (set s takes rounds s, s+2, ...): each thread scales its 4 partial sums by the phase
+// w^{blk k}, keeps the one whose index is q and hands the other three to the partner warps of its set through
+// `exch` (a reduce-scatter over blk).
+__device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc, int gi, int64_t m, const float2 *phase,
+                                               float2 *exch_all, float2 *cand, int set, int q, int lane)
 {
-    const int q = warp & 3, j = warp >> 2, blk = q >> 1;
-    const int t = ((q & 1) << 5) + lane;
-    const uint32_t acc0 = acc_set + ((uint32_t)(q * 32) << 16);
-    const int nch = p.N >> 3;
-    float2 keep[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-        const int c = j + 4 * u;
-        keep[u] = make_float2(0.f, 0.f);
-        if (c < nch) {
-            uint32_t v0[8], v1[8];
-            tmem_ld8(acc0 + (uint32_t)(c * 8), v0);
-            tmem_ld8(acc0 + (uint32_t)(p.N + c * 8), v1);
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-            for (int jj = 0; jj < 2; ++jj) {
-                const int w = 2 * c + jj;
-                if (w < p.W) {
-                    const float r0 = __uint_as_float(v0[4 * jj]) + __uint_as_float(v0[4 * jj + 2]) * (1.0f / 2048.0f);
-                    const float i0 = -(__uint_as_float(v0[4 * jj + 1]) + __uint_as_float(v0[4 * jj + 3]) * (1.0f / 2048.0f));
-                    const float r1 = __uint_as_float(v1[4 * jj]) + __uint_as_float(v1[4 * jj + 2]) * (1.0f / 2048.0f);
-                    const float i1 = -(__uint_as_float(v1[4 * jj + 1]) + __uint_as_float(v1[4 * jj + 3]) * (1.0f / 2048.0f));
-                    const float2 f0 = phase[blk * p.W + w], f1 = phase[(2 + blk) * p.W + w];
-                    const float xr = (f0.x * r0 - f0.y * i0) + (f1.x * r1 - f1.y * i1);
-                    const float xi = (f0.x * i0 + f0.y * r0) + (f1.x * i1 + f1.y * r1);
-                    if (jj == blk) keep[u] = make_float2(xr, xi);
-                    else exch[(c * 2 + blk) * 64 + t] = make_float2(xr, xi);
-                }
-            }
-        }
-    }
-    asm volatile("bar.sync 1, %0;" ::"n"(kWorkThreads) : "memory");
+    const uint32_t acc0 = acc + ((uint32_t)(q * 32) << 16);
+    float2 *exch = exch_all + set * (kEpiRound * 4 * 32);
     float best = -1.0f;
     int kbest = p.k_lo;
+#pragma unroll 1
+    for (int r0 = set * kEpiRound; r0 < p.W; r0 += 2 * kEpiRound) {
+        uint32_t v[16];
+        tmem_ld16(acc0 + (uint32_t)(4 * r0), v);
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        float2 keep = make_float2(0.f, 0.f);
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-        const int c = j + 4 * u, w = 2 * c + blk;
-        if (c < nch && w < p.W) {
-            const float2 o = exch[(c * 2 + (1 - blk)) * 64 + t];
-            const float xr = keep[u].x + o.x, xi = keep[u].y + o.y;
+        for (int j = 0; j < kEpiRound; ++j) {
+            const int w = r0 + j;
+            if (w < p.W) {
+                const float re = __uint_as_float(v[4 * j]) + __uint_as_float(v[4 * j + 2]) * (1.0f / 2048.0f);
+                const float im = -(__uint_as_float(v[4 * j + 1]) + __uint_as_float(v[4 * j + 3]) * (1.0f / 2048.0f));
+                const float2 f = phase[q * p.W + w];
+                const float2 P = make_float2(f.x * re - f.y * im, f.x * im + f.y * re);
+                if (j == q) keep = P;
+                else exch[(j * 4 + q) * 32 + lane] = P;
+            }
+        }
+        if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
+        const int w = r0 + q;
+        if (w < p.W) {
+            float xr = keep.x, xi = keep.y;
+#pragma unroll
+            for (int o = 1; o < 4; ++o) {
+                const float2 e = exch[(q * 4 + ((q + o) & 3)) * 32 + lane];
+                xr += e.x; xi += e.y;
+            }
             const float pw = xr * xr + xi * xi;
             if (pw > best) { best = pw; kbest = p.k_lo + w; }            // ascending w: lowest k kept on ties
         }
+        if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
     }
-    cand[(blk * 4 + j) * 64 + t] = make_float2(best, __int_as_float(kbest));
-    asm volatile("bar.sync 1, %0;" ::"n"(kWorkThreads) : "memory");
-    if (warp < 2) {
+    cand[(set * 4 + q) * 32 + lane] = make_float2(best, __int_as_float(kbest));
+    asm volatile("bar.sync 5, %0;" ::"n"(kSvcThreads) : "memory");
+    if (set == 0 && q == 0) {
         float bb = -1.0f;
         int kb = p.k_lo;
 #pragma unroll
         for (int s = 0; s < 8; ++s) {
-            const float2 c2 = cand[s * 64 + t];
+            const float2 c2 = cand[s * 32 + lane];
             const int ck = __float_as_int(c2.y);
             if (c2.x > bb || (c2.x == bb && ck < kb)) { bb = c2.x; kb = ck; }
         }
-        const int slot = ((lane & 1) << 5) + ((warp & 1) << 4) + ((lane >> 3) << 2) + ((lane & 7) >> 1);
-        const int d = p.perm[gi * 64 + slot];
+        const int slot = ((lane & 1) << 4) + ((lane >> 3) << 2) + ((lane & 7) >> 1);
+        const int d = p.perm[gi * 32 + slot];
         if (d >= 0) p.sig[(size_t)m * p.D + d] = make_float2(16777216.0f * sqrtf(fmaxf(bb, 0.0f)), (float)kb);
     }
 }
 
-template <int KS>   // KS = K/16 = B/64 k-steps per accumulator
+template <int KS>   // KS = K/16 = B/64 k-steps per group
 __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParams p)
 {
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned, still shared-space
     const MmaSmem L = mma_smem_layout(p.B, p.N, p.W, p.cap);
-    __shared__ uint64_t s_full, s_done[2];   // s_done[h]: the MMAs reading histogram half h (= pair h) have completed
+    // per histogram buffer: full (binned), done (transformed), free (cleared); per accumulator: tfree (read out)
+    __shared__ uint64_t s_full[2], s_done[2], s_free[2], s_tfree[2];
     __shared__ uint32_t s_tmem;
     __shared__ int s_n;
 
@@ -312,13 +312,15 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     float2 *cand = reinterpret_cast<float2 *>(smem + L.cand);
     float2 *phase = reinterpret_cast<float2 *>(smem + L.phase);
     constexpr int K = KS * 16;
-    const uint32_t hist_bytes = (uint32_t)p.B * kChunkBytes;
 
-    // ---- setup: barriers, TMEM, zero histogram, twiddle table, gather ------------------------------
+    // ---- setup: barriers, TMEM, zero histograms, twiddle table, gather ------------------------------
     if (tid == 0) {
-        mbar_init(&s_full, kWorkWarps);
-        mbar_init(&s_done[0], 1);
-        mbar_init(&s_done[1], 1);
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(&s_full[i], kBinWarps);
+            mbar_init(&s_done[i], 1);
+            mbar_init(&s_free[i], 1);
+            mbar_init(&s_tfree[i], kSvcWarps);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;");
         s_n = 0;
     }
@@ -327,8 +329,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     {
-        uint4 *h = reinterpret_cast<uint4 *>(smem + L.hist);
-        for (int i = tid; i < (int)(hist_bytes / 16); i += kMmaThreads) h[i] = make_uint4(0, 0, 0, 0);
+        uint4 *h = reinterpret_cast<uint4 *>(smem + L.hist0);
+        for (int i = tid; i < (int)(2 * L.hist_bytes / 16); i += kMmaThreads) h[i] = make_uint4(0, 0, 0, 0);   // both buffers
         uint4 *t = reinterpret_cast<uint4 *>(smem + L.table);
         for (int i = tid; i < K * p.N / 8; i += kMmaThreads) t[i] = p.table[i];
         for (int i = tid; i < 4 * p.W; i += kMmaThreads) phase[i] = p.phase[i];
@@ -347,88 +349,96 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
         // too many ions for the shared buffer: leave this material point to the FFT kernel
         if (chunk == 0 && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
     } else {
-        // Pipeline over items = (direction group, ion pass); one histogram buffer, two TMEM accumulator sets.
-        //   worker warps 0..15 : [wait done(it-1) -> clear the histogram] -> project-and-bin item it -> arrive full(it)
-        //                        -> epilogue of the previous group (its accumulators are in the other TMEM set)
-        //   MMA warp 16        : wait full(it) -> 2 x K/16 tcgen05.mma into set (group & 1) -> commit to done(it)
+        // Pipeline over items = (direction group, ion pass); item it uses histogram buffer it & 1 and the TMEM
+        // accumulator (group & 1):
+        //   binning warps 0..15 : wait free(buf) -> project-and-bin item it -> arrive full(buf)
+        //   MMA warp 16         : wait full(buf) [, tfree(acc)] -> K/16 tcgen05.mma -> commit to done(buf)
+        //   service warps 17..20: wait done(buf) -> clear the buffer -> arrive free(buf); after the last pass of a
+        //                         group: epilogue from TMEM -> arrive tfree(acc)
         const int npass = n > 2048 ? (n + 2047) / 2048 : 1;          // fp16 counters are exact up to 2048
         const int nitems = (g_end - g_begin) * npass;
-        if (warp < kWorkWarps) {
+        if (warp < kBinWarps) {
             BinConst c;
             c.half_b = (float)(p.B / 2); c.magic_a = magic_for(p.B); c.magic_b = 12582912.0f + 4.0f;
             c.scl = __int_as_float((127 - p.nl) << 23);                       // 2^-nl
-            c.kz = 16u - (uint32_t)kRowGroupBytes * (1u << p.nl);
-            c.k0 = smem_u32(smem + L.hist) + (uint32_t)(lane >> 2) * kChunkBytes + (uint32_t)(lane & 3) * 4u
-                   - 0x4B400000u * (uint32_t)kRowGroupBytes - 0x4B400000u * c.kz;
+            c.kz = 16u - (uint32_t)kBlkBytes * (1u << p.nl);
+            const int l = lane & 15, hw = warp * 2 + (lane >> 4);             // half-warp index 0..31
+            const uint32_t k0base = smem_u32(smem + L.hist0) + (uint32_t)(l >> 2) * kChunkBytes + (uint32_t)(l & 3) * 4u
+                                    - 0x4B400000u * (uint32_t)kBlkBytes - 0x4B400000u * c.kz;
             const uint32_t ions_s = smem_u32(ions);
             for (int it = 0; it < nitems; ++it) {
-                const int gl = it / npass, pass = it % npass;
+                const int gl = it / npass, pass = it % npass, buf = it & 1;
                 float na[3], nb[3];
                 {
-                    const float *da = p.dirs_sorted + (size_t)((g_begin + gl) * 64 + lane) * 3;
+                    const float *da = p.dirs_sorted + (size_t)((g_begin + gl) * 32 + l) * 3;
                     na[0] = da[0]; na[1] = da[1]; na[2] = da[2];
-                    nb[0] = da[96]; nb[1] = da[97]; nb[2] = da[98];
+                    nb[0] = da[48]; nb[1] = da[49]; nb[2] = da[50];
                 }
-                if (it > 0) {
-                    // clear each histogram half as soon as the MMAs that read it have completed
-                    uint4 *h = reinterpret_cast<uint4 *>(smem + L.hist);
-                    const int half16 = (int)(hist_bytes / 32);
-#pragma unroll
-                    for (int hh = 0; hh < 2; ++hh) {
-                        mbar_wait(&s_done[hh], (uint32_t)((it - 1) & 1));
-                        for (int i = tid; i < half16; i += kWorkThreads) h[hh * half16 + i] = make_uint4(0, 0, 0, 0);
-                    }
-                    asm volatile("tcgen05.fence::after_thread_sync;");
-                    asm volatile("bar.sync 2, %0;" ::"n"(kWorkThreads) : "memory");
-                }
+                if (it >= 2) mbar_wait(&s_free[buf], (uint32_t)(((it >> 1) - 1) & 1));    // cleared after item it-2
                 const int a0 = pass * 2048, a1 = min(n, a0 + 2048);
-                const int per = (((a1 - a0 + kWorkWarps - 1) / kWorkWarps) + 3) & ~3;
-                const int i0 = min(a1, a0 + warp * per), i1 = min(a1, i0 + per);
-                if (p.clamp) bin_ions<true>(ions_s, i0, i1, na, nb, c);
-                else bin_ions<false>(ions_s, i0, i1, na, nb, c);
+                const int per = (((a1 - a0 + 2 * kBinWarps - 1) / (2 * kBinWarps)) + 3) & ~3;
+                const int i0 = min(a1, a0 + hw * per), i1 = min(a1, i0 + per);
+                const uint32_t k0 = k0base + (uint32_t)buf * L.hist_bytes;
+                if (p.clamp) bin_ions<true>(ions_s, i0, i1, na, nb, c, k0);
+                else bin_ions<false>(ions_s, i0, i1, na, nb, c, k0);
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
-                asm volatile("tcgen05.fence::before_thread_sync;");              // earlier TMEM reads -> next MMA
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&s_full);
-                if (it > 0 && pass == 0)                                         // item it-1 closed group gl-1
-                    epilogue_group(p, tmem + (uint32_t)(((gl - 1) & 1) * 2 * p.N), g_begin + gl - 1, m, phase, exch, cand, warp, lane);
+                if (lane == 0) mbar_arrive(&s_full[buf]);
             }
-            if (nitems > 0) {
-                const int gl = (nitems - 1) / npass;
-                mbar_wait(&s_done[1], (uint32_t)((nitems - 1) & 1));
-                asm volatile("tcgen05.fence::after_thread_sync;");
-                epilogue_group(p, tmem + (uint32_t)((gl & 1) * 2 * p.N), g_begin + gl, m, phase, exch, cand, warp, lane);
-            }
-        } else {
+        } else if (warp == kMmaWarp) {
             // ---- MMA warp: descriptors advance by adding to the 14-bit start-address field ---------------
             const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(p.N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-            const uint32_t tb = smem_u32(smem + L.table), hb = smem_u32(smem + L.hist);
-            const uint32_t a_hi = (uint32_t)(kChunkBytes >> 4) | (1u << 14);                              // SBO, version 1, INTERLEAVE
-            const uint32_t a_lo0 = ((hb >> 4) & 0x3FFFu) | ((uint32_t)((2 * kRowGroupBytes) >> 4) << 16);   // LBO = 2304 B
-            const uint32_t b_hi = (uint32_t)(1024 >> 4) | (1u << 14) | (2u << 29);                          // SBO, version 1, SWIZZLE_128B
+            const uint32_t tb = smem_u32(smem + L.table), hb = smem_u32(smem + L.hist0);
+            const uint32_t a_hi = (uint32_t)(kChunkBytes >> 4) | (1u << 14);                         // SBO, version 1, INTERLEAVE
+            const uint32_t a_lo0 = ((hb >> 4) & 0x3FFFu) | ((uint32_t)(kGroupBytes >> 4) << 16);       // LBO = 2560 B
+            const uint32_t b_hi = (uint32_t)(1024 >> 4) | (1u << 14) | (2u << 29);                     // SBO, version 1, SWIZZLE_128B
             const uint32_t b_lo0 = ((tb >> 4) & 0x3FFFu) | (1u << 16);
-            const uint32_t pair_step = ((uint32_t)kRowGroupBytes * (uint32_t)(p.B / 16)) >> 4;
             const uint32_t kblk_step = (uint32_t)(p.N * 128) >> 4;
             for (int it = 0; it < nitems; ++it) {
-                const int gl = it / npass, pass = it % npass;
-                mbar_wait(&s_full, (uint32_t)(it & 1));
+                const int gl = it / npass, pass = it % npass, buf = it & 1;
+                mbar_wait<100>(&s_full[buf], (uint32_t)((it >> 1) & 1));
+                if (pass == 0 && gl >= 2) mbar_wait(&s_tfree[gl & 1], (uint32_t)(((gl >> 1) - 1) & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;");
-                const uint32_t acc = tmem + (uint32_t)((gl & 1) * 2 * p.N);
+                const uint32_t acc = tmem + (uint32_t)((gl & 1) * p.N);
                 if (lane == 0) {
+                    const uint32_t a_lo = a_lo0 + (uint32_t)buf * (L.hist_bytes >> 4);
 #pragma unroll
-                    for (int pr = 0; pr < 2; ++pr) {
-#pragma unroll
-                        for (int ks = 0; ks < KS; ++ks) {
-                            const uint64_t ad = ((uint64_t)a_hi << 32) | (a_lo0 + (uint32_t)pr * pair_step + (uint32_t)ks * ((4 * kRowGroupBytes) >> 4));
-                            const uint64_t bd = ((uint64_t)b_hi << 32) | (b_lo0 + (uint32_t)(ks >> 2) * kblk_step + (uint32_t)(ks & 3) * 2u);
-                            if (ks == 0) mma_f16_ss(acc + (uint32_t)(pr * p.N), ad, bd, idesc, pass > 0 ? 1u : 0u);
-                            else mma_f16_acc(acc + (uint32_t)(pr * p.N), ad, bd, idesc);
-                        }
-                        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
-                                     ::"r"(smem_u32(&s_done[pr])) : "memory");
+                    for (int ks = 0; ks < KS; ++ks) {
+                        const uint64_t ad = ((uint64_t)a_hi << 32) | (a_lo + (uint32_t)ks * ((2 * kGroupBytes) >> 4));
+                        const uint64_t bd = ((uint64_t)b_hi << 32) | (b_lo0 + (uint32_t)(ks >> 2) * kblk_step + (uint32_t)(ks & 3) * 2u);
+                        if (ks == 0) mma_f16_ss(acc, ad, bd, idesc, pass > 0 ? 1u : 0u);
+                        else mma_f16_acc(acc, ad, bd, idesc);
                     }
+                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
+                                 ::"r"(smem_u32(&s_done[buf])) : "memory");
                 }
                 __syncwarp();
+            }
+        } else {
+            // ---- service warps: clear the transformed histogram, then the epilogue ------------------------
+            const int q = warp & 3, st = tid - kSvcWarp0 * 32, set = (warp - kSvcWarp0) >> 2;
+            for (int it = 0; it < nitems; ++it) {
+                const int gl = it / npass, buf = it & 1;
+                const bool last_pass = (it % npass) == npass - 1;
+                mbar_wait<200>(&s_done[buf], (uint32_t)((it >> 1) & 1));
+                asm volatile("tcgen05.fence::after_thread_sync;");
+                if (st == 0) {
+                    // clear the buffer with bulk copies of zeros (TMA engine, no LSU work); free(buf) completes
+                    // when all bytes have landed
+                    const uint32_t dst = smem_u32(smem + (buf ? L.hist1 : L.hist0)), bar = smem_u32(&s_free[buf]);
+                    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(L.hist_bytes) : "memory");
+                    const uint32_t piece = L.hist_bytes / 4;
+#pragma unroll
+                    for (int c4 = 0; c4 < 4; ++c4)
+                        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                                     ::"r"(dst + c4 * piece), "l"((const char *)p.zeros + c4 * piece), "r"(piece), "r"(bar) : "memory");
+                }
+                if (last_pass) {
+                    epilogue_group(p, tmem + (uint32_t)((gl & 1) * p.N), g_begin + gl, m, phase, exch, cand, set, q, lane);
+                    asm volatile("tcgen05.fence::before_thread_sync;");
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&s_tfree[gl & 1]);
+                }
             }
         }
     }
@@ -452,17 +462,17 @@ bool mma_path_supported(const Plan *p)
 {
     if (p->B > 1024) return false;                       // B = 2048, 4096 stay on the FFT kernel
     const int N = mma_n_for(p->W);
-    if (4 * N > 512) return false;                       // two sets of two accumulators of N TMEM columns
+    if (2 * N > 512) return false;                       // two accumulators of N TMEM columns
     return mma_cap_for(p->B, N, p->W) >= 1024;           // room for a useful ion buffer
 }
 
-// Order the directions so that every run of 32 is a spatially compact patch: recursive bisection along the
-// widest axis, cutting at a multiple of 32.  Within one shared atomic the 32 lanes then project an ion onto
-// nearly parallel directions, their bins share the top three bits and the histogram layout is conflict-free.
+// Order the directions so that every run of 16 is a spatially compact patch: recursive bisection along the
+// widest axis, cutting at a multiple of 16.  Within one shared atomic the 16 lanes of a half-warp then project
+// an ion onto nearly parallel directions, their bins share the top three bits and hit 16 different banks.
 static void patch_order(const std::vector<float> &v, std::vector<int> &idx, int lo, int hi)
 {
     const int cnt = hi - lo;
-    if (cnt <= 32) return;
+    if (cnt <= 16) return;
     float mn[3] = {1e30f, 1e30f, 1e30f}, mx[3] = {-1e30f, -1e30f, -1e30f};
     for (int i = lo; i < hi; ++i)
         for (int a = 0; a < 3; ++a) {
@@ -472,8 +482,8 @@ static void patch_order(const std::vector<float> &v, std::vector<int> &idx, int 
     int ax = 0;
     for (int a = 1; a < 3; ++a)
         if (mx[a] - mn[a] > mx[ax] - mn[ax]) ax = a;
-    const int leaves = (cnt + 31) / 32;
-    const int left = (leaves / 2) * 32;
+    const int leaves = (cnt + 15) / 16;
+    const int left = (leaves / 2) * 16;
     std::nth_element(idx.begin() + lo, idx.begin() + lo + left, idx.begin() + hi,
                      [&](int a, int b) { return v[3 * (size_t)a + ax] < v[3 * (size_t)b + ax]; });
     patch_order(v, idx, lo, lo + left);
@@ -485,14 +495,14 @@ cudaError_t mma_path_prepare(Plan *p)
     const int B = p->B, K = B / 4, W = p->W, N = mma_n_for(W);
     int nl = 0;
     while ((8 << nl) < B) ++nl;                          // B = 8 * 2^nl
-    // twiddle table: K index k = kg*8 + hi3 stands for the bin part hi3*(B/8) + 2*kg
+    // twiddle table: K index k = kg*8 + hi3 stands for the bin part hi3*(B/8) + 4*kg
     std::vector<uint16_t> img((size_t)K * N, 0);
     for (int r = 0; r < K; ++r)
         for (int n = 0; n < N; ++n) {
             const int w = n / 4, c = n % 4;
             __half val = __float2half(0.0f);
             if (w < W) {
-                const int64_t binpart = (int64_t)(r & 7) * (B / 8) + 2 * (r >> 3);
+                const int64_t binpart = (int64_t)(r & 7) * (B / 8) + 4 * (r >> 3);
                 const double th = 2.0 * M_PI * (double)((binpart * (p->k_lo + w)) % B) / (double)B;
                 const double v = (c & 1) ? std::sin(th) : std::cos(th);
                 const __half hi = __float2half((float)v);
@@ -506,11 +516,11 @@ cudaError_t mma_path_prepare(Plan *p)
     if (e != cudaSuccess) return e;
     e = cudaMemcpy(p->d_mma_table, img.data(), img.size() * 2, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return e;
-    // recombination phases exp(-2 pi i (pair*B/16 + blk) k / B)
+    // recombination phases exp(-2 pi i blk k / B), blk = 0..3
     std::vector<float2> ph((size_t)4 * W);
     for (int pb = 0; pb < 4; ++pb)
         for (int w = 0; w < W; ++w) {
-            const int64_t off = (int64_t)(pb >> 1) * (B / 16) + (pb & 1);
+            const int64_t off = pb;
             const double th = 2.0 * M_PI * (double)((off * (p->k_lo + w)) % B) / (double)B;
             ph[(size_t)pb * W + w] = make_float2((float)std::cos(th), (float)-std::sin(th));
         }
@@ -519,6 +529,10 @@ cudaError_t mma_path_prepare(Plan *p)
     e = cudaMemcpy(p->d_mma_phase, ph.data(), ph.size() * sizeof(float2), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return e;
 
+    e = cudaMalloc(&p->d_mma_zero, (size_t)(B / 32) * kGroupBytes);
+    if (e != cudaSuccess) return e;
+    e = cudaMemset(p->d_mma_zero, 0, (size_t)(B / 32) * kGroupBytes);
+    if (e != cudaSuccess) return e;
     std::vector<float> nps((size_t)3 * p->D);
     e = cudaMemcpy(nps.data(), p->d_dirs_scaled, nps.size() * 4, cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) return e;
@@ -533,11 +547,11 @@ cudaError_t mma_path_prepare(Plan *p)
     }
     p->mma_clamp = unit ? 0 : 1;
 
-    // patch order + padding to a multiple of 64 (padding slots repeat the last direction, perm = -1)
+    // patch order + padding to a multiple of 32 (padding slots repeat the last direction, perm = -1)
     std::vector<int> idx(p->D);
     std::iota(idx.begin(), idx.end(), 0);
     patch_order(nps, idx, 0, p->D);
-    const int Dp = ((p->D + 63) / 64) * 64;
+    const int Dp = ((p->D + 31) / 32) * 32;
     std::vector<float> sorted((size_t)3 * Dp);
     std::vector<int> perm(Dp, -1);
     for (int i = 0; i < Dp; ++i) {
@@ -572,14 +586,14 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     MmaParams q;
     q.sorted = p->d_sorted; q.cell_start = p->d_cell_start; q.grid = p->d_grid; q.centres = centres;
     q.dirs_sorted = p->d_dirs_sorted; q.perm = p->d_dir_perm;
-    q.table = reinterpret_cast<const uint4 *>(p->d_mma_table); q.phase = p->d_mma_phase;
+    q.table = reinterpret_cast<const uint4 *>(p->d_mma_table); q.phase = p->d_mma_phase; q.zeros = p->d_mma_zero;
     q.sig = reinterpret_cast<float2 *>(sig); q.counts = counts; q.deferred = p->d_deferred;
     q.D = p->D; q.B = p->B; q.k_lo = p->k_lo; q.W = p->W; q.N = mma_n_for(p->W);
     q.nl = 0;
     while ((8 << q.nl) < p->B) ++q.nl;
     q.cap = mma_cap_for(p->B, q.N, p->W);
-    q.ngroups = p->Dp / 64;
-    int nchunks = (q.ngroups + 47) / 48;
+    q.ngroups = p->Dp / 32;
+    int nchunks = (q.ngroups + 95) / 96;
     const int64_t want = (int64_t)p->sm_count * 8;
     if (M * nchunks < want) nchunks = (int)((want + M - 1) / M);
     if (nchunks > (q.ngroups + 1) / 2) nchunks = (q.ngroups + 1) / 2;
@@ -587,7 +601,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.nchunks = nchunks;
     q.clamp = p->mma_clamp;
     uint32_t cols = 32;
-    while (cols < (uint32_t)(4 * q.N)) cols *= 2;
+    while (cols < (uint32_t)(2 * q.N)) cols *= 2;
     q.tmem_cols = cols;
     q.R = p->R; q.R2 = p->R2;
     const MmaSmem L = mma_smem_layout(p->B, q.N, p->W, q.cap);

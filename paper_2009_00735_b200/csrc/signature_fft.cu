@@ -1,201 +1,326 @@
 // signature_fft.cu -- general signature kernel (any window, B = 256..4096): steps a2, a4-a7.
-// One CTA = one material point x one chunk of directions.  The ROI's ions are gathered once into
-// shared memory (SoA), then each warp takes one direction at a time: bins the ions into a private
-// shared-memory histogram (Eq. 1), runs an in-place packed real FFT on it (the paper
-// calls MKL/FFTW per histogram, L379; this is the hand-written batched replacement), scans the window
-// for the largest |X_k|^2 (L75, L416) and stores (amplitude, bin).  Histograms never leave the SM.
+//
+// One CTA (16 warps) = one material point x a chunk of direction groups; a group = G directions
+// (G = 32 for B <= 1024, 16 for B = 2048, 8 for B = 4096: B*G*4 bytes = at most 128 KB of shared memory).
+//   gather   : the ROI's ions are collected once per CTA into shared memory (packed dx, dy, dz).
+//   binning  : lane = direction (lane % G), the warps split the ions; counter of (bin b, direction d) is the
+//              32-bit word b*G + d, so for G = 32 every lane of a shared atomic hits its own bank (Eq. 1,
+//              PAPER.md L68-71).  A pair costs FMUL, 2 FFMA, FADD.RM, IMAD, ATOMS.
+//   FFT      : the B counts of a direction are read as N = B/2 complex points z_j = (h_2j, h_2j+1) (real input
+//              packing; the paper calls a real-to-complex library FFT per histogram, L73/L379) and transformed
+//              in place by radix-8 decimation-in-frequency passes held in registers (plus one radix-2/4 pass):
+//              512/G threads per direction, each butterfly reads and writes only its own lane's bank.  The first
+//              pass converts the integer counts to float on load.
+//   peak     : the split step X_k = (Z_k + conj Z_{N-k})/2 - i w^k (Z_k - conj Z_{N-k})/2 is evaluated only for
+//              the window bins, |X_k|^2 arg-max with the lowest k on ties (L75, L416), one sqrt at the end.
+// Histograms and spectra never leave the SM.  ROIs with more ions than the shared buffer holds are binned by
+// streaming their cell rows from global memory again for every group (no size limit).
 #include "common.cuh"
 
 namespace apx {
 
-constexpr int kThreads = 256;
-constexpr int kWarps = kThreads / 32;
-constexpr int kDirChunk = 256;            // directions per CTA
+constexpr int kFftThreads = 512;
+constexpr int kFftWarps = kFftThreads / 32;
+
+struct FftParams {
+    const float4 *sorted;
+    const uint32_t *cell_start;
+    const GridParams *grid;
+    const float *centres;
+    const float *dirs_scaled;
+    const float2 *tw;          // [B/2] exp(-2 pi i r / B)
+    float2 *sig;
+    uint32_t *counts;
+    const uint32_t *list;      // nullptr = direct mode; else list[0] = count, list[1..] = material point ids
+    int D, k_lo, k_hi, cap, nchunks, ngroups;
+    float R, R2;
+};
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 mul_mi(float2 a) { return make_float2(a.y, -a.x); }          // a * (-i)
+
+// w_B^r for 0 <= r < B from the half table (w^{r + B/2} = -w^r)
+template <int B>
+__device__ __forceinline__ float2 twiddle(const float2 *tw, int r)
+{
+    const float2 w = tw[r & (B / 2 - 1)];
+    return (r & (B / 2)) ? make_float2(-w.x, -w.y) : w;
+}
+
+// forward DFT of R points in registers (R = 2, 4, 8), natural order in, natural order out
+template <int R>
+__device__ __forceinline__ void dft(float2 (&x)[R])
+{
+    if (R == 2) {
+        const float2 a = x[0], b = x[1];
+        x[0] = cadd(a, b); x[1] = csub(a, b);
+    } else if (R == 4) {
+        const float2 a = cadd(x[0], x[2]), b = csub(x[0], x[2]), c = cadd(x[1], x[3]), d = mul_mi(csub(x[1], x[3]));
+        x[0] = cadd(a, c); x[2] = csub(a, c); x[1] = cadd(b, d); x[3] = csub(b, d);
+    } else {
+        const float h = 0.70710678118654752440f;
+        // stage 1: pairs (m, m+4)
+        float2 a0 = cadd(x[0], x[4]), a1 = cadd(x[1], x[5]), a2 = cadd(x[2], x[6]), a3 = cadd(x[3], x[7]);
+        float2 b0 = csub(x[0], x[4]), b1 = csub(x[1], x[5]), b2 = csub(x[2], x[6]), b3 = csub(x[3], x[7]);
+        // twiddles w_8^m on the odd half: 1, (1-i)/sqrt2, -i, (-1-i)/sqrt2
+        b1 = make_float2(h * (b1.x + b1.y), h * (b1.y - b1.x));
+        b2 = mul_mi(b2);
+        b3 = make_float2(h * (b3.y - b3.x), -h * (b3.x + b3.y));
+        // two 4-point DFTs: even outputs from a, odd outputs from b
+        float2 c0 = cadd(a0, a2), c1 = csub(a0, a2), c2 = cadd(a1, a3), c3 = mul_mi(csub(a1, a3));
+        x[0] = cadd(c0, c2); x[4] = csub(c0, c2); x[2] = cadd(c1, c3); x[6] = csub(c1, c3);
+        float2 d0 = cadd(b0, b2), d1 = csub(b0, b2), d2 = cadd(b1, b3), d3 = mul_mi(csub(b1, b3));
+        x[1] = cadd(d0, d2); x[5] = csub(d0, d2); x[3] = cadd(d1, d3); x[7] = csub(d1, d3);
+    }
+}
+
+// One in-place decimation-in-frequency pass of radix R over sub-transforms of length L (N = B/2 points per
+// direction, T threads per direction, this thread = t).  Element e of direction d: re at word (2e)*G + d,
+// im at (2e+1)*G + d.  kFirst: the buffer still holds the integer counts.
+template <int B, int G, int R, bool kFirst>
+__device__ __forceinline__ void fft_pass(float *buf, const float2 *tw, int d, int t, int L)
+{
+    constexpr int N = B / 2, T = kFftThreads / G;
+    const int span = L / R;                                    // distance between the R inputs of a butterfly
+    for (int bi = t; bi < N / R; bi += T) {
+        const int j = bi & (span - 1), base = (bi - j) * R + j;  // block start + j
+        float2 x[R];
+#pragma unroll
+        for (int m = 0; m < R; ++m) {
+            const int e = base + m * span;
+            if (kFirst) {
+                const uint32_t *ub = reinterpret_cast<const uint32_t *>(buf);
+                x[m] = make_float2((float)ub[(2 * e) * G + d], (float)ub[(2 * e + 1) * G + d]);
+            } else {
+                x[m] = make_float2(buf[(2 * e) * G + d], buf[(2 * e + 1) * G + d]);
+            }
+        }
+        dft<R>(x);
+        const int tstep = j * (B / L);                          // w_L^{j q} = w_B^{j q B / L}
+#pragma unroll
+        for (int q = 0; q < R; ++q) {
+            const float2 y = (q == 0 || L == R) ? x[q] : cmul(x[q], twiddle<B>(tw, tstep * q));
+            const int e = base + q * span;
+            buf[(2 * e) * G + d] = y.x;
+            buf[(2 * e + 1) * G + d] = y.y;
+        }
+    }
+}
+
+// position of frequency k after the passes (radices 8, 8[, 8][, 2|4]): digit reversal in mixed radix
+template <int B>
+__device__ __forceinline__ int fft_pos(int k)
+{
+    constexpr int N = B / 2;
+    constexpr int kP8 = (N >= 512) ? 3 : 2;
+    int rem = N, pos = 0;
+#pragma unroll
+    for (int p = 0; p < kP8; ++p) {
+        rem >>= 3;
+        pos += (k & 7) * rem;
+        k >>= 3;
+    }
+    return pos + k;                                             // last digit (radix rem = 1, 2 or 4) has weight 1
+}
 
 // Gather (step a2): every warp walks x-rows of cells (contiguous in the sorted array), keeps ions with
-// r^2 <= R2 and appends d = p - c to shared SoA arrays.  Returns the ROI ion count in *s_n (may exceed cap;
-// then only the first cap are stored and the caller must use the streaming path).
-__device__ __forceinline__ void gather_roi(const float4 *__restrict__ sorted, const uint32_t *__restrict__ cell_start,
-                                           const GridParams &g, const RoiCells &rc, float cx, float cy, float cz,
-                                           float R2, float *sx, float *sy, float *sz, int cap, int *s_n)
+// r^2 <= R2 and appends d = p - c as a packed 12-byte record.  *s_n may exceed cap (then the streaming path is used).
+__device__ __forceinline__ void gather_roi(const FftParams &p, const GridParams &g, const RoiCells &rc,
+                                           float cx, float cy, float cz, float *ions, int *s_n)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int ny_r = rc.iy1 - rc.iy0 + 1, nz_r = rc.iz1 - rc.iz0 + 1;
-    for (int row = wid; row < ny_r * nz_r; row += kWarps) {
+    for (int row = wid; row < ny_r * nz_r; row += kFftWarps) {
         int iy = rc.iy0 + row % ny_r, iz = rc.iz0 + row / ny_r;
         int base = (iz * g.ny + iy) * g.nx;
-        uint32_t beg = cell_start[base + rc.ix0], end = cell_start[base + rc.ix1 + 1];
+        uint32_t beg = p.cell_start[base + rc.ix0], end = p.cell_start[base + rc.ix1 + 1];
         for (uint32_t i = beg + lane; i < ((end - beg + 31u) & ~31u) + beg; i += 32) {
             bool in = false;
             float dx = 0.f, dy = 0.f, dz = 0.f;
             if (i < end) {
-                float4 p = sorted[i];
-                dx = __fsub_rn(p.x, cx); dy = __fsub_rn(p.y, cy); dz = __fsub_rn(p.z, cz);
-                in = inside(dx, dy, dz, R2);
+                float4 q = p.sorted[i];
+                dx = __fsub_rn(q.x, cx); dy = __fsub_rn(q.y, cy); dz = __fsub_rn(q.z, cz);
+                in = inside(dx, dy, dz, p.R2);
             }
-            unsigned m = __ballot_sync(0xffffffffu, in);
-            if (m) {
+            unsigned msk = __ballot_sync(0xffffffffu, in);
+            if (msk) {
                 int pos = 0;
-                if (lane == 0) pos = atomicAdd(s_n, __popc(m));
-                pos = __shfl_sync(0xffffffffu, pos, 0) + __popc(m & ((1u << lane) - 1u));
-                if (in && pos < cap) { sx[pos] = dx; sy[pos] = dy; sz[pos] = dz; }
+                if (lane == 0) pos = atomicAdd(s_n, __popc(msk));
+                pos = __shfl_sync(0xffffffffu, pos, 0) + __popc(msk & ((1u << lane) - 1u));
+                if (in && pos < p.cap) { ions[3 * pos] = dx; ions[3 * pos + 1] = dy; ions[3 * pos + 2] = dz; }
             }
         }
     }
 }
 
-template <bool kStream>
-__device__ __forceinline__ void bin_direction(uint32_t *hist, float npx, float npy, float npz, float half_b,
-                                              float magic, const float *sx, const float *sy, const float *sz, int n,
-                                              const float4 *__restrict__ sorted, const uint32_t *__restrict__ cell_start,
-                                              const GridParams &g, const RoiCells &rc, float cx, float cy, float cz,
-                                              float R2)
+template <int B>
+__global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const FftParams p)
 {
-    const int lane = threadIdx.x & 31;
-    if (!kStream) {
-        for (int i = lane; i < n; i += 32)
-            atomicAdd(&hist[bin_of(npx, npy, npz, sx[i], sy[i], sz[i], half_b, magic)], 1u);
-    } else {
-        // ROI larger than the shared-memory ion buffer: stream the cell rows again for every direction
-        const int ny_r = rc.iy1 - rc.iy0 + 1, nz_r = rc.iz1 - rc.iz0 + 1;
-        for (int row = 0; row < ny_r * nz_r; ++row) {
-            int iy = rc.iy0 + row % ny_r, iz = rc.iz0 + row / ny_r;
-            int base = (iz * g.ny + iy) * g.nx;
-            uint32_t beg = cell_start[base + rc.ix0], end = cell_start[base + rc.ix1 + 1];
-            for (uint32_t i = beg + lane; i < end; i += 32) {
-                float4 p = sorted[i];
-                float dx = __fsub_rn(p.x, cx), dy = __fsub_rn(p.y, cy), dz = __fsub_rn(p.z, cz);
-                if (inside(dx, dy, dz, R2)) atomicAdd(&hist[bin_of(npx, npy, npz, dx, dy, dz, half_b, magic)], 1u);
-            }
-        }
-    }
-}
-
-// In-place radix-2 decimation-in-frequency FFT of N = B/2 complex points held by one warp in shared
-// memory; output in bit-reversed order.  tw[r] = exp(-2 pi i r / B), r < B/2.
-__device__ __forceinline__ void warp_fft_dif(float2 *z, const float2 *__restrict__ tw, int N, int B)
-{
-    const int lane = threadIdx.x & 31;
-    for (int half = N >> 1; half >= 1; half >>= 1) {
-        const int tstep = B / (2 * half);
-        for (int t = lane; t < (N >> 1); t += 32) {
-            int pos = t & (half - 1);
-            int i0 = ((t - pos) << 1) + pos;
-            float2 a = z[i0], b = z[i0 + half];
-            float2 w = tw[pos * tstep];
-            float dr = a.x - b.x, di = a.y - b.y;
-            z[i0] = make_float2(a.x + b.x, a.y + b.y);
-            z[i0 + half] = make_float2(dr * w.x - di * w.y, dr * w.y + di * w.x);
-        }
-        __syncwarp();
-    }
-}
-
-__global__ void __launch_bounds__(kThreads)
-k_signature_fft(const float4 *__restrict__ sorted, const uint32_t *__restrict__ cell_start,
-                const GridParams *__restrict__ gp, const float *__restrict__ centres,
-                const float *__restrict__ dirs_scaled, const float2 *__restrict__ g_tw,
-                float2 *__restrict__ sig, uint32_t *__restrict__ counts,
-                int D, int B, int k_lo, int k_hi, float R, float R2, int cap, int nchunks,
-                const uint32_t *__restrict__ list)
-{
+    constexpr int G = (B <= 1024) ? 32 : 32768 / B;            // directions per group
+    constexpr int N = B / 2, T = kFftThreads / G, LPD = 32 / G; // threads per direction, ions per warp instruction
+    constexpr int kP8 = (N >= 512) ? 3 : 2;                    // radix-8 passes
+    constexpr int kLast = N >> (3 * kP8);                      // remaining radix: 1, 2 or 4
     extern __shared__ __align__(16) unsigned char smem[];
-    uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem);                       // [kWarps][B]
-    float2 *s_tw = reinterpret_cast<float2 *>(s_hist + (size_t)kWarps * B);        // [B/2]
-    float2 *s_res = s_tw + B / 2;                                                 // [kDirChunk]
-    float *sx = reinterpret_cast<float *>(s_res + kDirChunk);                     // [cap] x3
-    float *sy = sx + cap, *sz = sy + cap;
+    float *buf = reinterpret_cast<float *>(smem);                                  // [B][G] counts, then the transform
+    float2 *s_tw = reinterpret_cast<float2 *>(buf + (size_t)B * G);                // [B/2]
+    float2 *cand = s_tw + B / 2;                                                   // [T][G]
+    float *ions = reinterpret_cast<float *>(cand + T * G);                         // [cap][3]
     __shared__ int s_n;
 
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    for (int i = threadIdx.x; i < B / 2; i += kThreads) s_tw[i] = g_tw[i];
-    // direct mode: one work item (material point, direction chunk) per CTA.  list mode: the grid is
-    // persistent and walks the items of the material points named in list[1 .. list[0]].
-    const int64_t n_items = list ? (int64_t)list[0] * nchunks : (int64_t)gridDim.x;
-    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
-    const int64_t m = list ? (int64_t)list[1 + item / nchunks] : item / nchunks;
-    const int chunk = (int)(item % nchunks);
-    const int d_begin = chunk * kDirChunk, d_end = min(D, d_begin + kDirChunk);
-    const GridParams g = *gp;
-    const float cx = centres[3 * m], cy = centres[3 * m + 1], cz = centres[3 * m + 2];
-    const RoiCells rc = roi_cells(g, cx, cy, cz, R);
-
-    __syncthreads();                 // previous item fully written out; s_tw loaded
-    if (threadIdx.x == 0) s_n = 0;
-    __syncthreads();
-    if (g.n_accepted) gather_roi(sorted, cell_start, g, rc, cx, cy, cz, R2, sx, sy, sz, cap, &s_n);
-    __syncthreads();
-    const int n = s_n;
-    if (chunk == 0 && threadIdx.x == 0 && counts) counts[m] = (uint32_t)n;
-    const bool stream = n > cap;
-
-    const int N = B >> 1;
-    const int logN = 31 - __clz(N);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int d = lane % G, t = warp * LPD + lane / G;                             // direction slot, thread index within it
+    for (int i = tid; i < B / 2; i += kFftThreads) s_tw[i] = p.tw[i];
+    const GridParams g = *p.grid;
     const float half_b = (float)(B / 2), magic = magic_for(B);
-    uint32_t *hist = s_hist + (size_t)wid * B;
-    float *hf = reinterpret_cast<float *>(hist);
-    float2 *z = reinterpret_cast<float2 *>(hist);
 
-    for (int d = d_begin + wid; d < d_end; d += kWarps) {
-        for (int j = lane; j < B; j += 32) hist[j] = 0u;
-        __syncwarp();
-        const float npx = dirs_scaled[3 * d], npy = dirs_scaled[3 * d + 1], npz = dirs_scaled[3 * d + 2];
-        if (!stream)
-            bin_direction<false>(hist, npx, npy, npz, half_b, magic, sx, sy, sz, n, sorted, cell_start, g, rc, cx, cy, cz, R2);
-        else
-            bin_direction<true>(hist, npx, npy, npz, half_b, magic, sx, sy, sz, n, sorted, cell_start, g, rc, cx, cy, cz, R2);
-        __syncwarp();
-        // counts -> float in place: z[j] = (h[2j], h[2j+1]) packs the real sequence into N complex points
-        for (int j = lane; j < B; j += 32) hf[j] = (float)hist[j];
-        __syncwarp();
-        warp_fft_dif(z, s_tw, N, B);
-        // unpack the window: X_k = (Z_k + conj Z_{N-k})/2 - i e^{-2 pi i k/B} (Z_k - conj Z_{N-k})/2
-        float best = -1.0f;
-        int kbest = k_lo;
-        for (int k = k_lo + lane; k <= k_hi; k += 32) {
-            int ka = k & (N - 1), kb = (N - k) & (N - 1);
-            float2 za = z[__brev((unsigned)ka) >> (32 - logN)];
-            float2 zb = z[__brev((unsigned)kb) >> (32 - logN)];
-            float2 w = (k < N) ? s_tw[k] : make_float2(-1.0f, 0.0f);
-            float er = za.x + zb.x, ei = za.y - zb.y;          // Z_k + conj Z_{N-k}
-            float orr = za.x - zb.x, oi = za.y + zb.y;         // Z_k - conj Z_{N-k}
-            // -i * w * (orr + i oi) = (w.y*orr + w.x*oi) + i (w.y*oi - w.x*orr)
-            float xr = er + (w.y * orr + w.x * oi);
-            float xi = ei + (w.y * oi - w.x * orr);
-            float pw = xr * xr + xi * xi;                       // 4 |X_k|^2
-            if (pw > best) { best = pw; kbest = k; }            // ascending k per lane: lowest k kept on ties
+    // direct mode: one (material point, chunk) per CTA.  list mode: a persistent grid walks the items of the
+    // material points named in list[1 .. list[0]].
+    const int64_t n_items = p.list ? (int64_t)p.list[0] * p.nchunks : (int64_t)gridDim.x;
+    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const int64_t m = p.list ? (int64_t)p.list[1 + item / p.nchunks] : item / p.nchunks;
+        const int chunk = (int)(item % p.nchunks);
+        const int g_begin = (int)((int64_t)chunk * p.ngroups / p.nchunks);
+        const int g_end = (int)((int64_t)(chunk + 1) * p.ngroups / p.nchunks);
+        const float cx = p.centres[3 * m], cy = p.centres[3 * m + 1], cz = p.centres[3 * m + 2];
+        const RoiCells rc = roi_cells(g, cx, cy, cz, p.R);
+
+        __syncthreads();                 // previous item done with the shared buffers; s_tw loaded
+        if (tid == 0) s_n = 0;
+        __syncthreads();
+        if (g.n_accepted) gather_roi(p, g, rc, cx, cy, cz, ions, &s_n);
+        __syncthreads();
+        const int n = s_n;
+        if (chunk == 0 && tid == 0 && p.counts) p.counts[m] = (uint32_t)n;
+        const bool stream = n > p.cap;
+
+        for (int gi = g_begin; gi < g_end; ++gi) {
+            // ---- clear the counters -----------------------------------------------------------------
+            {
+                uint4 *h = reinterpret_cast<uint4 *>(buf);
+                for (int i = tid; i < B * G / 4; i += kFftThreads) h[i] = make_uint4(0, 0, 0, 0);
+            }
+            __syncthreads();
+            // ---- project-and-bin (step a4): lane = direction, the T threads of a direction split the ions --
+            {
+                const int dg = min(gi * G + d, p.D - 1);
+                const float npx = p.dirs_scaled[3 * dg], npy = p.dirs_scaled[3 * dg + 1], npz = p.dirs_scaled[3 * dg + 2];
+                uint32_t *cnt = reinterpret_cast<uint32_t *>(buf) + d;
+                if (!stream) {
+                    for (int i = t; i < n; i += T)
+                        atomicAdd(cnt + bin_of(npx, npy, npz, ions[3 * i], ions[3 * i + 1], ions[3 * i + 2], half_b, magic) * G, 1u);
+                } else {
+                    // ROI larger than the shared ion buffer: walk the cell rows again, one ion per (warp, lane / G)
+                    const int ny_r = rc.iy1 - rc.iy0 + 1, nz_r = rc.iz1 - rc.iz0 + 1;
+                    for (int row = warp; row < ny_r * nz_r; row += kFftWarps) {
+                        const int iy = rc.iy0 + row % ny_r, iz = rc.iz0 + row / ny_r;
+                        const int base = (iz * g.ny + iy) * g.nx;
+                        const uint32_t beg = p.cell_start[base + rc.ix0], end = p.cell_start[base + rc.ix1 + 1];
+                        for (uint32_t i = beg + lane / G; i < end; i += LPD) {
+                            const float4 q = p.sorted[i];
+                            const float dx = __fsub_rn(q.x, cx), dy = __fsub_rn(q.y, cy), dz = __fsub_rn(q.z, cz);
+                            if (inside(dx, dy, dz, p.R2)) atomicAdd(cnt + bin_of(npx, npy, npz, dx, dy, dz, half_b, magic) * G, 1u);
+                        }
+                    }
+                }
+            }
+            __syncthreads();
+            // ---- packed real FFT (step a5): radix-8 DIF passes in place, then the remaining radix 2 / 4 ----
+            fft_pass<B, G, 8, true>(buf, s_tw, d, t, N);
+            __syncthreads();
+            fft_pass<B, G, 8, false>(buf, s_tw, d, t, N / 8);
+            __syncthreads();
+            if (kP8 == 3) {
+                fft_pass<B, G, 8, false>(buf, s_tw, d, t, N / 64);
+                __syncthreads();
+            }
+            if (kLast > 1) {
+                fft_pass<B, G, (kLast > 1 ? kLast : 2), false>(buf, s_tw, d, t, kLast);
+                __syncthreads();
+            }
+            // ---- split step on the window + arg-max (steps a5 tail, a6) ------------------------------------
+            float best = -1.0f;
+            int kbest = p.k_lo;
+            for (int k = p.k_lo + t; k <= p.k_hi; k += T) {
+                const int ea = fft_pos<B>(k & (N - 1)), eb = fft_pos<B>((N - k) & (N - 1));
+                const float2 za = make_float2(buf[(2 * ea) * G + d], buf[(2 * ea + 1) * G + d]);
+                const float2 zb = make_float2(buf[(2 * eb) * G + d], buf[(2 * eb + 1) * G + d]);
+                const float2 w = (k < N) ? s_tw[k] : make_float2(-1.0f, 0.0f);
+                const float er = za.x + zb.x, ei = za.y - zb.y;          // Z_k + conj Z_{N-k}
+                const float orr = za.x - zb.x, oi = za.y + zb.y;         // Z_k - conj Z_{N-k}
+                // -i * w * (orr + i oi) = (w.y*orr + w.x*oi) + i (w.y*oi - w.x*orr)
+                const float xr = er + (w.y * orr + w.x * oi);
+                const float xi = ei + (w.y * oi - w.x * orr);
+                const float pw = xr * xr + xi * xi;                       // 4 |X_k|^2
+                if (pw > best) { best = pw; kbest = k; }                  // ascending k per thread: lowest k kept on ties
+            }
+            cand[t * G + d] = make_float2(best, __int_as_float(kbest));
+            __syncthreads();
+            if (tid < G) {
+                float bb = -1.0f;
+                int kb = p.k_lo;
+                for (int s = 0; s < T; ++s) {
+                    const float2 c = cand[s * G + tid];
+                    const int ck = __float_as_int(c.y);
+                    if (c.x > bb || (c.x == bb && ck < kb)) { bb = c.x; kb = ck; }
+                }
+                const int dg = gi * G + tid;
+                if (dg < p.D) p.sig[(size_t)m * p.D + dg] = make_float2(0.5f * sqrtf(fmaxf(bb, 0.0f)), (float)kb);
+            }
+            // the next group's clear of buf is ordered after this group's reads by the barrier above; cand is
+            // rewritten only after three more barriers
         }
-#pragma unroll
-        for (int o = 16; o; o >>= 1) {
-            float ob = __shfl_xor_sync(0xffffffffu, best, o);
-            int ok = __shfl_xor_sync(0xffffffffu, kbest, o);
-            if (ob > best || (ob == best && ok < kbest)) { best = ob; kbest = ok; }
-        }
-        if (lane == 0) s_res[d - d_begin] = make_float2(0.5f * sqrtf(fmaxf(best, 0.0f)), (float)kbest);
-        __syncwarp();
-    }
-    __syncthreads();
-    float2 *out = sig + (size_t)m * D + d_begin;
-    for (int i = threadIdx.x; i < d_end - d_begin; i += kThreads) out[i] = s_res[i];
     }
 }
 
-static int fft_cap_for(int B) { return B <= 1024 ? 3072 : (B == 2048 ? 2688 : 4096); }
+static int fft_groups_of(int B) { return B <= 1024 ? 32 : 32768 / B; }
+static size_t fft_smem_for(int B, int cap)
+{
+    const int G = fft_groups_of(B), T = kFftThreads / G;
+    return (size_t)B * G * 4 + (size_t)(B / 2) * 8 + (size_t)T * G * 8 + (size_t)cap * 12;
+}
+static int fft_cap_for(int B)
+{
+    const size_t budget = 232448 - 256;
+    return (int)(((budget - fft_smem_for(B, 0)) / 12) & ~(size_t)63);
+}
 
 static cudaError_t launch_fft_common(Plan *p, const float *centres, int64_t M, const uint32_t *list, float *sig,
                                      uint32_t *counts, cudaStream_t st)
 {
-    const int B = p->B, cap = fft_cap_for(B);
-    const int nchunks = (p->D + kDirChunk - 1) / kDirChunk;
-    size_t smem = (size_t)kWarps * B * 4 + (size_t)(B / 2) * 8 + (size_t)kDirChunk * 8 + (size_t)cap * 12;
-    cudaError_t e = cudaFuncSetAttribute(k_signature_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    int64_t blocks = list ? (int64_t)p->sm_count * 2 : M * nchunks;
+    const int B = p->B, G = fft_groups_of(B);
+    FftParams q;
+    q.sorted = p->d_sorted; q.cell_start = p->d_cell_start; q.grid = p->d_grid; q.centres = centres;
+    q.dirs_scaled = p->d_dirs_scaled; q.tw = p->d_twiddle; q.sig = reinterpret_cast<float2 *>(sig); q.counts = counts;
+    q.list = list; q.D = p->D; q.k_lo = p->k_lo; q.k_hi = p->k_hi; q.cap = fft_cap_for(B);
+    q.ngroups = (p->D + G - 1) / G;
+    // enough CTAs to fill the machine a few times over, but at least a handful of groups per CTA (one gather each)
+    int nchunks = (q.ngroups + 63) / 64;
+    const int64_t want = (int64_t)p->sm_count * 4;
+    const int64_t Mx = list ? 1 : M;
+    if (Mx * nchunks < want) nchunks = (int)((want + Mx - 1) / Mx);
+    if (nchunks > (q.ngroups + 1) / 2) nchunks = (q.ngroups + 1) / 2;
+    if (nchunks < 1) nchunks = 1;
+    q.nchunks = nchunks;
+    q.R = p->R; q.R2 = p->R2;
+    const size_t smem = fft_smem_for(B, q.cap);
+    const int64_t blocks = list ? (int64_t)p->sm_count : M * nchunks;
     if (blocks > 0x7FFFFFFFLL) return cudaErrorInvalidConfiguration;
-    k_signature_fft<<<(unsigned)blocks, kThreads, smem, st>>>(
-        p->d_sorted, p->d_cell_start, p->d_grid, centres, p->d_dirs_scaled, p->d_twiddle,
-        reinterpret_cast<float2 *>(sig), counts, p->D, B, p->k_lo, p->k_hi, p->R, p->R2, cap, nchunks, list);
-    return cudaGetLastError();
+    auto launch = [&](auto kern) -> cudaError_t {
+        cudaError_t le = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (le != cudaSuccess) return le;
+        kern<<<(unsigned)blocks, kFftThreads, smem, st>>>(q);
+        return cudaGetLastError();
+    };
+    switch (B) {
+        case 256: return launch(k_signature_fft<256>);
+        case 512: return launch(k_signature_fft<512>);
+        case 1024: return launch(k_signature_fft<1024>);
+        case 2048: return launch(k_signature_fft<2048>);
+        case 4096: return launch(k_signature_fft<4096>);
+        default: return cudaErrorInvalidValue;
+    }
 }
 
 cudaError_t launch_signature_fft(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts,

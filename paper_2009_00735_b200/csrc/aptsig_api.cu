@@ -115,6 +115,18 @@ extern "C" int apx_plan_create(const apx_plan_desc *desc, apx_plan **out)
     CUF(cudaMemcpy(p->d_type_mask, mask, 32, cudaMemcpyHostToDevice));
     CUF(cudaStreamCreateWithFlags(&p->own_stream, cudaStreamNonBlocking));
 
+    // the clamp of Eq. 1's bin index can be skipped when it provably never triggers: paper padding (pad = 1) and
+    // directions that are unit vectors to fp32 accuracy => |x| <= (B/2-1)(1+2e-5) < B/2 - 0.25
+    {
+        bool unit = p->pad == 1;
+        const double lim = (double)p->s * 1.00001;
+        for (int d = 0; d < p->D && unit; ++d) {
+            const double nn = std::sqrt((double)nps[3 * d] * nps[3 * d] + (double)nps[3 * d + 1] * nps[3 * d + 1] +
+                                        (double)nps[3 * d + 2] * nps[3 * d + 2]);
+            if (!(nn <= lim)) unit = false;
+        }
+        p->need_clamp = unit ? 0 : 1;
+    }
     p->path = 0;
     if (!(desc->flags & APX_FLAG_FORCE_FFT) && mma_path_supported(p)) {
         CUF(mma_path_prepare(p));

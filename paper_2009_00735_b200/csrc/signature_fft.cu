@@ -32,7 +32,7 @@ struct FftParams {
     float2 *sig;
     uint32_t *counts;
     const uint32_t *list;      // nullptr = direct mode; else list[0] = count, list[1..] = material point ids
-    int D, k_lo, k_hi, cap, nchunks, ngroups;
+    int D, k_lo, k_hi, cap, nchunks, ngroups, clamp;
     float R, R2;
 };
 
@@ -208,7 +208,22 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const FftParam
                 const float npx = p.dirs_scaled[3 * dg], npy = p.dirs_scaled[3 * dg + 1], npz = p.dirs_scaled[3 * dg + 2];
                 uint32_t *cnt = reinterpret_cast<uint32_t *>(buf) + d;
                 if (!stream) {
-                    for (int i = t; i < n; i += T)
+                    // thread t takes ions t, t+T, ...; four independent chains per iteration
+                    const uint32_t cb = (uint32_t)__cvta_generic_to_shared(cnt) - 0x4B400000u * (uint32_t)(4 * G);
+                    int i = t;
+                    for (; i + 3 * T < n; i += 4 * T) {
+                        float3 q[4];
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) q[u] = make_float3(ions[3 * (i + u * T)], ions[3 * (i + u * T) + 1], ions[3 * (i + u * T) + 2]);
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            float x = __fmaf_rn(npz, q[u].z, __fmaf_rn(npy, q[u].y, __fmul_rn(npx, q[u].x)));
+                            if (p.clamp) x = fminf(fmaxf(x, -half_b), half_b - 0.25f);
+                            const uint32_t ua = __float_as_uint(__fadd_rd(x, magic));
+                            asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(ua * (uint32_t)(4 * G) + cb), "r"(1u) : "memory");
+                        }
+                    }
+                    for (; i < n; i += T)
                         atomicAdd(cnt + bin_of(npx, npy, npz, ions[3 * i], ions[3 * i + 1], ions[3 * i + 2], half_b, magic) * G, 1u);
                 } else {
                     // ROI larger than the shared ion buffer: walk the cell rows again, one ion per (warp, lane / G)
@@ -304,6 +319,7 @@ static cudaError_t launch_fft_common(Plan *p, const float *centres, int64_t M, c
     if (nchunks < 1) nchunks = 1;
     q.nchunks = nchunks;
     q.R = p->R; q.R2 = p->R2;
+    q.clamp = p->need_clamp;
     const size_t smem = fft_smem_for(B, q.cap);
     const int64_t blocks = list ? (int64_t)p->sm_count : M * nchunks;
     if (blocks > 0x7FFFFFFFLL) return cudaErrorInvalidConfiguration;

@@ -536,17 +536,6 @@ cudaError_t mma_path_prepare(Plan *p)
     std::vector<float> nps((size_t)3 * p->D);
     e = cudaMemcpy(nps.data(), p->d_dirs_scaled, nps.size() * 4, cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) return e;
-    // the clamp of Eq. 1's bin index can be skipped when it provably never triggers: paper padding
-    // (pad = 1) and directions that are unit vectors to fp32 accuracy => |x| <= (B/2-1)(1+2e-5) < B/2 - 0.25
-    bool unit = p->pad == 1;
-    const double lim = (double)p->s * 1.00001;
-    for (int d = 0; d < p->D && unit; ++d) {
-        double nn = std::sqrt((double)nps[3 * d] * nps[3 * d] + (double)nps[3 * d + 1] * nps[3 * d + 1] +
-                              (double)nps[3 * d + 2] * nps[3 * d + 2]);
-        if (!(nn <= lim)) unit = false;
-    }
-    p->mma_clamp = unit ? 0 : 1;
-
     // patch order + padding to a multiple of 32 (padding slots repeat the last direction, perm = -1)
     std::vector<int> idx(p->D);
     std::iota(idx.begin(), idx.end(), 0);
@@ -599,7 +588,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     if (nchunks > (q.ngroups + 1) / 2) nchunks = (q.ngroups + 1) / 2;
     if (nchunks < 1) nchunks = 1;
     q.nchunks = nchunks;
-    q.clamp = p->mma_clamp;
+    q.clamp = p->need_clamp;
     uint32_t cols = 32;
     while (cols < (uint32_t)(2 * q.N)) cols *= 2;
     q.tmem_cols = cols;

@@ -1,0 +1,113 @@
+"""GPU parity on the edge cases of the path: empty inputs, ROIs that overflow the kernels' shared-memory ion
+buffers (deferred list, streaming fallback, multi-pass binning), every B the ABI admits, pad = 0 with the bin
+clamp active, non-unit directions, ragged direction counts.  Same comparator and tolerances as test_gpu_parity."""
+from types import SimpleNamespace
+
+import numpy as np
+import pytest
+
+import paper_2009_00735_b200 as apx
+from oracle import oracle as O
+from workloads.lattices import fcc_basis, lattice_in_ball, random_rotation, jitter_thin_shuffle
+from workloads.configs import A_AL, window_for
+from _parity import run_gpu, assert_parity
+
+pytestmark = pytest.mark.gpu
+PATHS = [pytest.param(apx.APX_FLAG_FORCE_FFT, id="fft"), pytest.param(0, id="auto")]
+
+
+def _ball(R_cloud, eta=1.0, sigma=0.0, seed=7):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    rot = random_rotation(rng)
+    sites = lattice_in_ball(A_AL, fcc_basis, rot, (0, 0, 0), R_cloud)
+    xyz, _, _, _ = jitter_thin_shuffle(sites, rng, eta, sigma)
+    return xyz, np.zeros(len(xyz), np.uint8)
+
+
+def _case(xyz, types, R, B):
+    return SimpleNamespace(xyz=xyz, types=types, R=R, B=B)
+
+
+def _check(w, dirs, centres, window, flags, pad=1):
+    got, cnt, path = run_gpu(apx, w, dirs, centres, window=window, flags=flags, pad=pad)
+    k_lo, k_hi = window if window else (0, 0)
+    ref, rc, win = O.signatures(w.xyz, w.types, centres, dirs, w.R, w.B, pad=pad, k_lo=k_lo, k_hi=k_hi, want_window=True)
+    assert_parity(got, cnt, ref, rc, win, k_lo if window else 1)
+    return path, cnt
+
+
+@pytest.mark.parametrize("flags", PATHS)
+def test_empty_cloud_and_no_centres(flags):
+    import torch
+    dirs = O.dirs_fibonacci(100)
+    plan = apx.Plan(1.0, 256, dirs, k_lo=7, k_hi=17, device=0, flags=flags)
+    dev = torch.device("cuda:0")
+    xyz = torch.zeros((0, 3), dtype=torch.float32, device=dev)
+    centres = torch.tensor([[0.0, 0.0, 0.0], [1.0, 2.0, 3.0]], dtype=torch.float32, device=dev)
+    sig = torch.full((2, 100, 2), -7.0, dtype=torch.float32, device=dev)
+    counts = torch.full((2,), 9, dtype=torch.int32, device=dev)
+    plan.apx_run(xyz, None, centres, sig, counts)                 # N = 0: every ROI empty
+    plan.apx_query(centres[:0], sig[:0], counts[:0])              # M = 0 is valid
+    torch.cuda.synchronize()
+    assert (counts.cpu().numpy() == 0).all()
+    s = sig.cpu().numpy()
+    assert (s[..., 0] == 0.0).all() and (s[..., 1] == 7.0).all()   # empty ROI: (0, k_lo)
+    plan.apx_plan_destroy()
+
+
+@pytest.mark.parametrize("flags", PATHS)
+def test_dense_roi_overflows_mma_ion_buffer(flags):
+    """Noiseless full-density fcc Al, R = 2.2 nm: ~2700 ions per ROI > the MMA kernel's shared ion buffer at
+    B = 1024, so the auto path defers these material points to the FFT kernel."""
+    xyz, types = _ball(3.0)
+    dirs = O.dirs_fibonacci(200)
+    centres = np.array([[0, 0, 0], [0.3, -0.2, 0.1], [2.5, 0, 0]], np.float32)    # the last one is a partial ROI
+    w = _case(xyz, types, 2.2, 1024)
+    path, cnt = _check(w, dirs, centres, window_for(2.2, 1024), flags)
+    assert cnt[0] > 2048
+
+
+def test_multipass_binning_mma_b256():
+    """B = 256 leaves room for 4096 ions in the MMA kernel: a ROI with more than 2048 ions is binned in two passes
+    (u16 counters read as fp16 are exact up to 2048) that accumulate in TMEM."""
+    xyz, types = _ball(3.0)
+    dirs = O.dirs_fibonacci(96)
+    centres = np.array([[0, 0, 0], [0.2, 0.1, -0.3]], np.float32)
+    w = _case(xyz, types, 2.2, 256)
+    path, cnt = _check(w, dirs, centres, window_for(2.2, 256), 0)
+    assert path == 1 and cnt.min() > 2048
+
+
+def test_streaming_fallback_fft():
+    """ROI larger than the FFT kernel's shared ion buffer (~6900 ions at B = 1024): cell rows are streamed again
+    for every direction group."""
+    xyz, types = _ball(4.0)
+    dirs = O.dirs_fibonacci(64)
+    centres = np.array([[0, 0, 0]], np.float32)
+    w = _case(xyz, types, 3.3, 1024)
+    path, cnt = _check(w, dirs, centres, (20, 60), apx.APX_FLAG_FORCE_FFT)
+    assert cnt[0] > 7500
+
+
+@pytest.mark.parametrize("flags", PATHS)
+@pytest.mark.parametrize("B", [256, 512, 1024, 2048, 4096])
+def test_every_bin_count(flags, B):
+    xyz, types = _ball(1.6, eta=0.6, sigma=0.04, seed=11)
+    dirs = O.dirs_fibonacci(77)                                    # ragged: not a multiple of 32 / 16 / 8
+    centres = np.array([[0, 0, 0], [0.4, 0.4, -0.2]], np.float32)
+    w = _case(xyz, types, 1.2, B)
+    _check(w, dirs, centres, window_for(1.2, B), flags)
+    if B <= 512:
+        _check(w, dirs[:40], centres, None, flags)                 # full window [1, B/2]
+
+
+@pytest.mark.parametrize("flags", PATHS)
+def test_pad0_and_non_unit_directions_clamp(flags):
+    """pad = 0 (north_star's [-R, R]) puts ions on the last bin edge, and directions 3 % longer than unit push
+    projections past +-R: the bin clamp of Eq. 1 (reading #5) must act on both paths."""
+    xyz, types = _ball(1.6, eta=0.7, sigma=0.03, seed=13)
+    dirs = (O.dirs_fibonacci(64).astype(np.float64) * 1.03).astype(np.float32)
+    centres = np.array([[0, 0, 0]], np.float32)
+    w = _case(xyz, types, 1.2, 512)
+    _check(w, dirs, centres, (5, 20), flags, pad=0)
+    _check(w, dirs, centres, (5, 20), flags, pad=1)

@@ -95,3 +95,56 @@ def test_cfg4_sample(flags):
     got, cnt, _ = run_gpu(apx, w, dirs, centres, window=w.window, flags=flags)
     ref, rc, rwin, klo = _oracle(w, dirs, centres, w.window)
     assert_parity(got, cnt, ref, rc, rwin, klo)
+
+
+def _full_launch(w, dirs, accepted=None):
+    """The whole config in ONE apx_run (the launch configuration bench.py times); results stay on the device."""
+    import torch
+    dev = torch.device("cuda:0")
+    plan = apx.Plan(w.R, w.B, dirs, k_lo=w.window[0], k_hi=w.window[1], accepted_types=accepted, device=0)
+    xyz = torch.from_numpy(w.xyz).to(dev)
+    types = torch.from_numpy(w.types).to(dev)
+    c = torch.from_numpy(w.centres).to(dev)
+    M = c.shape[0]
+    sig = torch.full((M, len(dirs), 2), -7.0, dtype=torch.float32, device=dev)
+    counts = torch.full((M,), -1, dtype=torch.int32, device=dev)
+    plan.apx_run(xyz, types, c, sig, counts)
+    torch.cuda.synchronize()
+    plan.apx_plan_destroy()
+    return sig, counts
+
+
+def _check_full(w, dirs, sig, counts, idx, accepted=None):
+    import torch
+    M = len(w.centres)
+    # every material point: ROI ion count against the oracle's brute force (one direction is enough for counts)
+    _, rc_all = O.signatures(w.xyz, w.types, w.centres, dirs[:1], w.R, w.B, k_lo=w.window[0], k_hi=w.window[1],
+                             accepted=accepted)
+    cnt = counts.cpu().numpy().astype(np.uint32)
+    assert (cnt == rc_all).all()
+    # properties that hold for every output: 0 <= A <= N_c (P4), k inside the window, nothing left unwritten
+    amp, k = sig[..., 0], sig[..., 1]
+    assert bool((amp >= 0).all()) and bool((amp <= counts.to(torch.float32)[:, None] * (1 + 1e-5) + 1e-3).all())
+    assert bool((k >= w.window[0]).all()) and bool((k <= w.window[1]).all())
+    # sampled material points x all directions, element by element
+    got = sig[torch.from_numpy(idx).cuda()].cpu().numpy()
+    ref, rc, rwin = O.signatures(w.xyz, w.types, w.centres[idx], dirs, w.R, w.B, k_lo=w.window[0], k_hi=w.window[1],
+                                 accepted=accepted, want_window=True)
+    assert_parity(got, cnt[idx], ref, rc, rwin, w.window[0])
+
+
+def test_cfg2_full_size_bench_launch():
+    w = make_config(2)
+    dirs = O.dirs_fibonacci(w.D)
+    sig, counts = _full_launch(w, dirs)
+    _check_full(w, dirs, sig, counts, np.array([0, 99, 137, 455, 500, 555, 900, 999]))
+
+
+def test_cfg3_full_size_al_filter():
+    """Config 3 at full size (27 000 material points x 40 962 geodesic directions, 8.85 GB of signatures), Al filter."""
+    w = make_config(3)
+    dirs = O.dirs_geodesic(6)
+    sig, counts = _full_launch(w, dirs, accepted={0})
+    g = np.arange(27000).reshape(30, 30, 30)
+    idx = np.array([g[14, 10, 10], g[15, 10, 10], g[0, 0, 0], g[29, 15, 3], g[3, 20, 20], g[7, 7, 29]])
+    _check_full(w, dirs, sig, counts, idx, accepted={0})

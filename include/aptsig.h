@@ -88,8 +88,10 @@ int apx_query(apx_plan *plan, const float *centres, int64_t M, float *sig, uint3
 int apx_run(apx_plan *plan, const float *xyz, const uint8_t *types, int64_t N,
             const float *centres, int64_t M, float *sig, uint32_t *counts, void *cuda_stream);
 
-/* Same as apx_run but every array is a HOST pointer; copies in and out on an internal stream and
- * synchronises before returning (the end-to-end entry bench.py's "e2e" figure is timed through). */
+/* Same as apx_run but every array is a HOST pointer (pinned memory makes the copies asynchronous): inputs are
+ * copied in on an internal stream, the material points are processed in up to four slabs, and the signatures of a
+ * slab travel back on a second internal stream while the next slab is computed.  Synchronises before returning
+ * (the end-to-end entry bench.py's "e2e" figure is timed through). */
 int apx_run_host(apx_plan *plan, const float *xyz, const uint8_t *types, int64_t N,
                  const float *centres, int64_t M, float *sig, uint32_t *counts);
 

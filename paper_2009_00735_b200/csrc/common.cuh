@@ -49,7 +49,8 @@ struct Plan {
     float4 *d_sorted;              // [capacity]  (x, y, z, original index bits)
     int64_t capacity;              // ions the sorted buffers can hold
     // host staging for apx_run_host
-    cudaStream_t own_stream;
+    cudaStream_t own_stream, copy_stream;
+    cudaEvent_t slab_done[2];
     void *h2d_xyz, *h2d_types, *h2d_centres, *d2h_sig, *d2h_counts;   // device-side staging
     int64_t cap_xyz, cap_types, cap_centres, cap_sig, cap_counts;
 };

@@ -110,7 +110,7 @@ struct MmaParams {
     float2 *sig;
     uint32_t *counts;
     uint32_t *deferred;        // [0] = count, [1..] = material point ids left to the FFT kernel
-    int D, B, nl, k_lo, W, N, cap, nchunks, ngroups, clamp;
+    int D, B, nl, k_lo, W, N, cap, cap_big, nchunks, ngroups, clamp;
     uint32_t tmem_cols;
     float R, R2;
 };
@@ -126,11 +126,12 @@ __host__ __device__ inline MmaSmem mma_smem_layout(int B, int N, int W, int cap)
     s.hist_bytes = (uint32_t)(B / 32) * kGroupBytes;             // K/8 = B/32 K groups of 2560 B
     s.table = off; off += (uint32_t)(B / 4) * N * 2;             // (K/64) * N * 128 with K = B/4; multiple of 1024
     s.hist0 = off; off += s.hist_bytes;
-    s.hist1 = off; off += s.hist_bytes;
     s.exch = off; off += 2u * kEpiRound * 4 * 32 * 8;             // per set, one epilogue round: 4 bins x 4 blk x 32 slots x float2
     s.cand = off; off += 8u * 32 * 8;
     s.phase = off; off += 4u * W * 8;
     s.ions = off; off += (uint32_t)cap * 12;
+    s.hist1 = off; off += s.hist_bytes;                            // directly behind the ion buffer: a ROI with more than
+                                                                   // `cap` ions spills into it and runs single-buffered
     s.total = off + 1024;                                          // slack for 1024-byte alignment
     return s;
 }
@@ -158,7 +159,7 @@ __device__ __forceinline__ void gather_roi3(const MmaParams &p, const GridParams
                 int pos = 0;
                 if (lane == 0) pos = atomicAdd(s_n, __popc(msk));
                 pos = __shfl_sync(0xffffffffu, pos, 0) + __popc(msk & ((1u << lane) - 1u));
-                if (in && pos < p.cap) { ions[3 * pos] = dx; ions[3 * pos + 1] = dy; ions[3 * pos + 2] = dz; }
+                if (in && pos < p.cap_big) { ions[3 * pos] = dx; ions[3 * pos + 1] = dy; ions[3 * pos + 2] = dz; }
             }
         }
     }
@@ -288,6 +289,111 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
     }
 }
 
+// The warp-specialised pipeline of one (material point, chunk).  kBig: the ROI's ions have spilled into the second
+// histogram buffer, so only buffer 0 is used and bin -> transform -> clear are serial per item.
+template <int KS, bool kBig>
+__device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &L, unsigned char *smem, uint32_t tmem, int n,
+                                             int g_begin, int g_end, int64_t m, const float *ions, const float2 *phase,
+                                             float2 *exch, float2 *cand, uint64_t *s_full, uint64_t *s_done,
+                                             uint64_t *s_free, uint64_t *s_tfree)
+{
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // Pipeline over items = (direction group, ion pass); item it uses histogram buffer it & 1 and the TMEM
+    // accumulator (group & 1):
+    //   binning warps 0..15 : wait free(buf) -> project-and-bin item it -> arrive full(buf)
+    //   MMA warp 16         : wait full(buf) [, tfree(acc)] -> K/16 tcgen05.mma -> commit to done(buf)
+    //   service warps 17..20: wait done(buf) -> clear the buffer -> arrive free(buf); after the last pass of a
+    //                         group: epilogue from TMEM -> arrive tfree(acc)
+    // A ROI with more than `cap` ions has spilled into the second histogram buffer: it runs with buffer 0 only
+    // (bin -> transform -> clear serial per item); `use` counts the uses of a buffer.
+    const int npass = n > 2048 ? (n + 2047) / 2048 : 1;          // fp16 counters are exact up to 2048
+    const int nitems = (g_end - g_begin) * npass;
+    if (warp < kBinWarps) {
+        BinConst c;
+        c.half_b = (float)(p.B / 2); c.magic_a = magic_for(p.B); c.magic_b = 12582912.0f + 4.0f;
+        c.scl = __int_as_float((127 - p.nl) << 23);                       // 2^-nl
+        c.kz = 16u - (uint32_t)kBlkBytes * (1u << p.nl);
+        const int l = lane & 15, hw = warp * 2 + (lane >> 4);             // half-warp index 0..31
+        const uint32_t k0base = smem_u32(smem + L.hist0) + (uint32_t)(l >> 2) * kChunkBytes + (uint32_t)(l & 3) * 4u
+                                - 0x4B400000u * (uint32_t)kBlkBytes - 0x4B400000u * c.kz;
+        const uint32_t ions_s = smem_u32(ions);
+        for (int it = 0; it < nitems; ++it) {
+            const int gl = it / npass, pass = it % npass, buf = kBig ? 0 : (it & 1), use = kBig ? it : (it >> 1);
+            float na[3], nb[3];
+            {
+                const float *da = p.dirs_sorted + (size_t)((g_begin + gl) * 32 + l) * 3;
+                na[0] = da[0]; na[1] = da[1]; na[2] = da[2];
+                nb[0] = da[48]; nb[1] = da[49]; nb[2] = da[50];
+            }
+            if (use >= 1) mbar_wait(&s_free[buf], (uint32_t)((use - 1) & 1));         // cleared after its previous use
+            const int a0 = pass * 2048, a1 = min(n, a0 + 2048);
+            const int per = (((a1 - a0 + 2 * kBinWarps - 1) / (2 * kBinWarps)) + 3) & ~3;
+            const int i0 = min(a1, a0 + hw * per), i1 = min(a1, i0 + per);
+            const uint32_t k0 = k0base + (uint32_t)buf * (L.hist1 - L.hist0);
+            if (p.clamp) bin_ions<true>(ions_s, i0, i1, na, nb, c, k0);
+            else bin_ions<false>(ions_s, i0, i1, na, nb, c, k0);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&s_full[buf]);
+        }
+    } else if (warp == kMmaWarp) {
+        // ---- MMA warp: descriptors advance by adding to the 14-bit start-address field ---------------
+        const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(p.N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+        const uint32_t tb = smem_u32(smem + L.table), hb = smem_u32(smem + L.hist0);
+        const uint32_t a_hi = (uint32_t)(kChunkBytes >> 4) | (1u << 14);                         // SBO, version 1, INTERLEAVE
+        const uint32_t a_lo0 = ((hb >> 4) & 0x3FFFu) | ((uint32_t)(kGroupBytes >> 4) << 16);       // LBO = 2560 B
+        const uint32_t b_hi = (uint32_t)(1024 >> 4) | (1u << 14) | (2u << 29);                     // SBO, version 1, SWIZZLE_128B
+        const uint32_t b_lo0 = ((tb >> 4) & 0x3FFFu) | (1u << 16);
+        const uint32_t kblk_step = (uint32_t)(p.N * 128) >> 4;
+        for (int it = 0; it < nitems; ++it) {
+            const int gl = it / npass, pass = it % npass, buf = kBig ? 0 : (it & 1), use = kBig ? it : (it >> 1);
+            mbar_wait<100>(&s_full[buf], (uint32_t)(use & 1));
+            if (pass == 0 && gl >= 2) mbar_wait(&s_tfree[gl & 1], (uint32_t)(((gl >> 1) - 1) & 1));
+            asm volatile("tcgen05.fence::after_thread_sync;");
+            const uint32_t acc = tmem + (uint32_t)((gl & 1) * p.N);
+            if (lane == 0) {
+                const uint32_t a_lo = a_lo0 + (uint32_t)buf * ((L.hist1 - L.hist0) >> 4);
+#pragma unroll
+                for (int ks = 0; ks < KS; ++ks) {
+                    const uint64_t ad = ((uint64_t)a_hi << 32) | (a_lo + (uint32_t)ks * ((2 * kGroupBytes) >> 4));
+                    const uint64_t bd = ((uint64_t)b_hi << 32) | (b_lo0 + (uint32_t)(ks >> 2) * kblk_step + (uint32_t)(ks & 3) * 2u);
+                    if (ks == 0) mma_f16_ss(acc, ad, bd, idesc, pass > 0 ? 1u : 0u);
+                    else mma_f16_acc(acc, ad, bd, idesc);
+                }
+                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
+                             ::"r"(smem_u32(&s_done[buf])) : "memory");
+            }
+            __syncwarp();
+        }
+    } else {
+        // ---- service warps: clear the transformed histogram, then the epilogue ------------------------
+        const int q = warp & 3, st = tid - kSvcWarp0 * 32, set = (warp - kSvcWarp0) >> 2;
+        for (int it = 0; it < nitems; ++it) {
+            const int gl = it / npass, buf = kBig ? 0 : (it & 1), use = kBig ? it : (it >> 1);
+            const bool last_pass = (it % npass) == npass - 1;
+            mbar_wait<200>(&s_done[buf], (uint32_t)(use & 1));
+            asm volatile("tcgen05.fence::after_thread_sync;");
+            if (st == 0) {
+                // clear the buffer with bulk copies of zeros (TMA engine, no LSU work); free(buf) completes
+                // when all bytes have landed
+                const uint32_t dst = smem_u32(smem + (buf ? L.hist1 : L.hist0)), bar = smem_u32(&s_free[buf]);
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(L.hist_bytes) : "memory");
+                const uint32_t piece = L.hist_bytes / 4;
+#pragma unroll
+                for (int c4 = 0; c4 < 4; ++c4)
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                                 ::"r"(dst + c4 * piece), "l"((const char *)p.zeros + c4 * piece), "r"(piece), "r"(bar) : "memory");
+            }
+            if (last_pass) {
+                epilogue_group(p, tmem + (uint32_t)((gl & 1) * p.N), g_begin + gl, m, phase, exch, cand, set, q, lane);
+                asm volatile("tcgen05.fence::before_thread_sync;");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&s_tfree[gl & 1]);
+            }
+        }
+    }
+}
+
 template <int KS>   // KS = K/16 = B/64 k-steps per group
 __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParams p)
 {
@@ -329,8 +435,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     {
-        uint4 *h = reinterpret_cast<uint4 *>(smem + L.hist0);
-        for (int i = tid; i < (int)(2 * L.hist_bytes / 16); i += kMmaThreads) h[i] = make_uint4(0, 0, 0, 0);   // both buffers
+        uint4 *h0 = reinterpret_cast<uint4 *>(smem + L.hist0), *h1 = reinterpret_cast<uint4 *>(smem + L.hist1);
+        for (int i = tid; i < (int)(L.hist_bytes / 16); i += kMmaThreads) { h0[i] = make_uint4(0, 0, 0, 0); h1[i] = make_uint4(0, 0, 0, 0); }
         uint4 *t = reinterpret_cast<uint4 *>(smem + L.table);
         for (int i = tid; i < K * p.N / 8; i += kMmaThreads) t[i] = p.table[i];
         for (int i = tid; i < 4 * p.W; i += kMmaThreads) phase[i] = p.phase[i];
@@ -345,102 +451,12 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     const int n = s_n;
     if (chunk == 0 && tid == 0 && p.counts) p.counts[m] = (uint32_t)n;
 
-    if (n > p.cap) {
-        // too many ions for the shared buffer: leave this material point to the FFT kernel
+    if (n > p.cap_big) {
+        // too many ions even for ion buffer + second histogram buffer: leave this material point to the FFT kernel
         if (chunk == 0 && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
     } else {
-        // Pipeline over items = (direction group, ion pass); item it uses histogram buffer it & 1 and the TMEM
-        // accumulator (group & 1):
-        //   binning warps 0..15 : wait free(buf) -> project-and-bin item it -> arrive full(buf)
-        //   MMA warp 16         : wait full(buf) [, tfree(acc)] -> K/16 tcgen05.mma -> commit to done(buf)
-        //   service warps 17..20: wait done(buf) -> clear the buffer -> arrive free(buf); after the last pass of a
-        //                         group: epilogue from TMEM -> arrive tfree(acc)
-        const int npass = n > 2048 ? (n + 2047) / 2048 : 1;          // fp16 counters are exact up to 2048
-        const int nitems = (g_end - g_begin) * npass;
-        if (warp < kBinWarps) {
-            BinConst c;
-            c.half_b = (float)(p.B / 2); c.magic_a = magic_for(p.B); c.magic_b = 12582912.0f + 4.0f;
-            c.scl = __int_as_float((127 - p.nl) << 23);                       // 2^-nl
-            c.kz = 16u - (uint32_t)kBlkBytes * (1u << p.nl);
-            const int l = lane & 15, hw = warp * 2 + (lane >> 4);             // half-warp index 0..31
-            const uint32_t k0base = smem_u32(smem + L.hist0) + (uint32_t)(l >> 2) * kChunkBytes + (uint32_t)(l & 3) * 4u
-                                    - 0x4B400000u * (uint32_t)kBlkBytes - 0x4B400000u * c.kz;
-            const uint32_t ions_s = smem_u32(ions);
-            for (int it = 0; it < nitems; ++it) {
-                const int gl = it / npass, pass = it % npass, buf = it & 1;
-                float na[3], nb[3];
-                {
-                    const float *da = p.dirs_sorted + (size_t)((g_begin + gl) * 32 + l) * 3;
-                    na[0] = da[0]; na[1] = da[1]; na[2] = da[2];
-                    nb[0] = da[48]; nb[1] = da[49]; nb[2] = da[50];
-                }
-                if (it >= 2) mbar_wait(&s_free[buf], (uint32_t)(((it >> 1) - 1) & 1));    // cleared after item it-2
-                const int a0 = pass * 2048, a1 = min(n, a0 + 2048);
-                const int per = (((a1 - a0 + 2 * kBinWarps - 1) / (2 * kBinWarps)) + 3) & ~3;
-                const int i0 = min(a1, a0 + hw * per), i1 = min(a1, i0 + per);
-                const uint32_t k0 = k0base + (uint32_t)buf * L.hist_bytes;
-                if (p.clamp) bin_ions<true>(ions_s, i0, i1, na, nb, c, k0);
-                else bin_ions<false>(ions_s, i0, i1, na, nb, c, k0);
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&s_full[buf]);
-            }
-        } else if (warp == kMmaWarp) {
-            // ---- MMA warp: descriptors advance by adding to the 14-bit start-address field ---------------
-            const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(p.N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-            const uint32_t tb = smem_u32(smem + L.table), hb = smem_u32(smem + L.hist0);
-            const uint32_t a_hi = (uint32_t)(kChunkBytes >> 4) | (1u << 14);                         // SBO, version 1, INTERLEAVE
-            const uint32_t a_lo0 = ((hb >> 4) & 0x3FFFu) | ((uint32_t)(kGroupBytes >> 4) << 16);       // LBO = 2560 B
-            const uint32_t b_hi = (uint32_t)(1024 >> 4) | (1u << 14) | (2u << 29);                     // SBO, version 1, SWIZZLE_128B
-            const uint32_t b_lo0 = ((tb >> 4) & 0x3FFFu) | (1u << 16);
-            const uint32_t kblk_step = (uint32_t)(p.N * 128) >> 4;
-            for (int it = 0; it < nitems; ++it) {
-                const int gl = it / npass, pass = it % npass, buf = it & 1;
-                mbar_wait<100>(&s_full[buf], (uint32_t)((it >> 1) & 1));
-                if (pass == 0 && gl >= 2) mbar_wait(&s_tfree[gl & 1], (uint32_t)(((gl >> 1) - 1) & 1));
-                asm volatile("tcgen05.fence::after_thread_sync;");
-                const uint32_t acc = tmem + (uint32_t)((gl & 1) * p.N);
-                if (lane == 0) {
-                    const uint32_t a_lo = a_lo0 + (uint32_t)buf * (L.hist_bytes >> 4);
-#pragma unroll
-                    for (int ks = 0; ks < KS; ++ks) {
-                        const uint64_t ad = ((uint64_t)a_hi << 32) | (a_lo + (uint32_t)ks * ((2 * kGroupBytes) >> 4));
-                        const uint64_t bd = ((uint64_t)b_hi << 32) | (b_lo0 + (uint32_t)(ks >> 2) * kblk_step + (uint32_t)(ks & 3) * 2u);
-                        if (ks == 0) mma_f16_ss(acc, ad, bd, idesc, pass > 0 ? 1u : 0u);
-                        else mma_f16_acc(acc, ad, bd, idesc);
-                    }
-                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
-                                 ::"r"(smem_u32(&s_done[buf])) : "memory");
-                }
-                __syncwarp();
-            }
-        } else {
-            // ---- service warps: clear the transformed histogram, then the epilogue ------------------------
-            const int q = warp & 3, st = tid - kSvcWarp0 * 32, set = (warp - kSvcWarp0) >> 2;
-            for (int it = 0; it < nitems; ++it) {
-                const int gl = it / npass, buf = it & 1;
-                const bool last_pass = (it % npass) == npass - 1;
-                mbar_wait<200>(&s_done[buf], (uint32_t)((it >> 1) & 1));
-                asm volatile("tcgen05.fence::after_thread_sync;");
-                if (st == 0) {
-                    // clear the buffer with bulk copies of zeros (TMA engine, no LSU work); free(buf) completes
-                    // when all bytes have landed
-                    const uint32_t dst = smem_u32(smem + (buf ? L.hist1 : L.hist0)), bar = smem_u32(&s_free[buf]);
-                    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(L.hist_bytes) : "memory");
-                    const uint32_t piece = L.hist_bytes / 4;
-#pragma unroll
-                    for (int c4 = 0; c4 < 4; ++c4)
-                        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                                     ::"r"(dst + c4 * piece), "l"((const char *)p.zeros + c4 * piece), "r"(piece), "r"(bar) : "memory");
-                }
-                if (last_pass) {
-                    epilogue_group(p, tmem + (uint32_t)((gl & 1) * p.N), g_begin + gl, m, phase, exch, cand, set, q, lane);
-                    asm volatile("tcgen05.fence::before_thread_sync;");
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(&s_tfree[gl & 1]);
-                }
-            }
-        }
+        if (n > p.cap) run_pipeline<KS, true>(p, L, smem, tmem, n, g_begin, g_end, m, ions, phase, exch, cand, s_full, s_done, s_free, s_tfree);
+        else run_pipeline<KS, false>(p, L, smem, tmem, n, g_begin, g_end, m, ions, phase, exch, cand, s_full, s_done, s_free, s_tfree);
     }
     // ---- teardown ---------------------------------------------------------------------------------
     asm volatile("tcgen05.fence::before_thread_sync;");
@@ -581,6 +597,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.nl = 0;
     while ((8 << q.nl) < p->B) ++q.nl;
     q.cap = mma_cap_for(p->B, q.N, p->W);
+    q.cap_big = std::min(8192, q.cap + (int)((size_t)(p->B / 32) * kGroupBytes / 12));
     q.ngroups = p->Dp / 32;
     int nchunks = (q.ngroups + 95) / 96;
     const int64_t want = (int64_t)p->sm_count * 8;

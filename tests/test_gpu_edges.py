@@ -111,3 +111,25 @@ def test_pad0_and_non_unit_directions_clamp(flags):
     w = _case(xyz, types, 1.2, 512)
     _check(w, dirs, centres, (5, 20), flags, pad=0)
     _check(w, dirs, centres, (5, 20), flags, pad=1)
+
+
+def test_run_host_matches_device_path():
+    """apx_run_host (host pointers, slabbed and pipelined copies) returns exactly what apx_run leaves on the device."""
+    import torch
+    xyz, types = _ball(2.4, eta=0.5, sigma=0.05, seed=17)
+    rng = np.random.default_rng(3)
+    centres = ((rng.random((301, 3)) - 0.5) * 2.0).astype(np.float32)       # 301 points: four ragged slabs
+    dirs = O.dirs_fibonacci(96)
+    plan = apx.Plan(1.0, 256, dirs, k_lo=7, k_hi=17, device=0)
+    dev = torch.device("cuda:0")
+    sig_d = torch.empty((301, 96, 2), dtype=torch.float32, device=dev)
+    cnt_d = torch.empty(301, dtype=torch.int32, device=dev)
+    plan.apx_run(torch.from_numpy(xyz).to(dev), torch.from_numpy(types).to(dev), torch.from_numpy(centres).to(dev), sig_d, cnt_d)
+    torch.cuda.synchronize()
+    sig_h = torch.empty((301, 96, 2), dtype=torch.float32).pin_memory()
+    cnt_h = torch.empty(301, dtype=torch.int32).pin_memory()
+    plan.apx_run_host(torch.from_numpy(xyz), torch.from_numpy(types), torch.from_numpy(centres), sig_h, cnt_h)
+    assert torch.equal(sig_h, sig_d.cpu()) and torch.equal(cnt_h, cnt_d.cpu())
+    ref, rc = O.signatures(xyz, types, centres[:5], dirs, 1.0, 256, k_lo=7, k_hi=17)
+    assert (cnt_h[:5].numpy().astype(np.uint32) == rc).all()
+    plan.apx_plan_destroy()

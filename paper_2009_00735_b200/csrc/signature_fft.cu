@@ -311,7 +311,7 @@ static cudaError_t launch_fft_common(Plan *p, const float *centres, int64_t M, c
     q.list = list; q.D = p->D; q.k_lo = p->k_lo; q.k_hi = p->k_hi; q.cap = fft_cap_for(B);
     q.ngroups = (p->D + G - 1) / G;
     // enough CTAs to fill the machine a few times over, but at least a handful of groups per CTA (one gather each)
-    int nchunks = (q.ngroups + 63) / 64;
+    int nchunks = 1;
     const int64_t want = (int64_t)p->sm_count * 4;
     const int64_t Mx = list ? 1 : M;
     if (Mx * nchunks < want) nchunks = (int)((want + Mx - 1) / Mx);

@@ -22,7 +22,8 @@
 //              2^11 cos_lo, 2^11 sin_lo) so amplitudes reach ~1e-7.
 //   peak     : |X_k|^2 arg-max over the window, lowest k on ties (L75, L416); A* = 2^24 sqrt(max).
 // Two histogram buffers and two TMEM accumulators: while the 16 binning warps fill buffer (g+1)&1, the tensor
-// core transforms buffer g&1 and four service warps clear it and run the epilogue of group g.  ROIs with more
+// core transforms buffer g&1, a TMA bulk copy clears it and one of two sets of four service warps runs the epilogue
+// of group g.  ROIs with more
 // ions than the shared-memory ion buffer are appended to a deferred list and handled by the general FFT kernel.
 #include <algorithm>
 #include <cmath>
@@ -35,8 +36,9 @@ namespace apx {
 
 constexpr int kBinWarps = 16;            // warps 0..15: project-and-bin
 constexpr int kMmaWarp = 16;             // tcgen05.mma issuer
-constexpr int kSvcWarp0 = 17;            // warps 17..24: histogram clearing + epilogue (TMEM quarter = warp & 3),
-constexpr int kSvcWarps = 8;             // two sets of four warps that take alternate rounds of window bins
+constexpr int kClrWarp = 17;             // issues the TMA bulk clears
+constexpr int kSvcWarp0 = 18;            // warps 18..25: epilogue (TMEM quarter = warp & 3),
+constexpr int kSvcWarps = 8;             // two sets of four warps; set s takes the groups with (group & 1) == s
 constexpr int kMmaWarps = kSvcWarp0 + kSvcWarps;
 constexpr int kMmaThreads = kMmaWarps * 32;
 constexpr int kSvcThreads = kSvcWarps * 32;
@@ -228,20 +230,19 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
     }
 }
 
-// Epilogue of one direction group (a5 tail, a6, a7) by the eight service warps.  Service warp (set, q) reads TMEM
+// Epilogue of one direction group (a5 tail, a6, a7) by one set of four service warps.  Service warp q reads TMEM
 // lane quarter q = M rows 32q..32q+31 = part blk = q of all 32 direction slots (slot from the lane).  Window bins
-// are handled in rounds of 4 (set s takes rounds s, s+2, ...): each thread scales its 4 partial sums by the phase
-// w^{blk k}, keeps the one whose index is q and hands the other three to the partner warps of its set through
-// `exch` (a reduce-scatter over blk).
+// are handled in rounds of 4: each thread scales its 4 partial sums by the phase w^{blk k}, keeps the one whose
+// index is q and hands the other three to the partner warps of its set through `exch` (a reduce-scatter over blk).
 __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc, int gi, int64_t m, const float2 *phase,
-                                               float2 *exch_all, float2 *cand, int set, int q, int lane)
+                                               float2 *exch_all, float2 *cand_all, int set, int q, int lane)
 {
     const uint32_t acc0 = acc + ((uint32_t)(q * 32) << 16);
-    float2 *exch = exch_all + set * (kEpiRound * 4 * 32);
+    float2 *exch = exch_all + set * (kEpiRound * 4 * 32), *cand = cand_all + set * (4 * 32);
     float best = -1.0f;
     int kbest = p.k_lo;
 #pragma unroll 1
-    for (int r0 = set * kEpiRound; r0 < p.W; r0 += 2 * kEpiRound) {
+    for (int r0 = 0; r0 < p.W; r0 += kEpiRound) {
         uint32_t v[16];
         tmem_ld16(acc0 + (uint32_t)(4 * r0), v);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
@@ -272,13 +273,13 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
         }
         if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
     }
-    cand[(set * 4 + q) * 32 + lane] = make_float2(best, __int_as_float(kbest));
-    asm volatile("bar.sync 5, %0;" ::"n"(kSvcThreads) : "memory");
-    if (set == 0 && q == 0) {
+    cand[q * 32 + lane] = make_float2(best, __int_as_float(kbest));
+    if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
+    if (q == 0) {
         float bb = -1.0f;
         int kb = p.k_lo;
 #pragma unroll
-        for (int s = 0; s < 8; ++s) {
+        for (int s = 0; s < 4; ++s) {
             const float2 c2 = cand[s * 32 + lane];
             const int ck = __float_as_int(c2.y);
             if (c2.x > bb || (c2.x == bb && ck < kb)) { bb = c2.x; kb = ck; }
@@ -287,6 +288,7 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
         const int d = p.perm[gi * 32 + slot];
         if (d >= 0) p.sig[(size_t)m * p.D + d] = make_float2(16777216.0f * sqrtf(fmaxf(bb, 0.0f)), (float)kb);
     }
+    // the set's cand is rewritten only after the barriers of the rounds of its next epilogue
 }
 
 // The warp-specialised pipeline of one (material point, chunk).  kBig: the ROI's ions have spilled into the second
@@ -295,7 +297,7 @@ template <int KS, bool kBig>
 __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &L, unsigned char *smem, uint32_t tmem, int n,
                                              int g_begin, int g_end, int64_t m, const float *ions, const float2 *phase,
                                              float2 *exch, float2 *cand, uint64_t *s_full, uint64_t *s_done,
-                                             uint64_t *s_free, uint64_t *s_tfree)
+                                             uint64_t *s_free, uint64_t *s_epi, uint64_t *s_tfree)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // Pipeline over items = (direction group, ion pass); item it uses histogram buffer it & 1 and the TMEM
@@ -362,20 +364,19 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                 }
                 asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
                              ::"r"(smem_u32(&s_done[buf])) : "memory");
+                if (pass == npass - 1)                                           // the group's accumulator is complete
+                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
+                                 ::"r"(smem_u32(&s_epi[gl & 1])) : "memory");
             }
             __syncwarp();
         }
-    } else {
-        // ---- service warps: clear the transformed histogram, then the epilogue ------------------------
-        const int q = warp & 3, st = tid - kSvcWarp0 * 32, set = (warp - kSvcWarp0) >> 2;
+    } else if (warp == kClrWarp) {
+        // ---- clear warp: once the tensor core has read a buffer, clear it with bulk copies of zeros (TMA engine, no
+        //      LSU work); free(buf) completes when all bytes have landed
         for (int it = 0; it < nitems; ++it) {
-            const int gl = it / npass, buf = kBig ? 0 : (it & 1), use = kBig ? it : (it >> 1);
-            const bool last_pass = (it % npass) == npass - 1;
-            mbar_wait<200>(&s_done[buf], (uint32_t)(use & 1));
-            asm volatile("tcgen05.fence::after_thread_sync;");
-            if (st == 0) {
-                // clear the buffer with bulk copies of zeros (TMA engine, no LSU work); free(buf) completes
-                // when all bytes have landed
+            const int buf = kBig ? 0 : (it & 1), use = kBig ? it : (it >> 1);
+            mbar_wait<100>(&s_done[buf], (uint32_t)(use & 1));
+            if (lane == 0) {
                 const uint32_t dst = smem_u32(smem + (buf ? L.hist1 : L.hist0)), bar = smem_u32(&s_free[buf]);
                 asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(L.hist_bytes) : "memory");
                 const uint32_t piece = L.hist_bytes / 4;
@@ -384,12 +385,18 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                                  ::"r"(dst + c4 * piece), "l"((const char *)p.zeros + c4 * piece), "r"(piece), "r"(bar) : "memory");
             }
-            if (last_pass) {
-                epilogue_group(p, tmem + (uint32_t)((gl & 1) * p.N), g_begin + gl, m, phase, exch, cand, set, q, lane);
-                asm volatile("tcgen05.fence::before_thread_sync;");
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&s_tfree[gl & 1]);
-            }
+            __syncwarp();
+        }
+    } else {
+        // ---- service warps: set s runs the epilogue of the groups with (group & 1) == s -----------------
+        const int q = warp & 3, set = (warp - kSvcWarp0) >> 2;
+        for (int gl = set; gl < g_end - g_begin; gl += 2) {
+            mbar_wait<200>(&s_epi[set], (uint32_t)((gl >> 1) & 1));
+            asm volatile("tcgen05.fence::after_thread_sync;");
+            epilogue_group(p, tmem + (uint32_t)(set * p.N), g_begin + gl, m, phase, exch, cand, set, q, lane);
+            asm volatile("tcgen05.fence::before_thread_sync;");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&s_tfree[set]);
         }
     }
 }
@@ -401,7 +408,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned, still shared-space
     const MmaSmem L = mma_smem_layout(p.B, p.N, p.W, p.cap);
     // per histogram buffer: full (binned), done (transformed), free (cleared); per accumulator: tfree (read out)
-    __shared__ uint64_t s_full[2], s_done[2], s_free[2], s_tfree[2];
+    __shared__ uint64_t s_full[2], s_done[2], s_free[2], s_epi[2], s_tfree[2];
     __shared__ uint32_t s_tmem;
     __shared__ int s_n;
 
@@ -425,7 +432,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
             mbar_init(&s_full[i], kBinWarps);
             mbar_init(&s_done[i], 1);
             mbar_init(&s_free[i], 1);
-            mbar_init(&s_tfree[i], kSvcWarps);
+            mbar_init(&s_epi[i], 1);
+            mbar_init(&s_tfree[i], 4);
         }
         asm volatile("fence.mbarrier_init.release.cluster;");
         s_n = 0;
@@ -455,8 +463,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
         // too many ions even for ion buffer + second histogram buffer: leave this material point to the FFT kernel
         if (chunk == 0 && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
     } else {
-        if (n > p.cap) run_pipeline<KS, true>(p, L, smem, tmem, n, g_begin, g_end, m, ions, phase, exch, cand, s_full, s_done, s_free, s_tfree);
-        else run_pipeline<KS, false>(p, L, smem, tmem, n, g_begin, g_end, m, ions, phase, exch, cand, s_full, s_done, s_free, s_tfree);
+        if (n > p.cap) run_pipeline<KS, true>(p, L, smem, tmem, n, g_begin, g_end, m, ions, phase, exch, cand, s_full, s_done, s_free, s_epi, s_tfree);
+        else run_pipeline<KS, false>(p, L, smem, tmem, n, g_begin, g_end, m, ions, phase, exch, cand, s_full, s_done, s_free, s_epi, s_tfree);
     }
     // ---- teardown ---------------------------------------------------------------------------------
     asm volatile("tcgen05.fence::before_thread_sync;");
@@ -599,7 +607,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.cap = mma_cap_for(p->B, q.N, p->W);
     q.cap_big = std::min(8192, q.cap + (int)((size_t)(p->B / 32) * kGroupBytes / 12));
     q.ngroups = p->Dp / 32;
-    int nchunks = (q.ngroups + 95) / 96;
+    int nchunks = 1;                                       // one gather per material point when there are enough of them
     const int64_t want = (int64_t)p->sm_count * 8;
     if (M * nchunks < want) nchunks = (int)((want + M - 1) / M);
     if (nchunks > (q.ngroups + 1) / 2) nchunks = (q.ngroups + 1) / 2;

@@ -41,10 +41,10 @@ constexpr int kSvcWarp0 = 18;            // warps 18..25: epilogue (TMEM quarter
 constexpr int kSvcWarps = 8;             // two sets of four warps; set s takes the groups with (group & 1) == s
 constexpr int kMmaWarps = kSvcWarp0 + kSvcWarps;
 constexpr int kMmaThreads = kMmaWarps * 32;
-constexpr int kSvcThreads = kSvcWarps * 32;
 constexpr int kChunkBytes = 160;         // SBO: 8 directions x 8 rows x 2 B + 32 B skew
 constexpr int kBlkBytes = 640;           // 4 M-chunks: one (blk, kg) slab of 8 K rows x 32 directions
 constexpr int kGroupBytes = 2560;        // LBO: 16 M-chunks = the 4 blk slabs of one 8-row K group
+constexpr int kStsClearBelow = 700;      // ROIs with fewer ions clear with plain stores instead of TMA copies from L2
 constexpr int kEpiRound = 4;             // window bins per epilogue round (one tcgen05.ld x16)
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -376,7 +376,13 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         for (int it = 0; it < nitems; ++it) {
             const int buf = kBig ? 0 : (it & 1), use = kBig ? it : (it >> 1);
             mbar_wait<100>(&s_done[buf], (uint32_t)(use & 1));
-            if (lane == 0) {
+            if (n < kStsClearBelow) {
+                // few ions: the LSU pipe has room, clear with plain stores and spare the L2 the zero traffic
+                uint4 *h = reinterpret_cast<uint4 *>(smem + (buf ? L.hist1 : L.hist0));
+                for (int i = lane; i < (int)(L.hist_bytes / 16); i += 32) h[i] = make_uint4(0, 0, 0, 0);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&s_free[buf]);
+            } else if (lane == 0) {
                 const uint32_t dst = smem_u32(smem + (buf ? L.hist1 : L.hist0)), bar = smem_u32(&s_free[buf]);
                 asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(L.hist_bytes) : "memory");
                 const uint32_t piece = L.hist_bytes / 4;
@@ -412,7 +418,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     __shared__ uint32_t s_tmem;
     __shared__ int s_n;
 
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, warp = tid >> 5;
     const int64_t m = blockIdx.x / p.nchunks;
     const int chunk = blockIdx.x % p.nchunks;
     const int g_begin = (int)((int64_t)chunk * p.ngroups / p.nchunks);

@@ -36,7 +36,7 @@ PAIR_FLOP = 6.0          # FMUL + 2 FFMA + round-down FADD of Eq. 1's projection
 PAIR_SLOTS_MMA = 8.0     # + FFMA.RD (hi3) + 2 IMAD (address) + 1 shared atomic: issue slots per pair, MMA kernel
 # traffic (dram__bytes_read.sum + dram__bytes_write.sum per launch) of the dominant kernel from the committed
 # ncu --set full capture (profiles/), config 2; None for a kernel/config that was not captured
-NCU_TRAFFIC = {"k_signature_mma": 25.9e6, "k_signature_fft": None}
+NCU_TRAFFIC = {"k_signature_mma": 25.6e6, "k_signature_fft": 28.4e6}
 
 
 def algorithmic_flops(n_pairs, n_hist, B, path):

@@ -25,6 +25,8 @@ sys.path.insert(0, ROOT)
 
 METRIC = "direction-histograms/s"
 UNIT = "histograms/s"
+WORKLOAD = ("cfg2_single_crystal: fcc Al 20^3 nm (~241k ions), 1000 material points x 10000 Fibonacci directions, "
+            "R=2.0 nm, B=1024, window [15,34]")
 # nominal FP32 peak used as the "alu" roofline denominator (B200_PROFILING.md: 148 SMs, 1965 MHz max SM clock;
 # 128 FP32 lanes per SM, FFMA = 2 flop): derived in DESIGN.md "Roofline".
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
@@ -60,7 +62,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._read, daemon=True).start()
         except Exception:
@@ -134,8 +136,7 @@ def run_reference(args, rank, world):
         "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "material_points_per_s": v / w.D,
-        "config": {"workload": "cfg2_single_crystal: fcc Al 20^3 nm, 1000 material points x 10000 Fibonacci "
-                               "directions, R=2.0 nm, B=1024, window [15,34]", "sample": sample},
+        "config": {"workload": WORKLOAD, "sample": sample},
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
@@ -246,8 +247,7 @@ def run_ours(args, rank, world, local_rank):
         "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "material_points_per_s": value / D,
-        "config": {"workload": "cfg2_single_crystal: fcc Al 20^3 nm (~241k ions), 1000 material points x 10000 "
-                               "Fibonacci directions, R=2.0 nm, B=1024, window [15,34]",
+        "config": {"workload": WORKLOAD,
                    "kernel_path": "mma" if plan.apx_plan_path() == 1 else "fft",
                    "l2": "flushed between timed steps (256 MiB fill, untimed)",
                    "ions": int(len(w.xyz)), "mean_ions_per_roi": float(n_c.mean()),

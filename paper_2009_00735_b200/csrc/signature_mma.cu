@@ -23,8 +23,8 @@
 //   peak     : |X_k|^2 arg-max over the window, lowest k on ties (L75, L416); A* = 2^24 sqrt(max).
 // Two histogram buffers and two TMEM accumulators: while the 16 binning warps fill buffer (g+1)&1, the tensor
 // core transforms buffer g&1, a TMA bulk copy clears it and one of two sets of four service warps runs the epilogue
-// of group g.  ROIs with more
-// ions than the shared-memory ion buffer are appended to a deferred list and handled by the general FFT kernel.
+// of group g.  A ROI with more ions than the ion buffer spills into the second histogram buffer and runs
+// single-buffered; only ROIs beyond that are appended to a deferred list for the general FFT kernel.
 #include <algorithm>
 #include <cmath>
 #include <cuda_fp16.h>

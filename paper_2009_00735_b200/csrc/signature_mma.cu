@@ -112,7 +112,7 @@ struct MmaParams {
     float2 *sig;
     uint32_t *counts;
     uint32_t *deferred;        // [0] = count, [1..] = material point ids left to the FFT kernel
-    int D, B, nl, k_lo, W, N, cap, cap_big, nchunks, ngroups, clamp;
+    int D, B, nl, k_lo, W, N, cap, cap_big, nchunks, ngroups, clamp, M;
     uint32_t tmem_cols;
     float R, R2;
 };
@@ -419,10 +419,19 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     __shared__ int s_n;
 
     const int tid = threadIdx.x, warp = tid >> 5;
-    const int64_t m = blockIdx.x / p.nchunks;
-    const int chunk = blockIdx.x % p.nchunks;
-    const int g_begin = (int)((int64_t)chunk * p.ngroups / p.nchunks);
-    const int g_end = (int)((int64_t)(chunk + 1) * p.ngroups / p.nchunks);
+    // CTAs are ordered chunk-major; with up to 6 chunks per material point the chunks shrink geometrically (weights
+    // 2^(nchunks-1-c)), so the last waves of the grid consist of the smallest work items
+    const int chunk = blockIdx.x / p.M;
+    const int64_t m = blockIdx.x % p.M;
+    int g_begin, g_end;
+    if (p.nchunks <= 6) {
+        const int wtot = (1 << p.nchunks) - 1, wlo = wtot - ((1 << (p.nchunks - chunk)) - 1);
+        g_begin = (int)((int64_t)wlo * p.ngroups / wtot);
+        g_end = (int)((int64_t)(wlo + (1 << (p.nchunks - 1 - chunk))) * p.ngroups / wtot);
+    } else {                                                   // few material points: many equal chunks
+        g_begin = (int)((int64_t)chunk * p.ngroups / p.nchunks);
+        g_end = (int)((int64_t)(chunk + 1) * p.ngroups / p.nchunks);
+    }
     const GridParams g = *p.grid;
     const float cx = p.centres[3 * m], cy = p.centres[3 * m + 1], cz = p.centres[3 * m + 2];
     const RoiCells rc = roi_cells(g, cx, cy, cz, p.R);
@@ -618,7 +627,9 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     if (M * nchunks < want) nchunks = (int)((want + M - 1) / M);
     if (nchunks > (q.ngroups + 1) / 2) nchunks = (q.ngroups + 1) / 2;
     if (nchunks < 1) nchunks = 1;
+    if (nchunks > 1 && nchunks < 6 && (q.ngroups >> (nchunks + 1)) >= 2) ++nchunks;   // one more, smaller, tail chunk
     q.nchunks = nchunks;
+    q.M = (int)M;
     q.clamp = p->need_clamp;
     uint32_t cols = 32;
     while (cols < (uint32_t)(2 * q.N)) cols *= 2;

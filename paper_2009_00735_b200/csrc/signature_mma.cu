@@ -138,7 +138,8 @@ __host__ __device__ inline MmaSmem mma_smem_layout(int B, int N, int W, int cap)
     return s;
 }
 
-// Gather (step a2) into packed 12-byte records (dx, dy, dz): four ions = three LDS.128 for the binning warps.
+// Gather (step a2) into quad-blocked records: four ions = 48 B = [dx0..dx3][dy0..dy3][dz0..dz3], i.e. three LDS.128
+// whose register pairs are the operands of the packed fp32x2 arithmetic of the binning warps.
 __device__ __forceinline__ void gather_roi3(const MmaParams &p, const GridParams &g, const RoiCells &rc,
                                             float cx, float cy, float cz, float *ions, int *s_n)
 {
@@ -161,20 +162,35 @@ __device__ __forceinline__ void gather_roi3(const MmaParams &p, const GridParams
                 int pos = 0;
                 if (lane == 0) pos = atomicAdd(s_n, __popc(msk));
                 pos = __shfl_sync(0xffffffffu, pos, 0) + __popc(msk & ((1u << lane) - 1u));
-                if (in && pos < p.cap_big) { ions[3 * pos] = dx; ions[3 * pos + 1] = dy; ions[3 * pos + 2] = dz; }
+                if (in && pos < p.cap_big) {                   // quad-blocked: [x0..x3][y0..y3][z0..z3] per four ions
+                    float *q = ions + (pos >> 2) * 12 + (pos & 3);
+                    q[0] = dx; q[4] = dy; q[8] = dz;
+                }
             }
         }
     }
 }
 
-// Project-and-bin (step a4) of one ion for one direction of this lane.
+// Project-and-bin (step a4).  All 32 lanes of a warp work on the SAME ions: lanes 0..15 for the 16 directions of
+// set A (low u16 of word l = lane & 15, increment 1), lanes 16..31 for the 16 directions of set B (high u16 of the same
+// word, increment 65536).  The plan pairs every compact patch A with the patch B nearest to its antipode, so
+// hi3(B) = 7 - hi3(A) has the other parity and the two half-warps fall on disjoint banks.
 //   ua = bits(RD(x + 1.5*2^23 + B/2))       = 0x4B400000 + b          (b = B/2 + floor(x), Eq. 1)
 //   va = bits(RD(x*2^-nl + 1.5*2^23 + 4))   = 0x4B400000 + hi3        (hi3 = b >> nl, exact: floor(floor(y)/n) = floor(y/n))
 //   address = hist + lane offset + 640*low + 16*hi3 = ua*640 + va*(16 - 640*2^nl) + k0   (mod 2^32)
+// Two ions are projected at once with the packed fp32x2 instructions of sm_100 (FMUL2 / FFMA2 / FADD2.RM /
+// FFMA2.RM: IEEE single roundings per component, same operation order as the contract): 5 packed + 2 x (2 IMAD +
+// ATOMS) = 5.5 issue slots per (ion, direction) pair instead of 8.
 struct BinConst {
     float half_b, magic_a, magic_b, scl;
     uint32_t kz;
 };
+__device__ __forceinline__ uint64_t pack2(float lo, float hi)
+{
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
 template <bool kClamp>
 __device__ __forceinline__ void bin_one(float dx, float dy, float dz, float npx, float npy, float npz, const BinConst &c,
                                         uint32_t k0, uint32_t inc)
@@ -185,48 +201,57 @@ __device__ __forceinline__ void bin_one(float dx, float dy, float dz, float npx,
     const uint32_t va = __float_as_uint(__fmaf_rd(x, c.scl, c.magic_b));
     red_shared_add(ua * (uint32_t)kBlkBytes + (va * c.kz + k0), inc);
 }
-template <bool kClamp>
-__device__ __forceinline__ void bin_two(float dx, float dy, float dz, const float (&na)[3], const float (&nb)[3],
-                                        const BinConst &c, uint32_t k0)
+// two ions (dx0,dx1), (dy0,dy1), (dz0,dz1) for this lane's direction
+__device__ __forceinline__ void bin_pair(float dx0, float dx1, float dy0, float dy1, float dz0, float dz1, uint64_t nx2,
+                                         uint64_t ny2, uint64_t nz2, uint64_t ma2, uint64_t sc2, uint64_t mb2, uint32_t kz,
+                                         uint32_t k0, uint32_t inc)
 {
-    bin_one<kClamp>(dx, dy, dz, na[0], na[1], na[2], c, k0, 1u);            // set A: low u16 of the lane's word
-    bin_one<kClamp>(dx, dy, dz, nb[0], nb[1], nb[2], c, k0, 65536u);        // set B: high u16
+    uint64_t t, ua, va;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(t) : "l"(nx2), "l"(pack2(dx0, dx1)));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(t) : "l"(ny2), "l"(pack2(dy0, dy1)), "l"(t));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(t) : "l"(nz2), "l"(pack2(dz0, dz1)), "l"(t));
+    asm("add.rm.f32x2 %0, %1, %2;" : "=l"(ua) : "l"(t), "l"(ma2));
+    asm("fma.rm.f32x2 %0, %1, %2, %3;" : "=l"(va) : "l"(t), "l"(sc2), "l"(mb2));
+    const uint32_t ua0 = (uint32_t)ua, ua1 = (uint32_t)(ua >> 32), va0 = (uint32_t)va, va1 = (uint32_t)(va >> 32);
+    red_shared_add(ua0 * (uint32_t)kBlkBytes + (va0 * kz + k0), inc);
+    red_shared_add(ua1 * (uint32_t)kBlkBytes + (va1 * kz + k0), inc);
 }
 
-// ions_s = shared-space byte address of the packed ion records; i0 is a multiple of 4 (per half-warp)
+// ions_s = shared-space byte address of the quad-blocked ion records; i0 is a multiple of 4
 template <bool kClamp>
-__device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const float (&na)[3], const float (&nb)[3],
-                                         const BinConst &c, uint32_t k0)
+__device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, float npx, float npy, float npz, const BinConst &c,
+                                         uint32_t k0, uint32_t inc)
 {
     int ib = i0;
-    for (; ib + 8 <= i1; ib += 8) {                          // 8 ions = 6 LDS.128, then 16 independent chains
-        float4 q[6];
+    if (!kClamp) {
+        const uint64_t nx2 = pack2(npx, npx), ny2 = pack2(npy, npy), nz2 = pack2(npz, npz);
+        const uint64_t ma2 = pack2(c.magic_a, c.magic_a), sc2 = pack2(c.scl, c.scl), mb2 = pack2(c.magic_b, c.magic_b);
+        for (; ib + 8 <= i1; ib += 8) {                      // 8 ions = 6 LDS.128, then 4 independent packed chains
+            float4 q[6];
 #pragma unroll
-        for (int u = 0; u < 6; ++u) q[u] = lds128(ions_s + (uint32_t)ib * 12u + (uint32_t)u * 16u);
+            for (int u = 0; u < 6; ++u) q[u] = lds128(ions_s + (uint32_t)ib * 12u + (uint32_t)u * 16u);
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const float4 a = q[3 * h], b = q[3 * h + 1], d = q[3 * h + 2];
-            bin_two<kClamp>(a.x, a.y, a.z, na, nb, c, k0);
-            bin_two<kClamp>(a.w, b.x, b.y, na, nb, c, k0);
-            bin_two<kClamp>(b.z, b.w, d.x, na, nb, c, k0);
-            bin_two<kClamp>(d.y, d.z, d.w, na, nb, c, k0);
+            for (int h = 0; h < 2; ++h) {
+                const float4 X = q[3 * h], Y = q[3 * h + 1], Z = q[3 * h + 2];
+                bin_pair(X.x, X.y, Y.x, Y.y, Z.x, Z.y, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc);
+                bin_pair(X.z, X.w, Y.z, Y.w, Z.z, Z.w, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc);
+            }
+        }
+        if (ib + 4 <= i1) {
+            const float4 X = lds128(ions_s + (uint32_t)ib * 12u), Y = lds128(ions_s + (uint32_t)ib * 12u + 16u),
+                         Z = lds128(ions_s + (uint32_t)ib * 12u + 32u);
+            bin_pair(X.x, X.y, Y.x, Y.y, Z.x, Z.y, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc);
+            bin_pair(X.z, X.w, Y.z, Y.w, Z.z, Z.w, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc);
+            ib += 4;
         }
     }
-    if (ib + 4 <= i1) {
-        const float4 a = lds128(ions_s + (uint32_t)ib * 12u), b = lds128(ions_s + (uint32_t)ib * 12u + 16u),
-                     d = lds128(ions_s + (uint32_t)ib * 12u + 32u);
-        bin_two<kClamp>(a.x, a.y, a.z, na, nb, c, k0);
-        bin_two<kClamp>(a.w, b.x, b.y, na, nb, c, k0);
-        bin_two<kClamp>(b.z, b.w, d.x, na, nb, c, k0);
-        bin_two<kClamp>(d.y, d.z, d.w, na, nb, c, k0);
-        ib += 4;
-    }
-    for (; ib < i1; ++ib) {
+    for (; ib < i1; ++ib) {                                  // ragged tail (and every ion when the clamp is needed)
+        const uint32_t a = ions_s + (uint32_t)(ib >> 2) * 48u + (uint32_t)(ib & 3) * 4u;
         float dx, dy, dz;
-        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dx) : "r"(ions_s + (uint32_t)ib * 12u));
-        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dy) : "r"(ions_s + (uint32_t)ib * 12u + 4u));
-        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(ions_s + (uint32_t)ib * 12u + 8u));
-        bin_two<kClamp>(dx, dy, dz, na, nb, c, k0);
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dx) : "r"(a));
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dy) : "r"(a + 16u));
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(a + 32u));
+        bin_one<kClamp>(dx, dy, dz, npx, npy, npz, c, k0, inc);
     }
 }
 
@@ -315,25 +340,22 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         c.half_b = (float)(p.B / 2); c.magic_a = magic_for(p.B); c.magic_b = 12582912.0f + 4.0f;
         c.scl = __int_as_float((127 - p.nl) << 23);                       // 2^-nl
         c.kz = 16u - (uint32_t)kBlkBytes * (1u << p.nl);
-        const int l = lane & 15, hw = warp * 2 + (lane >> 4);             // half-warp index 0..31
+        const int l = lane & 15;
+        const uint32_t inc = lane < 16 ? 1u : 65536u;                      // set A: low u16, set B: high u16
         const uint32_t k0base = smem_u32(smem + L.hist0) + (uint32_t)(l >> 2) * kChunkBytes + (uint32_t)(l & 3) * 4u
                                 - 0x4B400000u * (uint32_t)kBlkBytes - 0x4B400000u * c.kz;
         const uint32_t ions_s = smem_u32(ions);
         for (int it = 0; it < nitems; ++it) {
             const int gl = it / npass, pass = it % npass, buf = kBig ? 0 : (it & 1), use = kBig ? it : (it >> 1);
-            float na[3], nb[3];
-            {
-                const float *da = p.dirs_sorted + (size_t)((g_begin + gl) * 32 + l) * 3;
-                na[0] = da[0]; na[1] = da[1]; na[2] = da[2];
-                nb[0] = da[48]; nb[1] = da[49]; nb[2] = da[50];
-            }
+            const float *da = p.dirs_sorted + (size_t)((g_begin + gl) * 32 + lane) * 3;
+            const float npx = da[0], npy = da[1], npz = da[2];
             if (use >= 1) mbar_wait(&s_free[buf], (uint32_t)((use - 1) & 1));         // cleared after its previous use
             const int a0 = pass * 2048, a1 = min(n, a0 + 2048);
-            const int per = (((a1 - a0 + 2 * kBinWarps - 1) / (2 * kBinWarps)) + 3) & ~3;
-            const int i0 = min(a1, a0 + hw * per), i1 = min(a1, i0 + per);
+            const int nq = (a1 - a0 + 3) >> 2;                                       // quads of this pass, split evenly
+            const int i0 = a0 + 4 * ((warp * nq) / kBinWarps), i1 = min(a1, a0 + 4 * (((warp + 1) * nq) / kBinWarps));
             const uint32_t k0 = k0base + (uint32_t)buf * (L.hist1 - L.hist0);
-            if (p.clamp) bin_ions<true>(ions_s, i0, i1, na, nb, c, k0);
-            else bin_ions<false>(ions_s, i0, i1, na, nb, c, k0);
+            if (p.clamp) bin_ions<true>(ions_s, i0, i1, npx, npy, npz, c, k0, inc);
+            else bin_ions<false>(ions_s, i0, i1, npx, npy, npz, c, k0, inc);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
             __syncwarp();
             if (lane == 0) mbar_arrive(&s_full[buf]);
@@ -505,28 +527,79 @@ bool mma_path_supported(const Plan *p)
     return mma_cap_for(p->B, N, p->W) >= 1024;           // room for a useful ion buffer
 }
 
-// Order the directions so that every run of 16 is a spatially compact patch: recursive bisection along the
-// widest axis, cutting at a multiple of 16.  Within one shared atomic the 16 lanes of a half-warp then project
-// an ion onto nearly parallel directions, their bins share the top three bits and hit 16 different banks.
-static void patch_order(const std::vector<float> &v, std::vector<int> &idx, int lo, int hi)
+// Direction order of the binning warps.  A group of 32 slots = a compact patch of 16 directions (set A, lanes 0..15)
+// followed by the 16 directions nearest to the ANTIPODE of that patch (set B, lanes 16..31).  Within one shared atomic
+// the 16 lanes of a half-warp project the ion onto nearly parallel directions, so their bins share the top three bits
+// (hi3) and hit 16 different banks; the other half-warp sees x -> -x, hi3 -> 7 - hi3, the other bank parity.
+// Construction: fold every direction onto one hemisphere (f = n or -n), split into the unflipped set P and the flipped
+// set Q (equal sizes for Fibonacci grids with even D and for antipodally symmetric grids; otherwise balanced by
+// moving the surplus), then bisect P and Q in lockstep along the widest axis of the folded coordinates, cutting both
+// at the same multiple of 16.  The order only affects bank conflicts, never results.
+struct FoldedDir {
+    float f[3];
+    int idx;
+};
+static void pair_bisect(std::vector<FoldedDir> &P, std::vector<FoldedDir> &Q, int lo, int hi)
 {
     const int cnt = hi - lo;
-    if (cnt <= 16) return;
+    const int pe = std::min(hi, (int)P.size()), qe = std::min(hi, (int)Q.size());
+    auto lex = [](const FoldedDir &a, const FoldedDir &b) {
+        return a.f[0] != b.f[0] ? a.f[0] < b.f[0] : (a.f[1] != b.f[1] ? a.f[1] < b.f[1] : a.f[2] < b.f[2]);
+    };
+    if (cnt <= 16) {                                     // leaf: same slot order on both sides (exact antipodes line up)
+        if (lo < pe) std::sort(P.begin() + lo, P.begin() + pe, lex);
+        if (lo < qe) std::sort(Q.begin() + lo, Q.begin() + qe, lex);
+        return;
+    }
     float mn[3] = {1e30f, 1e30f, 1e30f}, mx[3] = {-1e30f, -1e30f, -1e30f};
-    for (int i = lo; i < hi; ++i)
-        for (int a = 0; a < 3; ++a) {
-            mn[a] = std::min(mn[a], v[3 * (size_t)idx[i] + a]);
-            mx[a] = std::max(mx[a], v[3 * (size_t)idx[i] + a]);
-        }
+    for (int i = lo; i < pe; ++i)
+        for (int a = 0; a < 3; ++a) { mn[a] = std::min(mn[a], P[i].f[a]); mx[a] = std::max(mx[a], P[i].f[a]); }
+    for (int i = lo; i < qe; ++i)
+        for (int a = 0; a < 3; ++a) { mn[a] = std::min(mn[a], Q[i].f[a]); mx[a] = std::max(mx[a], Q[i].f[a]); }
     int ax = 0;
     for (int a = 1; a < 3; ++a)
         if (mx[a] - mn[a] > mx[ax] - mn[ax]) ax = a;
     const int leaves = (cnt + 15) / 16;
-    const int left = (leaves / 2) * 16;
-    std::nth_element(idx.begin() + lo, idx.begin() + lo + left, idx.begin() + hi,
-                     [&](int a, int b) { return v[3 * (size_t)a + ax] < v[3 * (size_t)b + ax]; });
-    patch_order(v, idx, lo, lo + left);
-    patch_order(v, idx, lo + left, hi);
+    const int mid = lo + (leaves / 2) * 16;
+    auto cmp = [&](const FoldedDir &a, const FoldedDir &b) { return a.f[ax] != b.f[ax] ? a.f[ax] < b.f[ax] : lex(a, b); };
+    if (mid < pe) std::nth_element(P.begin() + lo, P.begin() + mid, P.begin() + pe, cmp);
+    if (mid < qe) std::nth_element(Q.begin() + lo, Q.begin() + mid, Q.begin() + qe, cmp);
+    pair_bisect(P, Q, lo, mid);
+    pair_bisect(P, Q, mid, hi);
+}
+// v = [D][3]; returns the slot order (original index per slot, -1 = padding), length = multiple of 32
+static std::vector<int> pair_order(const std::vector<float> &v, int D)
+{
+    std::vector<FoldedDir> P, Q;
+    for (int i = 0; i < D; ++i) {
+        const float x = v[3 * (size_t)i], y = v[3 * (size_t)i + 1], z = v[3 * (size_t)i + 2];
+        const bool up = z > 0.f || (z == 0.f && (y > 0.f || (y == 0.f && x > 0.f)));
+        FoldedDir d;
+        d.idx = i;
+        for (int a = 0; a < 3; ++a) d.f[a] = up ? v[3 * (size_t)i + a] : -v[3 * (size_t)i + a];
+        (up ? P : Q).push_back(d);
+    }
+    auto move_surplus = [](std::vector<FoldedDir> &big, std::vector<FoldedDir> &small) {
+        while (big.size() > small.size() + 1) {          // unbalanced input: the surplus keeps f = -(its folded vector)
+            FoldedDir d = big.back();
+            big.pop_back();
+            for (int a = 0; a < 3; ++a) d.f[a] = -d.f[a];
+            small.push_back(d);
+        }
+    };
+    move_surplus(P, Q);
+    move_surplus(Q, P);
+    const int cnt = (int)std::max(P.size(), Q.size());
+    const int leaves = (cnt + 15) / 16;
+    if (leaves > 0) pair_bisect(P, Q, 0, leaves * 16);
+    std::vector<int> slots((size_t)leaves * 32, -1);
+    for (int j = 0; j < leaves; ++j)
+        for (int e = 0; e < 16; ++e) {
+            const int i = j * 16 + e;
+            if (i < (int)P.size()) slots[(size_t)j * 32 + e] = P[i].idx;
+            if (i < (int)Q.size()) slots[(size_t)j * 32 + 16 + e] = Q[i].idx;
+        }
+    return slots;
 }
 
 cudaError_t mma_path_prepare(Plan *p)
@@ -575,16 +648,12 @@ cudaError_t mma_path_prepare(Plan *p)
     std::vector<float> nps((size_t)3 * p->D);
     e = cudaMemcpy(nps.data(), p->d_dirs_scaled, nps.size() * 4, cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) return e;
-    // patch order + padding to a multiple of 32 (padding slots repeat the last direction, perm = -1)
-    std::vector<int> idx(p->D);
-    std::iota(idx.begin(), idx.end(), 0);
-    patch_order(nps, idx, 0, p->D);
-    const int Dp = ((p->D + 31) / 32) * 32;
+    // paired patch order, padded to a multiple of 32 (padding slots repeat direction 0, perm = -1)
+    const std::vector<int> perm = pair_order(nps, p->D);
+    const int Dp = (int)perm.size();
     std::vector<float> sorted((size_t)3 * Dp);
-    std::vector<int> perm(Dp, -1);
     for (int i = 0; i < Dp; ++i) {
-        const int src = idx[std::min(i, p->D - 1)];
-        if (i < p->D) perm[i] = src;
+        const int src = perm[i] >= 0 ? perm[i] : 0;
         for (int a = 0; a < 3; ++a) sorted[3 * (size_t)i + a] = nps[3 * (size_t)src + a];
     }
     p->Dp = Dp;

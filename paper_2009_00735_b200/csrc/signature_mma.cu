@@ -171,10 +171,11 @@ __device__ __forceinline__ void gather_roi3(const MmaParams &p, const GridParams
     }
 }
 
-// Project-and-bin (step a4).  All 32 lanes of a warp work on the SAME ions: lanes 0..15 for the 16 directions of
-// set A (low u16 of word l = lane & 15, increment 1), lanes 16..31 for the 16 directions of set B (high u16 of the same
-// word, increment 65536).  The plan pairs every compact patch A with the patch B nearest to its antipode, so
-// hi3(B) = 7 - hi3(A) has the other parity and the two half-warps fall on disjoint banks.
+// Project-and-bin (step a4).  Lane (h = lane >> 4, l = lane & 15) owns word l of every histogram row: the low u16 is
+// direction l of set A (increment 1), the high u16 direction l of set B (increment 65536).  The two half-warps take
+// alternate blocks of the warp's ions and every lane bins each of its ions for BOTH of its directions, so one ion
+// load (broadcast LDS.128, 2.2 clk on B200 whether the half-warps read the same or different addresses) serves two
+// (ion, direction) pairs.  The plan pairs every compact patch A with the patch B nearest to its antipode.
 //   ua = bits(RD(x + 1.5*2^23 + B/2))       = 0x4B400000 + b          (b = B/2 + floor(x), Eq. 1)
 //   va = bits(RD(x*2^-nl + 1.5*2^23 + 4))   = 0x4B400000 + hi3        (hi3 = b >> nl, exact: floor(floor(y)/n) = floor(y/n))
 //   address = hist + lane offset + 640*low + 16*hi3 = ua*640 + va*(16 - 640*2^nl) + k0   (mod 2^32)
@@ -217,41 +218,54 @@ __device__ __forceinline__ void bin_pair(float dx0, float dx1, float dy0, float 
     red_shared_add(ua1 * (uint32_t)kBlkBytes + (va1 * kz + k0), inc);
 }
 
-// ions_s = shared-space byte address of the quad-blocked ion records; i0 is a multiple of 4
+// One direction pair of a lane: set A (low u16, increment 1) and set B (high u16, increment 65536) of the same word.
+struct LaneDirs {
+    float ax, ay, az, bx, by, bz;
+};
+// ions_s = shared-space byte address of the quad-blocked ion records; i0 is a multiple of 4.  The two half-warps of a
+// warp take alternate blocks of ions (half h = lane >> 4), every lane bins each of its ions for BOTH of its directions,
+// so one ion load serves two (ion, direction) pairs.
 template <bool kClamp>
-__device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, float npx, float npy, float npz, const BinConst &c,
-                                         uint32_t k0, uint32_t inc)
+__device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const LaneDirs &n, const BinConst &c, uint32_t k0,
+                                         int h)
 {
     int ib = i0;
     if (!kClamp) {
-        const uint64_t nx2 = pack2(npx, npx), ny2 = pack2(npy, npy), nz2 = pack2(npz, npz);
+        const uint64_t ax2 = pack2(n.ax, n.ax), ay2 = pack2(n.ay, n.ay), az2 = pack2(n.az, n.az);
+        const uint64_t bx2 = pack2(n.bx, n.bx), by2 = pack2(n.by, n.by), bz2 = pack2(n.bz, n.bz);
         const uint64_t ma2 = pack2(c.magic_a, c.magic_a), sc2 = pack2(c.scl, c.scl), mb2 = pack2(c.magic_b, c.magic_b);
-        for (; ib + 8 <= i1; ib += 8) {                      // 8 ions = 6 LDS.128, then 4 independent packed chains
+        const uint32_t hoff = (uint32_t)h * 96u;
+        for (; ib + 16 <= i1; ib += 16) {                    // 8 ions per half-warp = 6 LDS.128, then 8 packed chains
             float4 q[6];
 #pragma unroll
-            for (int u = 0; u < 6; ++u) q[u] = lds128(ions_s + (uint32_t)ib * 12u + (uint32_t)u * 16u);
+            for (int u = 0; u < 6; ++u) q[u] = lds128(ions_s + (uint32_t)ib * 12u + hoff + (uint32_t)u * 16u);
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const float4 X = q[3 * h], Y = q[3 * h + 1], Z = q[3 * h + 2];
-                bin_pair(X.x, X.y, Y.x, Y.y, Z.x, Z.y, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc);
-                bin_pair(X.z, X.w, Y.z, Y.w, Z.z, Z.w, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc);
+            for (int hh = 0; hh < 2; ++hh) {
+                const float4 X = q[3 * hh], Y = q[3 * hh + 1], Z = q[3 * hh + 2];
+                bin_pair(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u);
+                bin_pair(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u);
+                bin_pair(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u);
+                bin_pair(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u);
             }
         }
-        if (ib + 4 <= i1) {
-            const float4 X = lds128(ions_s + (uint32_t)ib * 12u), Y = lds128(ions_s + (uint32_t)ib * 12u + 16u),
-                         Z = lds128(ions_s + (uint32_t)ib * 12u + 32u);
-            bin_pair(X.x, X.y, Y.x, Y.y, Z.x, Z.y, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc);
-            bin_pair(X.z, X.w, Y.z, Y.w, Z.z, Z.w, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc);
-            ib += 4;
+        if (ib + 8 <= i1) {                                  // one quad per half-warp
+            const uint32_t a = ions_s + (uint32_t)ib * 12u + (uint32_t)h * 48u;
+            const float4 X = lds128(a), Y = lds128(a + 16u), Z = lds128(a + 32u);
+            bin_pair(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u);
+            bin_pair(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u);
+            bin_pair(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u);
+            bin_pair(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u);
+            ib += 8;
         }
     }
-    for (; ib < i1; ++ib) {                                  // ragged tail (and every ion when the clamp is needed)
-        const uint32_t a = ions_s + (uint32_t)(ib >> 2) * 48u + (uint32_t)(ib & 3) * 4u;
+    for (int i = ib + h; i < i1; i += 2) {                   // ragged tail (and every ion when the clamp is needed)
+        const uint32_t a = ions_s + (uint32_t)(i >> 2) * 48u + (uint32_t)(i & 3) * 4u;
         float dx, dy, dz;
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dx) : "r"(a));
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dy) : "r"(a + 16u));
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(a + 32u));
-        bin_one<kClamp>(dx, dy, dz, npx, npy, npz, c, k0, inc);
+        bin_one<kClamp>(dx, dy, dz, n.ax, n.ay, n.az, c, k0, 1u);
+        bin_one<kClamp>(dx, dy, dz, n.bx, n.by, n.bz, c, k0, 65536u);
     }
 }
 
@@ -319,12 +333,13 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
 // The warp-specialised pipeline of one (material point, chunk).  kBig: the ROI's ions have spilled into the second
 // histogram buffer, so only buffer 0 is used and bin -> transform -> clear are serial per item.
 template <int KS, bool kBig>
-__device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &L, unsigned char *smem, uint32_t tmem, int n,
+__device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &L, unsigned char *smem, uint32_t tmem, int n_ions,
                                              int g_begin, int g_end, int64_t m, const float *ions, const float2 *phase,
                                              float2 *exch, float2 *cand, uint64_t *s_full, uint64_t *s_done,
                                              uint64_t *s_free, uint64_t *s_epi, uint64_t *s_tfree)
 {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);      // provably warp-uniform: ion addresses live in uniform registers
     // Pipeline over items = (direction group, ion pass); item it uses histogram buffer it & 1 and the TMEM
     // accumulator (group & 1):
     //   binning warps 0..15 : wait free(buf) -> project-and-bin item it -> arrive full(buf)
@@ -333,6 +348,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
     //                         group: epilogue from TMEM -> arrive tfree(acc)
     // A ROI with more than `cap` ions has spilled into the second histogram buffer: it runs with buffer 0 only
     // (bin -> transform -> clear serial per item); `use` counts the uses of a buffer.
+    const int n = n_ions;
     const int npass = n > 2048 ? (n + 2047) / 2048 : 1;          // fp16 counters are exact up to 2048
     const int nitems = (g_end - g_begin) * npass;
     if (warp < kBinWarps) {
@@ -340,22 +356,22 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         c.half_b = (float)(p.B / 2); c.magic_a = magic_for(p.B); c.magic_b = 12582912.0f + 4.0f;
         c.scl = __int_as_float((127 - p.nl) << 23);                       // 2^-nl
         c.kz = 16u - (uint32_t)kBlkBytes * (1u << p.nl);
-        const int l = lane & 15;
-        const uint32_t inc = lane < 16 ? 1u : 65536u;                      // set A: low u16, set B: high u16
+        const int l = lane & 15, h = lane >> 4;
         const uint32_t k0base = smem_u32(smem + L.hist0) + (uint32_t)(l >> 2) * kChunkBytes + (uint32_t)(l & 3) * 4u
                                 - 0x4B400000u * (uint32_t)kBlkBytes - 0x4B400000u * c.kz;
         const uint32_t ions_s = smem_u32(ions);
         for (int it = 0; it < nitems; ++it) {
             const int gl = it / npass, pass = it % npass, buf = kBig ? 0 : (it & 1), use = kBig ? it : (it >> 1);
-            const float *da = p.dirs_sorted + (size_t)((g_begin + gl) * 32 + lane) * 3;
-            const float npx = da[0], npy = da[1], npz = da[2];
+            const float *da = p.dirs_sorted + (size_t)((g_begin + gl) * 32 + l) * 3;
+            LaneDirs n;
+            n.ax = da[0]; n.ay = da[1]; n.az = da[2]; n.bx = da[48]; n.by = da[49]; n.bz = da[50];
             if (use >= 1) mbar_wait(&s_free[buf], (uint32_t)((use - 1) & 1));         // cleared after its previous use
-            const int a0 = pass * 2048, a1 = min(n, a0 + 2048);
+            const int a0 = pass * 2048, a1 = min(n_ions, a0 + 2048);
             const int nq = (a1 - a0 + 3) >> 2;                                       // quads of this pass, split evenly
             const int i0 = a0 + 4 * ((warp * nq) / kBinWarps), i1 = min(a1, a0 + 4 * (((warp + 1) * nq) / kBinWarps));
             const uint32_t k0 = k0base + (uint32_t)buf * (L.hist1 - L.hist0);
-            if (p.clamp) bin_ions<true>(ions_s, i0, i1, npx, npy, npz, c, k0, inc);
-            else bin_ions<false>(ions_s, i0, i1, npx, npy, npz, c, k0, inc);
+            if (p.clamp) bin_ions<true>(ions_s, i0, i1, n, c, k0, h);
+            else bin_ions<false>(ions_s, i0, i1, n, c, k0, h);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
             __syncwarp();
             if (lane == 0) mbar_arrive(&s_full[buf]);

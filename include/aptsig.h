@@ -38,6 +38,8 @@ typedef enum {
 #define APX_FLAG_FORCE_FFT 1   /* always use the general FFT kernel, even for a narrow window */
 #define APX_FLAG_FORCE_MMA 2   /* fail with APX_EINVAL instead of falling back when the tensor-core
                                   windowed-DFT kernel cannot serve the plan (window too wide) */
+#define APX_FLAG_NO_PAIRING 4  /* tensor-core kernel: bin every direction on its own even when the grid is
+                                  antipodally symmetric (test hook; results are identical either way) */
 
 typedef struct apx_plan apx_plan; /* opaque */
 
@@ -66,6 +68,9 @@ int apx_plan_destroy(apx_plan *plan);
 int apx_plan_constants(const apx_plan *plan, float *R2, float *s, float *freq_per_bin);
 /* 0 = general FFT kernel, 1 = tensor-core windowed-DFT kernel (chosen at create time from the window). */
 int apx_plan_path(const apx_plan *plan);
+/* 1 = the tensor-core kernel bins every antipodal direction pair (n, -n) with one projection (the grid is
+ * antipodally symmetric, e.g. the paper's geodesic mesh, L60), 0 = every direction on its own. */
+int apx_plan_paired(const apx_plan *plan);
 int apx_last_cuda_error(const apx_plan *plan);
 
 /* Step a1: ingest an ion cloud: drop ions of rejected types and non-finite coordinates, bucket the

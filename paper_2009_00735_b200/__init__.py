@@ -5,10 +5,10 @@ package is its ctypes binding.  Importing the package does not load the library;
 and raises if it has not been built (there is no CPU fallback).
 """
 from .binding import (Plan, ApxError, apx_dirs_fibonacci, apx_dirs_geodesic, apx_version, EXPORTS, LIB_PATH,
-                      APX_FLAG_FORCE_FFT, APX_FLAG_FORCE_MMA, APX_OK, APX_EINVAL, APX_ENOMEM, APX_ECUDA,
+                      APX_FLAG_FORCE_FFT, APX_FLAG_FORCE_MMA, APX_FLAG_NO_PAIRING, APX_OK, APX_EINVAL, APX_ENOMEM, APX_ECUDA,
                       APX_ESTATE, APX_ERANGE)
 
 from .parallel import shard_range, run_sharded, gather_counts
 
 __all__ = ["shard_range", "run_sharded", "gather_counts", "Plan", "ApxError", "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_version", "EXPORTS", "LIB_PATH",
-           "APX_FLAG_FORCE_FFT", "APX_FLAG_FORCE_MMA"]
+           "APX_FLAG_FORCE_FFT", "APX_FLAG_FORCE_MMA", "APX_FLAG_NO_PAIRING"]

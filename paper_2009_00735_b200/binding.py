@@ -13,9 +13,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libaptsig.so")
 
 APX_OK, APX_EINVAL, APX_ENOMEM, APX_ECUDA, APX_ESTATE, APX_ERANGE = 0, -1, -2, -3, -4, -5
-APX_FLAG_FORCE_FFT, APX_FLAG_FORCE_MMA = 1, 2
+APX_FLAG_FORCE_FFT, APX_FLAG_FORCE_MMA, APX_FLAG_NO_PAIRING = 1, 2, 4
 
-EXPORTS = ["apx_plan_create", "apx_plan_destroy", "apx_plan_constants", "apx_plan_path", "apx_last_cuda_error",
+EXPORTS = ["apx_plan_create", "apx_plan_destroy", "apx_plan_constants", "apx_plan_path", "apx_plan_paired", "apx_last_cuda_error",
            "apx_ingest", "apx_query", "apx_run", "apx_run_host", "apx_debug_histograms",
            "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_strerror", "apx_version"]
 
@@ -50,6 +50,7 @@ def _lib():
         L.apx_plan_destroy.argtypes = [vp]
         L.apx_plan_constants.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.apx_plan_path.argtypes = [vp]
+        L.apx_plan_paired.argtypes = [vp]
         L.apx_last_cuda_error.argtypes = [vp]
         L.apx_ingest.argtypes = [vp, vp, vp, i64, vp]
         L.apx_query.argtypes = [vp, vp, i64, vp, vp, vp]
@@ -148,6 +149,9 @@ class Plan:
 
     def apx_plan_path(self) -> int:
         return _lib().apx_plan_path(self._h)
+
+    def apx_plan_paired(self) -> int:
+        return _lib().apx_plan_paired(self._h)
 
     def apx_ingest(self, xyz, types=None, stream=None):
         self._check(_lib().apx_ingest(self._h, _ptr(xyz), _ptr(types), xyz.shape[0], _stream(stream)), "apx_ingest")

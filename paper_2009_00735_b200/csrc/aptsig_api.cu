@@ -155,6 +155,7 @@ extern "C" int apx_plan_constants(const apx_plan *p, float *R2, float *s, float 
 }
 
 extern "C" int apx_plan_path(const apx_plan *p) { return p ? p->path : APX_EINVAL; }
+extern "C" int apx_plan_paired(const apx_plan *p) { return p ? (p->path == 1 ? p->mma_paired : 0) : APX_EINVAL; }
 extern "C" int apx_last_cuda_error(const apx_plan *p) { return p ? p->last_cuda : (int)cudaErrorInvalidValue; }
 
 extern "C" int apx_ingest(apx_plan *p, const float *xyz, const uint8_t *types, int64_t N, void *stream)

@@ -38,6 +38,7 @@ struct Plan {
     float *d_dirs_sorted;          // [Dp][3] scaled directions in patch order (MMA path)
     int *d_dir_perm;               // [Dp] original index of each sorted slot, -1 = padding
     int Dp;                        // D rounded up to a multiple of 32
+    int mma_paired;                // 1 = set B of every group is the exact antipode of set A (MMA path, paired binning)
     int need_clamp;                // 1 = the bin clamp of Eq. 1 can trigger and must stay in the kernels' inner loops
     uint32_t *d_deferred;          // [0] count, [1..] material points the MMA kernel left to the FFT kernel
     int64_t cap_deferred;

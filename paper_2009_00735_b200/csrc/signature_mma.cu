@@ -113,6 +113,7 @@ struct MmaParams {
     uint32_t *counts;
     uint32_t *deferred;        // [0] = count, [1..] = material point ids left to the FFT kernel
     int D, B, nl, k_lo, W, N, cap, cap_big, nchunks, ngroups, clamp, M;
+    int paired;                // 1 = set B of every group is the exact antipode of set A: one projection serves both
     uint32_t tmem_cols;
     float R, R2;
 };
@@ -269,6 +270,83 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
     }
 }
 
+// ---- paired mode: direction l of set B is EXACTLY -(direction l of set A) (antipodally symmetric grids such as the
+// geodesic mesh of the paper, L60).  Then x_B = -x_A bit for bit (every product and sum is negated exactly), so
+// b_B = B/2 + floor(-x) = B - 1 - b_A whenever x is not an integer.  The histogram of set B is stored MIRRORED
+// (bin j at the position of bin B-1-j), which leaves its amplitude spectrum unchanged (|X_k| of a reversed real
+// sequence), so ONE projection and ONE shared atomic of 0x00010001 serve both directions.  x is an integer exactly
+// when rounding x + magic down and up gives the same number; then b_B = B - b_A, one position lower in the mirrored
+// histogram, and the two counters are incremented separately (rare: ~1e-5 of all pairs).
+__device__ __forceinline__ uint32_t addr_of_ua(uint32_t ua, uint32_t kz, uint32_t k0, int nl)
+{
+    const uint32_t b = ua - 0x4B400000u;
+    return ua * (uint32_t)kBlkBytes + ((0x4B400000u + (b >> nl)) * kz + k0);
+}
+__device__ __noinline__ void bin_sym_integer(uint32_t ua, uint32_t kz, uint32_t k0, int nl)
+{
+    red_shared_add(addr_of_ua(ua, kz, k0, nl), 1u);                 // set A: bin b
+    red_shared_add(addr_of_ua(ua - 1u, kz, k0, nl), 65536u);        // set B: bin B - b, stored at position b - 1
+}
+__device__ __forceinline__ void bin_pair_sym(float dx0, float dx1, float dy0, float dy1, float dz0, float dz1, uint64_t nx2,
+                                             uint64_t ny2, uint64_t nz2, uint64_t ma2, uint64_t sc2, uint64_t mb2, uint32_t kz,
+                                             uint32_t k0, int nl)
+{
+    uint64_t t, ua, up, va;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(t) : "l"(nx2), "l"(pack2(dx0, dx1)));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(t) : "l"(ny2), "l"(pack2(dy0, dy1)), "l"(t));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(t) : "l"(nz2), "l"(pack2(dz0, dz1)), "l"(t));
+    asm("add.rm.f32x2 %0, %1, %2;" : "=l"(ua) : "l"(t), "l"(ma2));
+    asm("add.rp.f32x2 %0, %1, %2;" : "=l"(up) : "l"(t), "l"(ma2));
+    asm("fma.rm.f32x2 %0, %1, %2, %3;" : "=l"(va) : "l"(t), "l"(sc2), "l"(mb2));
+    const uint32_t ua0 = (uint32_t)ua, ua1 = (uint32_t)(ua >> 32), va0 = (uint32_t)va, va1 = (uint32_t)(va >> 32);
+    const bool int0 = ua0 == (uint32_t)up, int1 = ua1 == (uint32_t)(up >> 32);
+    if (__builtin_expect(int0 | int1, 0)) {
+        if (int0) bin_sym_integer(ua0, kz, k0, nl); else red_shared_add(ua0 * (uint32_t)kBlkBytes + (va0 * kz + k0), 0x00010001u);
+        if (int1) bin_sym_integer(ua1, kz, k0, nl); else red_shared_add(ua1 * (uint32_t)kBlkBytes + (va1 * kz + k0), 0x00010001u);
+    } else {
+        red_shared_add(ua0 * (uint32_t)kBlkBytes + (va0 * kz + k0), 0x00010001u);
+        red_shared_add(ua1 * (uint32_t)kBlkBytes + (va1 * kz + k0), 0x00010001u);
+    }
+}
+// paired-mode counterpart of bin_ions (never with the clamp: the plan pairs only when the clamp cannot trigger)
+__device__ __forceinline__ void bin_ions_sym(uint32_t ions_s, int i0, int i1, float npx, float npy, float npz, const BinConst &c,
+                                             uint32_t k0, int h, int nl)
+{
+    const uint64_t nx2 = pack2(npx, npx), ny2 = pack2(npy, npy), nz2 = pack2(npz, npz);
+    const uint64_t ma2 = pack2(c.magic_a, c.magic_a), sc2 = pack2(c.scl, c.scl), mb2 = pack2(c.magic_b, c.magic_b);
+    const uint32_t hoff = (uint32_t)h * 96u;
+    int ib = i0;
+    for (; ib + 16 <= i1; ib += 16) {                        // 8 ions per half-warp = 6 LDS.128, then 4 packed chains
+        float4 q[6];
+#pragma unroll
+        for (int u = 0; u < 6; ++u) q[u] = lds128(ions_s + (uint32_t)ib * 12u + hoff + (uint32_t)u * 16u);
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+            const float4 X = q[3 * hh], Y = q[3 * hh + 1], Z = q[3 * hh + 2];
+            bin_pair_sym(X.x, X.y, Y.x, Y.y, Z.x, Z.y, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, nl);
+            bin_pair_sym(X.z, X.w, Y.z, Y.w, Z.z, Z.w, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, nl);
+        }
+    }
+    if (ib + 8 <= i1) {                                      // one quad per half-warp
+        const uint32_t a = ions_s + (uint32_t)ib * 12u + (uint32_t)h * 48u;
+        const float4 X = lds128(a), Y = lds128(a + 16u), Z = lds128(a + 32u);
+        bin_pair_sym(X.x, X.y, Y.x, Y.y, Z.x, Z.y, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, nl);
+        bin_pair_sym(X.z, X.w, Y.z, Y.w, Z.z, Z.w, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, nl);
+        ib += 8;
+    }
+    for (int i = ib + h; i < i1; i += 2) {                   // ragged tail
+        const uint32_t a = ions_s + (uint32_t)(i >> 2) * 48u + (uint32_t)(i & 3) * 4u;
+        float dx, dy, dz;
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dx) : "r"(a));
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dy) : "r"(a + 16u));
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(a + 32u));
+        const float x = __fmaf_rn(npz, dz, __fmaf_rn(npy, dy, __fmul_rn(npx, dx)));
+        const uint32_t ua = __float_as_uint(__fadd_rd(x, c.magic_a)), up = __float_as_uint(__fadd_ru(x, c.magic_a));
+        if (ua == up) bin_sym_integer(ua, c.kz, k0, nl);
+        else red_shared_add(addr_of_ua(ua, c.kz, k0, nl), 0x00010001u);
+    }
+}
+
 // Epilogue of one direction group (a5 tail, a6, a7) by one set of four service warps.  Service warp q reads TMEM
 // lane quarter q = M rows 32q..32q+31 = part blk = q of all 32 direction slots (slot from the lane).  Window bins
 // are handled in rounds of 4: each thread scales its 4 partial sums by the phase w^{blk k}, keeps the one whose
@@ -370,7 +448,8 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             const int nq = (a1 - a0 + 3) >> 2;                                       // quads of this pass, split evenly
             const int i0 = a0 + 4 * ((warp * nq) / kBinWarps), i1 = min(a1, a0 + 4 * (((warp + 1) * nq) / kBinWarps));
             const uint32_t k0 = k0base + (uint32_t)buf * (L.hist1 - L.hist0);
-            if (p.clamp) bin_ions<true>(ions_s, i0, i1, n, c, k0, h);
+            if (p.paired) bin_ions_sym(ions_s, i0, i1, n.ax, n.ay, n.az, c, k0, h, p.nl);
+            else if (p.clamp) bin_ions<true>(ions_s, i0, i1, n, c, k0, h);
             else bin_ions<false>(ions_s, i0, i1, n, c, k0, h);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
             __syncwarp();
@@ -672,6 +751,16 @@ cudaError_t mma_path_prepare(Plan *p)
         const int src = perm[i] >= 0 ? perm[i] : 0;
         for (int a = 0; a < 3; ++a) sorted[3 * (size_t)i + a] = nps[3 * (size_t)src + a];
     }
+    for (int i = 0; i < Dp; ++i)                         // a padding slot of set B mirrors its set-A partner
+        if ((i & 16) && perm[i] < 0)
+            for (int a = 0; a < 3; ++a) sorted[3 * (size_t)i + a] = -sorted[3 * (size_t)(i - 16) + a];
+    // paired mode: every set-B direction is the exact negative of its set-A partner (antipodally symmetric grid)
+    bool paired = !p->need_clamp && !(p->desc.flags & APX_FLAG_NO_PAIRING);
+    for (int i = 0; i < Dp && paired; ++i)
+        if (i & 16)
+            for (int a = 0; a < 3; ++a)
+                if (!(sorted[3 * (size_t)i + a] == -sorted[3 * (size_t)(i - 16) + a])) paired = false;
+    p->mma_paired = paired ? 1 : 0;
     p->Dp = Dp;
     e = cudaMalloc(&p->d_dirs_sorted, sorted.size() * 4);
     if (e != cudaSuccess) return e;
@@ -716,6 +805,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.nchunks = nchunks;
     q.M = (int)M;
     q.clamp = p->need_clamp;
+    q.paired = p->mma_paired;
     uint32_t cols = 32;
     while (cols < (uint32_t)(2 * q.N)) cols *= 2;
     q.tmem_cols = cols;

@@ -133,3 +133,33 @@ def test_run_host_matches_device_path():
     ref, rc = O.signatures(xyz, types, centres[:5], dirs, 1.0, 256, k_lo=7, k_hi=17)
     assert (cnt_h[:5].numpy().astype(np.uint32) == rc).all()
     plan.apx_plan_destroy()
+
+
+@pytest.mark.parametrize("flags", [pytest.param(0, id="paired"), pytest.param(apx.APX_FLAG_NO_PAIRING, id="unpaired")])
+def test_antipodal_pairs_with_exact_integer_projections(flags):
+    """Paired binning of (n, -n) on a symmetric grid: b(-n) = B-1-b(n) holds only while n'.d is not an integer
+    (floor(-x) = -floor(x) - 1); for an exact integer b(-n) = B - b(n).  R = 511/256 makes s = 256 exactly, so ions
+    on a 1/4 grid project to exact integers along the axis directions (+-x, +-y, +-z are vertices of the geodesic
+    grid), an ion sits exactly on every centre (x = +-0 for every direction), and a random half of the cloud does
+    not: a missed special case would shift the grid ions against the rest by one bin and change the amplitudes."""
+    rng = np.random.Generator(np.random.PCG64(11))
+    R, B = 511.0 / 256.0, 1024
+    g = np.arange(-10, 11) / 4.0
+    grid = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+    grid = grid[(grid ** 2).sum(1) <= 2.6 ** 2]
+    grid = grid[rng.random(len(grid)) < 0.25]
+    grid = np.concatenate([grid, np.zeros((1, 3)), [[0.25, 0.5, -0.25]]])          # ions exactly on both centres
+    rnd = rng.uniform(-2.6, 2.6, size=(900, 3))
+    xyz = np.concatenate([grid, rnd]).astype(np.float32)
+    rng.shuffle(xyz)
+    dirs = apx.apx_dirs_geodesic(3)
+    assert any((np.abs(d) == (1, 0, 0)).all() for d in dirs)
+    centres = np.array([[0, 0, 0], [0.25, 0.5, -0.25]], np.float32)
+    w = _case(xyz, np.zeros(len(xyz), np.uint8), R, B)
+    import torch
+    plan = apx.Plan(R, B, dirs, k_lo=15, k_hi=34, device=0, flags=flags)
+    assert plan.apx_plan_path() == 1 and plan.apx_plan_paired() == (0 if flags else 1)
+    _, s, _ = plan.apx_plan_constants()
+    assert s == 256.0
+    plan.apx_plan_destroy()
+    _check(w, dirs, centres, (15, 34), flags)

@@ -38,8 +38,8 @@ typedef enum {
 #define APX_FLAG_FORCE_FFT 1   /* always use the general FFT kernel, even for a narrow window */
 #define APX_FLAG_FORCE_MMA 2   /* fail with APX_EINVAL instead of falling back when the tensor-core
                                   windowed-DFT kernel cannot serve the plan (window too wide) */
-#define APX_FLAG_NO_PAIRING 4  /* tensor-core kernel: bin every direction on its own even when the grid is
-                                  antipodally symmetric (test hook; results are identical either way) */
+#define APX_FLAG_NO_PAIRING 4  /* tensor-core kernel: no half-grid mode even when the grid is antipodally
+                                  symmetric (test hook; results are identical either way) */
 
 typedef struct apx_plan apx_plan; /* opaque */
 
@@ -68,8 +68,11 @@ int apx_plan_destroy(apx_plan *plan);
 int apx_plan_constants(const apx_plan *plan, float *R2, float *s, float *freq_per_bin);
 /* 0 = general FFT kernel, 1 = tensor-core windowed-DFT kernel (chosen at create time from the window). */
 int apx_plan_path(const apx_plan *plan);
-/* 1 = the tensor-core kernel bins every antipodal direction pair (n, -n) with one projection (the grid is
- * antipodally symmetric, e.g. the paper's geodesic mesh, L60), 0 = every direction on its own. */
+/* 1 = half-grid mode of the tensor-core kernel: the direction grid is antipodally symmetric (every n has its exact
+ * negative in the grid, e.g. the paper's geodesic mesh, L60), so one member of every pair (n, -n) is binned and its
+ * peak serves both (the histogram of -n is the mirror image: same amplitude spectrum); pairs with an ion whose
+ * projection is an exact integer, where the mirror symmetry of Eq. 1's floor fails, are redone on their own.
+ * 0 = every direction on its own.  Results are identical either way. */
 int apx_plan_paired(const apx_plan *plan);
 int apx_last_cuda_error(const apx_plan *plan);
 

@@ -37,8 +37,9 @@ struct Plan {
     float2 *d_mma_phase;           // [4][W] recombination phases of the four bin parts (MMA path)
     float *d_dirs_sorted;          // [Dp][3] scaled directions in patch order (MMA path)
     int *d_dir_perm;               // [Dp] original index of each sorted slot, -1 = padding
+    int *d_dir_perm_mirror;        // [Dp] half-grid mode: index of the direction opposite to the slot's
     int Dp;                        // D rounded up to a multiple of 32
-    int mma_paired;                // 1 = set B of every group is the exact antipode of set A (MMA path, paired binning)
+    int mma_paired;                // 1 = half-grid mode: the grid is antipodally symmetric, one direction per pair is binned
     int need_clamp;                // 1 = the bin clamp of Eq. 1 can trigger and must stay in the kernels' inner loops
     uint32_t *d_deferred;          // [0] count, [1..] material points the MMA kernel left to the FFT kernel
     int64_t cap_deferred;

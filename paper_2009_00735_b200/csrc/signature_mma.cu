@@ -26,6 +26,9 @@
 // of group g.  A ROI with more ions than the ion buffer spills into the second histogram buffer and runs
 // single-buffered; only ROIs beyond that are appended to a deferred list for the general FFT kernel.
 #include <algorithm>
+#include <array>
+#include <cstring>
+#include <map>
 #include <cmath>
 #include <cuda_fp16.h>
 #include <numeric>
@@ -106,6 +109,7 @@ struct MmaParams {
     const float *centres;
     const float *dirs_sorted;  // [Dp][3] scaled directions in patch order (Dp = D rounded up to 32)
     const int *perm;           // [Dp] original direction index of each sorted slot, -1 = padding
+    const int *perm_mirror;    // [Dp] half-grid mode: index of the direction opposite to the slot's, else nullptr
     const uint4 *table;        // pre-swizzled twiddle operand image, (K/64) blocks of [N][128 B]
     const float2 *phase;       // [4][W] recombination phases w^{blk k}
     const void *zeros;         // hist_bytes of zeros: source of the bulk copies that clear a histogram buffer
@@ -113,7 +117,7 @@ struct MmaParams {
     uint32_t *counts;
     uint32_t *deferred;        // [0] = count, [1..] = material point ids left to the FFT kernel
     int D, B, nl, k_lo, W, N, cap, cap_big, nchunks, ngroups, clamp, M;
-    int paired;                // 1 = set B of every group is the exact antipode of set A: one projection serves both
+    int half;                  // 1 = half-grid mode: one direction per antipodal pair is binned (perm_mirror != nullptr)
     uint32_t tmem_cols;
     float R, R2;
 };
@@ -193,20 +197,47 @@ __device__ __forceinline__ uint64_t pack2(float lo, float hi)
     asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
     return r;
 }
-template <bool kClamp>
+struct Detect;
+__device__ void flag_pair(uint32_t *flag, int *nfix, uint16_t *fix, uint32_t bit, uint32_t id);
+template <bool kClamp, bool kDetect>
 __device__ __forceinline__ void bin_one(float dx, float dy, float dz, float npx, float npy, float npz, const BinConst &c,
-                                        uint32_t k0, uint32_t inc)
+                                        uint32_t k0, uint32_t inc, uint32_t *flag, int *nfix, uint16_t *fix, uint32_t bit, uint32_t id)
 {
     float x = __fmaf_rn(npz, dz, __fmaf_rn(npy, dy, __fmul_rn(npx, dx)));
     if (kClamp) x = fminf(fmaxf(x, -c.half_b), c.half_b - 0.25f);
     const uint32_t ua = __float_as_uint(__fadd_rd(x, c.magic_a));
+    if (kDetect && ua == __float_as_uint(__fadd_ru(x, c.magic_a))) flag_pair(flag, nfix, fix, bit, id);
     const uint32_t va = __float_as_uint(__fmaf_rd(x, c.scl, c.magic_b));
     red_shared_add(ua * (uint32_t)kBlkBytes + (va * c.kz + k0), inc);
 }
+// Half-grid mode (antipodally symmetric direction grids such as the geodesic mesh of the paper, L60): only one
+// direction v of every pair (v, -v) is binned.  x(-v) = -x(v) bit for bit (every product and sum is negated exactly), so
+// b(-v) = B/2 + floor(-x) = B - 1 - b(v) whenever x is not an integer: the histogram of -v is the mirror image of the
+// histogram of v and has the same amplitude spectrum.  x is an integer exactly when rounding x + magic down and up gives
+// the same number; a pair for which that happens for any ion (~1e-5 of all (ion, direction) pairs) is flagged, its -v
+// member gets no output from this group and is binned on its own in a fix-up group.
+constexpr int kFixCap = 512;             // flagged pairs per sub-range of kSubGroups groups
+constexpr int kSubGroups = 128;
+struct Detect {
+    uint32_t *flag;                      // bit s = slot s of this group has met an exact-integer projection
+    int *nfix;
+    uint16_t *fix;                       // flagged pairs: (group within the sub-range) * 32 + slot
+    uint32_t bit, id;
+};
+__device__ __noinline__ void flag_pair(uint32_t *flag, int *nfix, uint16_t *fix, uint32_t bit, uint32_t id)
+{
+    const uint32_t old = atomicOr(flag, bit);
+    if (!(old & bit)) {
+        const int i = atomicAdd(nfix, 1);
+        if (i < kFixCap) fix[i] = (uint16_t)id;
+    }
+}
 // two ions (dx0,dx1), (dy0,dy1), (dz0,dz1) for this lane's direction
-__device__ __forceinline__ void bin_pair(float dx0, float dx1, float dy0, float dy1, float dz0, float dz1, uint64_t nx2,
+// returns (only with kDetect) the number of the two projections that are NOT exact integers
+template <bool kDetect>
+__device__ __forceinline__ uint32_t bin_pair(float dx0, float dx1, float dy0, float dy1, float dz0, float dz1, uint64_t nx2,
                                          uint64_t ny2, uint64_t nz2, uint64_t ma2, uint64_t sc2, uint64_t mb2, uint32_t kz,
-                                         uint32_t k0, uint32_t inc)
+                                         uint32_t k0, uint32_t inc, const Detect &dt)
 {
     uint64_t t, ua, va;
     asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(t) : "l"(nx2), "l"(pack2(dx0, dx1)));
@@ -217,6 +248,12 @@ __device__ __forceinline__ void bin_pair(float dx0, float dx1, float dy0, float 
     const uint32_t ua0 = (uint32_t)ua, ua1 = (uint32_t)(ua >> 32), va0 = (uint32_t)va, va1 = (uint32_t)(va >> 32);
     red_shared_add(ua0 * (uint32_t)kBlkBytes + (va0 * kz + k0), inc);
     red_shared_add(ua1 * (uint32_t)kBlkBytes + (va1 * kz + k0), inc);
+    if (kDetect) {                                       // RU(x + magic) - RD(x + magic) = 1, or 0 for an integer x
+        uint64_t up;
+        asm("add.rp.f32x2 %0, %1, %2;" : "=l"(up) : "l"(t), "l"(ma2));
+        return ((uint32_t)up - ua0) + ((uint32_t)(up >> 32) - ua1);
+    }
+    return 0u;
 }
 
 // One direction pair of a lane: set A (low u16, increment 1) and set B (high u16, increment 65536) of the same word.
@@ -226,36 +263,46 @@ struct LaneDirs {
 // ions_s = shared-space byte address of the quad-blocked ion records; i0 is a multiple of 4.  The two half-warps of a
 // warp take alternate blocks of ions (half h = lane >> 4), every lane bins each of its ions for BOTH of its directions,
 // so one ion load serves two (ion, direction) pairs.
-template <bool kClamp>
+template <bool kClamp, bool kDetect>
 __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const LaneDirs &n, const BinConst &c, uint32_t k0,
-                                         int h)
+                                         int h, const Detect &da, const Detect &db)
 {
     int ib = i0;
     if (!kClamp) {
         const uint64_t ax2 = pack2(n.ax, n.ax), ay2 = pack2(n.ay, n.ay), az2 = pack2(n.az, n.az);
         const uint64_t bx2 = pack2(n.bx, n.bx), by2 = pack2(n.by, n.by), bz2 = pack2(n.bz, n.bz);
         const uint64_t ma2 = pack2(c.magic_a, c.magic_a), sc2 = pack2(c.scl, c.scl), mb2 = pack2(c.magic_b, c.magic_b);
-        const uint32_t hoff = (uint32_t)h * 96u;
-        for (; ib + 16 <= i1; ib += 16) {                    // 8 ions per half-warp = 6 LDS.128, then 8 packed chains
+        uint32_t src = ions_s + (uint32_t)ib * 12u + (uint32_t)h * 96u;
+        for (; ib + 16 <= i1; ib += 16, src += 192u) {       // 8 ions per half-warp = 6 LDS.128, then 8 packed chains
             float4 q[6];
 #pragma unroll
-            for (int u = 0; u < 6; ++u) q[u] = lds128(ions_s + (uint32_t)ib * 12u + hoff + (uint32_t)u * 16u);
+            for (int u = 0; u < 6; ++u) q[u] = lds128(src + (uint32_t)u * 16u);
+            uint32_t na = 0u, nb = 0u;
 #pragma unroll
             for (int hh = 0; hh < 2; ++hh) {
                 const float4 X = q[3 * hh], Y = q[3 * hh + 1], Z = q[3 * hh + 2];
-                bin_pair(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u);
-                bin_pair(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u);
-                bin_pair(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u);
-                bin_pair(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u);
+                na += bin_pair<kDetect>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
+                na += bin_pair<kDetect>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
+                nb += bin_pair<kDetect>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
+                nb += bin_pair<kDetect>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
+            }
+            if (kDetect) {
+                if (__builtin_expect(na != 8u, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
+                if (__builtin_expect(nb != 8u, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
             }
         }
         if (ib + 8 <= i1) {                                  // one quad per half-warp
             const uint32_t a = ions_s + (uint32_t)ib * 12u + (uint32_t)h * 48u;
             const float4 X = lds128(a), Y = lds128(a + 16u), Z = lds128(a + 32u);
-            bin_pair(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u);
-            bin_pair(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u);
-            bin_pair(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u);
-            bin_pair(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u);
+            uint32_t na = 0u, nb = 0u;
+            na += bin_pair<kDetect>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
+            na += bin_pair<kDetect>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
+            nb += bin_pair<kDetect>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
+            nb += bin_pair<kDetect>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
+            if (kDetect) {
+                if (__builtin_expect(na != 4u, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
+                if (__builtin_expect(nb != 4u, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
+            }
             ib += 8;
         }
     }
@@ -265,85 +312,8 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dx) : "r"(a));
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dy) : "r"(a + 16u));
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(a + 32u));
-        bin_one<kClamp>(dx, dy, dz, n.ax, n.ay, n.az, c, k0, 1u);
-        bin_one<kClamp>(dx, dy, dz, n.bx, n.by, n.bz, c, k0, 65536u);
-    }
-}
-
-// ---- paired mode: direction l of set B is EXACTLY -(direction l of set A) (antipodally symmetric grids such as the
-// geodesic mesh of the paper, L60).  Then x_B = -x_A bit for bit (every product and sum is negated exactly), so
-// b_B = B/2 + floor(-x) = B - 1 - b_A whenever x is not an integer.  The histogram of set B is stored MIRRORED
-// (bin j at the position of bin B-1-j), which leaves its amplitude spectrum unchanged (|X_k| of a reversed real
-// sequence), so ONE projection and ONE shared atomic of 0x00010001 serve both directions.  x is an integer exactly
-// when rounding x + magic down and up gives the same number; then b_B = B - b_A, one position lower in the mirrored
-// histogram, and the two counters are incremented separately (rare: ~1e-5 of all pairs).
-__device__ __forceinline__ uint32_t addr_of_ua(uint32_t ua, uint32_t kz, uint32_t k0, int nl)
-{
-    const uint32_t b = ua - 0x4B400000u;
-    return ua * (uint32_t)kBlkBytes + ((0x4B400000u + (b >> nl)) * kz + k0);
-}
-__device__ __noinline__ void bin_sym_integer(uint32_t ua, uint32_t kz, uint32_t k0, int nl)
-{
-    red_shared_add(addr_of_ua(ua, kz, k0, nl), 1u);                 // set A: bin b
-    red_shared_add(addr_of_ua(ua - 1u, kz, k0, nl), 65536u);        // set B: bin B - b, stored at position b - 1
-}
-__device__ __forceinline__ void bin_pair_sym(float dx0, float dx1, float dy0, float dy1, float dz0, float dz1, uint64_t nx2,
-                                             uint64_t ny2, uint64_t nz2, uint64_t ma2, uint64_t sc2, uint64_t mb2, uint32_t kz,
-                                             uint32_t k0, int nl)
-{
-    uint64_t t, ua, up, va;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(t) : "l"(nx2), "l"(pack2(dx0, dx1)));
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(t) : "l"(ny2), "l"(pack2(dy0, dy1)), "l"(t));
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(t) : "l"(nz2), "l"(pack2(dz0, dz1)), "l"(t));
-    asm("add.rm.f32x2 %0, %1, %2;" : "=l"(ua) : "l"(t), "l"(ma2));
-    asm("add.rp.f32x2 %0, %1, %2;" : "=l"(up) : "l"(t), "l"(ma2));
-    asm("fma.rm.f32x2 %0, %1, %2, %3;" : "=l"(va) : "l"(t), "l"(sc2), "l"(mb2));
-    const uint32_t ua0 = (uint32_t)ua, ua1 = (uint32_t)(ua >> 32), va0 = (uint32_t)va, va1 = (uint32_t)(va >> 32);
-    const bool int0 = ua0 == (uint32_t)up, int1 = ua1 == (uint32_t)(up >> 32);
-    if (__builtin_expect(int0 | int1, 0)) {
-        if (int0) bin_sym_integer(ua0, kz, k0, nl); else red_shared_add(ua0 * (uint32_t)kBlkBytes + (va0 * kz + k0), 0x00010001u);
-        if (int1) bin_sym_integer(ua1, kz, k0, nl); else red_shared_add(ua1 * (uint32_t)kBlkBytes + (va1 * kz + k0), 0x00010001u);
-    } else {
-        red_shared_add(ua0 * (uint32_t)kBlkBytes + (va0 * kz + k0), 0x00010001u);
-        red_shared_add(ua1 * (uint32_t)kBlkBytes + (va1 * kz + k0), 0x00010001u);
-    }
-}
-// paired-mode counterpart of bin_ions (never with the clamp: the plan pairs only when the clamp cannot trigger)
-__device__ __forceinline__ void bin_ions_sym(uint32_t ions_s, int i0, int i1, float npx, float npy, float npz, const BinConst &c,
-                                             uint32_t k0, int h, int nl)
-{
-    const uint64_t nx2 = pack2(npx, npx), ny2 = pack2(npy, npy), nz2 = pack2(npz, npz);
-    const uint64_t ma2 = pack2(c.magic_a, c.magic_a), sc2 = pack2(c.scl, c.scl), mb2 = pack2(c.magic_b, c.magic_b);
-    const uint32_t hoff = (uint32_t)h * 96u;
-    int ib = i0;
-    for (; ib + 16 <= i1; ib += 16) {                        // 8 ions per half-warp = 6 LDS.128, then 4 packed chains
-        float4 q[6];
-#pragma unroll
-        for (int u = 0; u < 6; ++u) q[u] = lds128(ions_s + (uint32_t)ib * 12u + hoff + (uint32_t)u * 16u);
-#pragma unroll
-        for (int hh = 0; hh < 2; ++hh) {
-            const float4 X = q[3 * hh], Y = q[3 * hh + 1], Z = q[3 * hh + 2];
-            bin_pair_sym(X.x, X.y, Y.x, Y.y, Z.x, Z.y, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, nl);
-            bin_pair_sym(X.z, X.w, Y.z, Y.w, Z.z, Z.w, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, nl);
-        }
-    }
-    if (ib + 8 <= i1) {                                      // one quad per half-warp
-        const uint32_t a = ions_s + (uint32_t)ib * 12u + (uint32_t)h * 48u;
-        const float4 X = lds128(a), Y = lds128(a + 16u), Z = lds128(a + 32u);
-        bin_pair_sym(X.x, X.y, Y.x, Y.y, Z.x, Z.y, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, nl);
-        bin_pair_sym(X.z, X.w, Y.z, Y.w, Z.z, Z.w, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, nl);
-        ib += 8;
-    }
-    for (int i = ib + h; i < i1; i += 2) {                   // ragged tail
-        const uint32_t a = ions_s + (uint32_t)(i >> 2) * 48u + (uint32_t)(i & 3) * 4u;
-        float dx, dy, dz;
-        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dx) : "r"(a));
-        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dy) : "r"(a + 16u));
-        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(a + 32u));
-        const float x = __fmaf_rn(npz, dz, __fmaf_rn(npy, dy, __fmul_rn(npx, dx)));
-        const uint32_t ua = __float_as_uint(__fadd_rd(x, c.magic_a)), up = __float_as_uint(__fadd_ru(x, c.magic_a));
-        if (ua == up) bin_sym_integer(ua, c.kz, k0, nl);
-        else red_shared_add(addr_of_ua(ua, c.kz, k0, nl), 0x00010001u);
+        bin_one<kClamp, kDetect>(dx, dy, dz, n.ax, n.ay, n.az, c, k0, 1u, da.flag, da.nfix, da.fix, da.bit, da.id);
+        bin_one<kClamp, kDetect>(dx, dy, dz, n.bx, n.by, n.bz, c, k0, 65536u, db.flag, db.nfix, db.fix, db.bit, db.id);
     }
 }
 
@@ -351,9 +321,19 @@ __device__ __forceinline__ void bin_ions_sym(uint32_t ions_s, int i0, int i1, fl
 // lane quarter q = M rows 32q..32q+31 = part blk = q of all 32 direction slots (slot from the lane).  Window bins
 // are handled in rounds of 4: each thread scales its 4 partial sums by the phase w^{blk k}, keeps the one whose
 // index is q and hands the other three to the partner warps of its set through `exch` (a reduce-scatter over blk).
-__device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc, int gi, int64_t m, const float2 *phase,
+// Output: mode 0 (ordinary group gi) writes the slot's own direction and, in half-grid mode, the opposite direction
+// unless the pair was flagged (bit of `mask`); mode 1 (fix-up group) writes only the opposite direction of the listed pair.
+struct EpiOut {
+    int mode, gi, g0, f, nfix;           // g0 = first group of the sub-range, f = fix-up group, nfix = listed pairs
+    uint32_t *flag;                      // mode 0, half-grid: flag word of this group (read, then reset)
+    const uint16_t *fix;
+};
+template <bool kHalf>
+__device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc, const EpiOut &eo, int64_t m, const float2 *phase,
                                                float2 *exch_all, float2 *cand_all, int set, int q, int lane)
 {
+    const int mode = kHalf ? eo.mode : 0;
+    const uint32_t mask = (kHalf && mode == 0) ? *eo.flag : 0u;         // complete: every binning warp has arrived
     const uint32_t acc0 = acc + ((uint32_t)(q * 32) << 16);
     float2 *exch = exch_all + set * (kEpiRound * 4 * 32), *cand = cand_all + set * (4 * 32);
     float best = -1.0f;
@@ -393,6 +373,7 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
     cand[q * 32 + lane] = make_float2(best, __int_as_float(kbest));
     if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
     if (q == 0) {
+        if (kHalf && lane == 0 && mode == 0) *eo.flag = 0u;             // every thread of the set has read it (barriers above)
         float bb = -1.0f;
         int kb = p.k_lo;
 #pragma unroll
@@ -402,33 +383,62 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
             if (c2.x > bb || (c2.x == bb && ck < kb)) { bb = c2.x; kb = ck; }
         }
         const int slot = ((lane & 1) << 4) + ((lane >> 3) << 2) + ((lane & 7) >> 1);
-        const int d = p.perm[gi * 32 + slot];
-        if (d >= 0) p.sig[(size_t)m * p.D + d] = make_float2(16777216.0f * sqrtf(fmaxf(bb, 0.0f)), (float)kb);
+        const float2 res = make_float2(16777216.0f * sqrtf(fmaxf(bb, 0.0f)), (float)kb);
+        if (mode == 0) {
+            const int d = p.perm[eo.gi * 32 + slot];
+            if (d >= 0) p.sig[(size_t)m * p.D + d] = res;
+            if (kHalf && !((mask >> slot) & 1u)) {               // the mirrored histogram has the same amplitude spectrum
+                const int d2 = p.perm_mirror[eo.gi * 32 + slot];
+                if (d2 >= 0) p.sig[(size_t)m * p.D + d2] = res;
+            }
+        } else {
+            const int e = eo.f * 32 + slot;
+            if (e < eo.nfix) {
+                const int d2 = p.perm_mirror[eo.g0 * 32 + (int)eo.fix[e]];
+                if (d2 >= 0) p.sig[(size_t)m * p.D + d2] = res;
+            }
+        }
     }
     // the set's cand is rewritten only after the barriers of the rounds of its next epilogue
 }
 
+// A sequence of direction groups for run_pipeline.  mode 0: the ordinary groups [g0, g0 + ngrp) of the plan's slot
+// order.  mode 1: fix-up groups of the half-grid mode, built from the list of flagged pairs of the sub-range that
+// starts at group g0 (slot s of fix-up group f = list entry 32 f + s, binned as the direction OPPOSITE to the
+// slot's).  grp_base = groups this CTA has run before the sequence: buffer / accumulator / mbarrier parities
+// continue across sequences.
+struct Seq {
+    int mode, g0, ngrp, grp_base, nfix;
+};
+struct PipeShared {
+    uint64_t *full, *done, *free_, *epi, *tfree;
+    uint32_t *flag;
+    int *nfix;
+    uint16_t *fix;
+};
+
 // The warp-specialised pipeline of one (material point, chunk).  kBig: the ROI's ions have spilled into the second
 // histogram buffer, so only buffer 0 is used and bin -> transform -> clear are serial per item.
-template <int KS, bool kBig>
+template <int KS, bool kBig, bool kHalf>
 __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &L, unsigned char *smem, uint32_t tmem, int n_ions,
-                                             int g_begin, int g_end, int64_t m, const float *ions, const float2 *phase,
-                                             float2 *exch, float2 *cand, uint64_t *s_full, uint64_t *s_done,
-                                             uint64_t *s_free, uint64_t *s_epi, uint64_t *s_tfree)
+                                             const Seq &sq, int64_t m, const float *ions, const float2 *phase,
+                                             float2 *exch, float2 *cand, const PipeShared &ps)
 {
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);      // provably warp-uniform: ion addresses live in uniform registers
-    // Pipeline over items = (direction group, ion pass); item it uses histogram buffer it & 1 and the TMEM
-    // accumulator (group & 1):
-    //   binning warps 0..15 : wait free(buf) -> project-and-bin item it -> arrive full(buf)
-    //   MMA warp 16         : wait full(buf) [, tfree(acc)] -> K/16 tcgen05.mma -> commit to done(buf)
-    //   service warps 17..20: wait done(buf) -> clear the buffer -> arrive free(buf); after the last pass of a
-    //                         group: epilogue from TMEM -> arrive tfree(acc)
+    // Pipeline over items = (direction group, ion pass); item number itg (counted from the start of the CTA) uses
+    // histogram buffer itg & 1, group number gq the TMEM accumulator gq & 1:
+    //   binning warps 0..15 : wait free(buf) -> project-and-bin the item -> arrive full(buf)
+    //   MMA warp 16         : wait full(buf) [, tfree(acc)] -> K/16 tcgen05.mma -> commit to done(buf) [, epi(acc)]
+    //   clear warp 17       : wait done(buf) -> clear the buffer -> free(buf)
+    //   service warps 18..25: set s = gq & 1: wait epi(acc) -> epilogue from TMEM -> arrive tfree(acc)
     // A ROI with more than `cap` ions has spilled into the second histogram buffer: it runs with buffer 0 only
     // (bin -> transform -> clear serial per item); `use` counts the uses of a buffer.
     const int n = n_ions;
     const int npass = n > 2048 ? (n + 2047) / 2048 : 1;          // fp16 counters are exact up to 2048
-    const int nitems = (g_end - g_begin) * npass;
+    const int nitems = sq.ngrp * npass;
+    const int mode = kHalf ? sq.mode : 0;
+    const int it_base = sq.grp_base * npass;
     if (warp < kBinWarps) {
         BinConst c;
         c.half_b = (float)(p.B / 2); c.magic_a = magic_for(p.B); c.magic_b = 12582912.0f + 4.0f;
@@ -438,22 +448,40 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         const uint32_t k0base = smem_u32(smem + L.hist0) + (uint32_t)(l >> 2) * kChunkBytes + (uint32_t)(l & 3) * 4u
                                 - 0x4B400000u * (uint32_t)kBlkBytes - 0x4B400000u * c.kz;
         const uint32_t ions_s = smem_u32(ions);
-        for (int it = 0; it < nitems; ++it) {
-            const int gl = it / npass, pass = it % npass, buf = kBig ? 0 : (it & 1), use = kBig ? it : (it >> 1);
-            const float *da = p.dirs_sorted + (size_t)((g_begin + gl) * 32 + l) * 3;
+        const bool detect = kHalf && mode == 0;
+        for (int it = 0, gl = 0, pass = 0; it < nitems; ++it) {
+            const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
             LaneDirs n;
-            n.ax = da[0]; n.ay = da[1]; n.az = da[2]; n.bx = da[48]; n.by = da[49]; n.bz = da[50];
-            if (use >= 1) mbar_wait(&s_free[buf], (uint32_t)((use - 1) & 1));         // cleared after its previous use
+            if (mode == 0) {
+                const float *da = p.dirs_sorted + (size_t)((sq.g0 + gl) * 32 + l) * 3;
+                n.ax = da[0]; n.ay = da[1]; n.az = da[2]; n.bx = da[48]; n.by = da[49]; n.bz = da[50];
+            } else {                                                     // the opposite of a flagged pair's direction
+                const int ea = gl * 32 + l, eb = ea + 16;
+                const float *da = p.dirs_sorted + (ea < sq.nfix ? (size_t)(sq.g0 * 32 + (int)ps.fix[ea]) * 3 : 0);
+                const float *db = p.dirs_sorted + (eb < sq.nfix ? (size_t)(sq.g0 * 32 + (int)ps.fix[eb]) * 3 : 0);
+                n.ax = -da[0]; n.ay = -da[1]; n.az = -da[2]; n.bx = -db[0]; n.by = -db[1]; n.bz = -db[2];
+            }
+            if (use >= 1) mbar_wait(&ps.free_[buf], (uint32_t)((use - 1) & 1));       // cleared after its previous use
             const int a0 = pass * 2048, a1 = min(n_ions, a0 + 2048);
             const int nq = (a1 - a0 + 3) >> 2;                                       // quads of this pass, split evenly
             const int i0 = a0 + 4 * ((warp * nq) / kBinWarps), i1 = min(a1, a0 + 4 * (((warp + 1) * nq) / kBinWarps));
             const uint32_t k0 = k0base + (uint32_t)buf * (L.hist1 - L.hist0);
-            if (p.paired) bin_ions_sym(ions_s, i0, i1, n.ax, n.ay, n.az, c, k0, h, p.nl);
-            else if (p.clamp) bin_ions<true>(ions_s, i0, i1, n, c, k0, h);
-            else bin_ions<false>(ions_s, i0, i1, n, c, k0, h);
+            Detect dta, dtb;
+            if (detect) {
+                dta.flag = dtb.flag = &ps.flag[(sq.grp_base + gl) & 3];
+                dta.nfix = dtb.nfix = ps.nfix; dta.fix = dtb.fix = ps.fix;
+                dta.bit = 1u << l; dtb.bit = 65536u << l;
+                dta.id = (uint32_t)(gl * 32 + l); dtb.id = dta.id + 16u;
+                bin_ions<false, true>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
+            } else if (p.clamp) {
+                bin_ions<true, false>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
+            } else {
+                bin_ions<false, false>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
+            }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
             __syncwarp();
-            if (lane == 0) mbar_arrive(&s_full[buf]);
+            if (lane == 0) mbar_arrive(&ps.full[buf]);
+            if (++pass == npass) { pass = 0; ++gl; }
         }
     } else if (warp == kMmaWarp) {
         // ---- MMA warp: descriptors advance by adding to the 14-bit start-address field ---------------
@@ -464,12 +492,13 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         const uint32_t b_hi = (uint32_t)(1024 >> 4) | (1u << 14) | (2u << 29);                     // SBO, version 1, SWIZZLE_128B
         const uint32_t b_lo0 = ((tb >> 4) & 0x3FFFu) | (1u << 16);
         const uint32_t kblk_step = (uint32_t)(p.N * 128) >> 4;
-        for (int it = 0; it < nitems; ++it) {
-            const int gl = it / npass, pass = it % npass, buf = kBig ? 0 : (it & 1), use = kBig ? it : (it >> 1);
-            mbar_wait<100>(&s_full[buf], (uint32_t)(use & 1));
-            if (pass == 0 && gl >= 2) mbar_wait(&s_tfree[gl & 1], (uint32_t)(((gl >> 1) - 1) & 1));
+        for (int it = 0, gl = 0, pass = 0; it < nitems; ++it) {
+            const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
+            const int gq = sq.grp_base + gl;
+            mbar_wait<100>(&ps.full[buf], (uint32_t)(use & 1));
+            if (pass == 0 && gq >= 2) mbar_wait(&ps.tfree[gq & 1], (uint32_t)(((gq >> 1) - 1) & 1));
             asm volatile("tcgen05.fence::after_thread_sync;");
-            const uint32_t acc = tmem + (uint32_t)((gl & 1) * p.N);
+            const uint32_t acc = tmem + (uint32_t)((gq & 1) * p.N);
             if (lane == 0) {
                 const uint32_t a_lo = a_lo0 + (uint32_t)buf * ((L.hist1 - L.hist0) >> 4);
 #pragma unroll
@@ -480,27 +509,28 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                     else mma_f16_acc(acc, ad, bd, idesc);
                 }
                 asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
-                             ::"r"(smem_u32(&s_done[buf])) : "memory");
+                             ::"r"(smem_u32(&ps.done[buf])) : "memory");
                 if (pass == npass - 1)                                           // the group's accumulator is complete
                     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
-                                 ::"r"(smem_u32(&s_epi[gl & 1])) : "memory");
+                                 ::"r"(smem_u32(&ps.epi[gq & 1])) : "memory");
             }
             __syncwarp();
+            if (++pass == npass) { pass = 0; ++gl; }
         }
     } else if (warp == kClrWarp) {
         // ---- clear warp: once the tensor core has read a buffer, clear it with bulk copies of zeros (TMA engine, no
         //      LSU work); free(buf) completes when all bytes have landed
         for (int it = 0; it < nitems; ++it) {
-            const int buf = kBig ? 0 : (it & 1), use = kBig ? it : (it >> 1);
-            mbar_wait<100>(&s_done[buf], (uint32_t)(use & 1));
+            const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
+            mbar_wait<100>(&ps.done[buf], (uint32_t)(use & 1));
             if (n < kStsClearBelow) {
                 // few ions: the LSU pipe has room, clear with plain stores and spare the L2 the zero traffic
-                uint4 *h = reinterpret_cast<uint4 *>(smem + (buf ? L.hist1 : L.hist0));
-                for (int i = lane; i < (int)(L.hist_bytes / 16); i += 32) h[i] = make_uint4(0, 0, 0, 0);
+                uint4 *hp = reinterpret_cast<uint4 *>(smem + (buf ? L.hist1 : L.hist0));
+                for (int i = lane; i < (int)(L.hist_bytes / 16); i += 32) hp[i] = make_uint4(0, 0, 0, 0);
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&s_free[buf]);
+                if (lane == 0) mbar_arrive(&ps.free_[buf]);
             } else if (lane == 0) {
-                const uint32_t dst = smem_u32(smem + (buf ? L.hist1 : L.hist0)), bar = smem_u32(&s_free[buf]);
+                const uint32_t dst = smem_u32(smem + (buf ? L.hist1 : L.hist0)), bar = smem_u32(&ps.free_[buf]);
                 asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(L.hist_bytes) : "memory");
                 const uint32_t piece = L.hist_bytes / 4;
 #pragma unroll
@@ -511,20 +541,24 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             __syncwarp();
         }
     } else {
-        // ---- service warps: set s runs the epilogue of the groups with (group & 1) == s -----------------
+        // ---- service warps: set s runs the epilogue of the groups with (group number & 1) == s ----------
         const int q = warp & 3, set = (warp - kSvcWarp0) >> 2;
-        for (int gl = set; gl < g_end - g_begin; gl += 2) {
-            mbar_wait<200>(&s_epi[set], (uint32_t)((gl >> 1) & 1));
+        for (int gl = (set ^ sq.grp_base) & 1; gl < sq.ngrp; gl += 2) {
+            const int gq = sq.grp_base + gl;
+            mbar_wait<200>(&ps.epi[set], (uint32_t)((gq >> 1) & 1));
             asm volatile("tcgen05.fence::after_thread_sync;");
-            epilogue_group(p, tmem + (uint32_t)(set * p.N), g_begin + gl, m, phase, exch, cand, set, q, lane);
+            EpiOut eo;
+            eo.mode = mode; eo.gi = sq.g0 + gl; eo.g0 = sq.g0; eo.f = gl; eo.nfix = sq.nfix;
+            eo.flag = kHalf ? &ps.flag[gq & 3] : nullptr; eo.fix = ps.fix;
+            epilogue_group<kHalf>(p, tmem + (uint32_t)(set * p.N), eo, m, phase, exch, cand, set, q, lane);
             asm volatile("tcgen05.fence::before_thread_sync;");
             __syncwarp();
-            if (lane == 0) mbar_arrive(&s_tfree[set]);
+            if (lane == 0) mbar_arrive(&ps.tfree[set]);
         }
     }
 }
 
-template <int KS>   // KS = K/16 = B/64 k-steps per group
+template <int KS, bool kHalf>   // KS = K/16 = B/64 k-steps per group; kHalf = half-grid mode
 __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParams p)
 {
     extern __shared__ unsigned char smem_raw[];
@@ -533,7 +567,9 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     // per histogram buffer: full (binned), done (transformed), free (cleared); per accumulator: tfree (read out)
     __shared__ uint64_t s_full[2], s_done[2], s_free[2], s_epi[2], s_tfree[2];
     __shared__ uint32_t s_tmem;
-    __shared__ int s_n;
+    __shared__ int s_n, s_nfix;
+    __shared__ uint32_t s_flag[4];
+    __shared__ uint16_t s_fix[kFixCap];
 
     const int tid = threadIdx.x, warp = tid >> 5;
     // CTAs are ordered chunk-major; with up to 6 chunks per material point the chunks shrink geometrically (weights
@@ -568,7 +604,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
             mbar_init(&s_tfree[i], 4);
         }
         asm volatile("fence.mbarrier_init.release.cluster;");
-        s_n = 0;
+        s_n = 0; s_nfix = 0;
+        for (int i = 0; i < 4; ++i) s_flag[i] = 0u;
     }
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "r"(p.tmem_cols));
@@ -591,12 +628,50 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     const int n = s_n;
     if (chunk == 0 && tid == 0 && p.counts) p.counts[m] = (uint32_t)n;
 
+    PipeShared ps;
+    ps.full = s_full; ps.done = s_done; ps.free_ = s_free; ps.epi = s_epi; ps.tfree = s_tfree;
+    ps.flag = s_flag; ps.nfix = &s_nfix; ps.fix = s_fix;
+    int grp_total = 0;                                     // groups run by this CTA (ordinary + fix-up)
     if (n > p.cap_big) {
         // too many ions even for ion buffer + second histogram buffer: leave this material point to the FFT kernel
         if (chunk == 0 && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
     } else {
-        if (n > p.cap) run_pipeline<KS, true>(p, L, smem, tmem, n, g_begin, g_end, m, ions, phase, exch, cand, s_full, s_done, s_free, s_epi, s_tfree);
-        else run_pipeline<KS, false>(p, L, smem, tmem, n, g_begin, g_end, m, ions, phase, exch, cand, s_full, s_done, s_free, s_epi, s_tfree);
+        auto run = [&](const Seq &sq) {
+            if (n > p.cap) run_pipeline<KS, true, kHalf>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps);
+            else run_pipeline<KS, false, kHalf>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps);
+        };
+        // half-grid mode: sub-ranges of kSubGroups groups, each followed by the fix-up groups of its flagged pairs
+        const int sub = kHalf ? kSubGroups : (g_end - g_begin);
+        bool overflow = false;
+        for (int sg = g_begin; sg < g_end; sg += sub) {
+            Seq sq;
+            sq.mode = 0; sq.g0 = sg; sq.ngrp = min(sub, g_end - sg); sq.grp_base = grp_total; sq.nfix = 0;
+            run(sq);
+            grp_total += sq.ngrp;
+            if (kHalf) {
+                __syncthreads();                           // every epilogue of the sub-range is done, the list is complete
+                const int nf = s_nfix;
+                __syncthreads();
+                if (tid == 0) s_nfix = 0;
+                if (nf > kFixCap) overflow = true;         // pathological input: the FFT kernel redoes this material point
+                sq.mode = 1; sq.nfix = min(nf, kFixCap); sq.ngrp = (sq.nfix + 31) >> 5; sq.grp_base = grp_total;
+                if (sq.ngrp) run(sq);
+                grp_total += sq.ngrp;
+                __syncthreads();                           // the list is consumed before the next sub-range appends
+            }
+        }
+        if (overflow && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
+        // the bulk copies that clear the buffers after their last use must land before the CTA gives up its shared memory
+        if (warp == kClrWarp && grp_total > 0) {
+            const int npass = n > 2048 ? (n + 2047) / 2048 : 1, items = grp_total * npass;
+            if (n > p.cap) {
+                mbar_wait(&s_free[0], (uint32_t)((items - 1) & 1));
+            } else {
+                const int u0 = (items + 1) >> 1, u1 = items >> 1;
+                if (u0) mbar_wait(&s_free[0], (uint32_t)((u0 - 1) & 1));
+                if (u1) mbar_wait(&s_free[1], (uint32_t)((u1 - 1) & 1));
+            }
+        }
     }
     // ---- teardown ---------------------------------------------------------------------------------
     asm volatile("tcgen05.fence::before_thread_sync;");
@@ -608,7 +683,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
 static int mma_n_for(int W) { return ((4 * W + 15) / 16) * 16; }
 static int mma_cap_for(int B, int N, int W)
 {
-    const int budget = 232448 - 512;   // 227 KB opt-in shared memory per CTA on sm_100, minus static shared
+    const int budget = 232448 - 1280;  // 227 KB opt-in shared memory per CTA on sm_100, minus static shared (barriers, fix list)
     MmaSmem s = mma_smem_layout(B, N, W, 0);
     int cap = ((budget - (int)s.total) / 12) & ~63;
     return cap > 4096 ? 4096 : cap;
@@ -743,24 +818,75 @@ cudaError_t mma_path_prepare(Plan *p)
     std::vector<float> nps((size_t)3 * p->D);
     e = cudaMemcpy(nps.data(), p->d_dirs_scaled, nps.size() * 4, cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) return e;
-    // paired patch order, padded to a multiple of 32 (padding slots repeat direction 0, perm = -1)
-    const std::vector<int> perm = pair_order(nps, p->D);
-    const int Dp = (int)perm.size();
-    std::vector<float> sorted((size_t)3 * Dp);
-    for (int i = 0; i < Dp; ++i) {
-        const int src = perm[i] >= 0 ? perm[i] : 0;
-        for (int a = 0; a < 3; ++a) sorted[3 * (size_t)i + a] = nps[3 * (size_t)src + a];
+    // Antipodally symmetric grid (every direction has its exact negative in the grid, e.g. the paper's geodesic mesh):
+    // half-grid mode bins one member of every pair and writes its result to both directions.
+    const int D = p->D;
+    std::vector<int> partner((size_t)D, -1);
+    bool sym = !p->need_clamp && !(p->desc.flags & APX_FLAG_NO_PAIRING) && D >= 2 && D % 2 == 0;
+    if (sym) {
+        auto key = [&](int i, float sgn) {
+            std::array<uint32_t, 3> k;
+            for (int a = 0; a < 3; ++a) {
+                float v = sgn * nps[3 * (size_t)i + a];
+                if (v == 0.0f) v = 0.0f;                         // -0 and +0 are the same direction component
+                std::memcpy(&k[a], &v, 4);
+            }
+            return k;
+        };
+        std::map<std::array<uint32_t, 3>, int> index;
+        for (int i = 0; i < D && sym; ++i)
+            if (!index.emplace(key(i, 1.0f), i).second) sym = false;      // duplicate direction
+        for (int i = 0; i < D && sym; ++i) {
+            auto it = index.find(key(i, -1.0f));
+            if (it == index.end() || it->second == i) sym = false;
+            else partner[i] = it->second;
+        }
     }
-    for (int i = 0; i < Dp; ++i)                         // a padding slot of set B mirrors its set-A partner
-        if ((i & 16) && perm[i] < 0)
-            for (int a = 0; a < 3; ++a) sorted[3 * (size_t)i + a] = -sorted[3 * (size_t)(i - 16) + a];
-    // paired mode: every set-B direction is the exact negative of its set-A partner (antipodally symmetric grid)
-    bool paired = !p->need_clamp && !(p->desc.flags & APX_FLAG_NO_PAIRING);
-    for (int i = 0; i < Dp && paired; ++i)
-        if (i & 16)
-            for (int a = 0; a < 3; ++a)
-                if (!(sorted[3 * (size_t)i + a] == -sorted[3 * (size_t)(i - 16) + a])) paired = false;
-    p->mma_paired = paired ? 1 : 0;
+    std::vector<int> perm, mirror;
+    std::vector<float> sorted;
+    if (sym) {
+        // one representative per pair (the member on the upper hemisphere), ordered into compact patches of 16 by the same
+        // bisection; a group = patch 2g as it is (set A) and patch 2g+1 NEGATED (set B): the two neighbouring patches then
+        // project an ion to x and roughly -x, which puts their histogram rows on different shared-memory banks
+        std::vector<FoldedDir> P, Q;
+        for (int i = 0; i < D; ++i) {
+            const float x = nps[3 * (size_t)i], y = nps[3 * (size_t)i + 1], z = nps[3 * (size_t)i + 2];
+            const bool up = z > 0.f || (z == 0.f && (y > 0.f || (y == 0.f && x > 0.f)));
+            if (!up) continue;
+            FoldedDir d;
+            d.idx = i;
+            for (int a = 0; a < 3; ++a) d.f[a] = nps[3 * (size_t)i + a];
+            P.push_back(d);
+        }
+        if ((int)P.size() * 2 != D) sym = false;
+        else {
+            const int npairs = (int)P.size(), leaves = (npairs + 15) / 16, ngroups = (leaves + 1) / 2;
+            pair_bisect(P, Q, 0, leaves * 16);
+            perm.assign((size_t)ngroups * 32, -1);
+            mirror.assign((size_t)ngroups * 32, -1);
+            sorted.assign((size_t)ngroups * 32 * 3, 0.0f);
+            for (int sl = 0; sl < ngroups * 32; ++sl)          // padding: any valid vector
+                for (int a = 0; a < 3; ++a) sorted[3 * (size_t)sl + a] = nps[a];
+            for (int i = 0; i < npairs; ++i) {
+                const int j = i / 16, e = i % 16, sl = (j / 2) * 32 + (j & 1) * 16 + e;
+                const int own = (j & 1) ? partner[P[i].idx] : P[i].idx;
+                perm[sl] = own; mirror[sl] = partner[own];
+                for (int a = 0; a < 3; ++a) sorted[3 * (size_t)sl + a] = nps[3 * (size_t)own + a];
+            }
+        }
+    }
+    if (!sym) {
+        // paired patch order, padded to a multiple of 32 (padding slots repeat direction 0, perm = -1)
+        perm = pair_order(nps, p->D);
+        mirror.clear();
+        sorted.assign(perm.size() * 3, 0.0f);
+        for (size_t i = 0; i < perm.size(); ++i) {
+            const int src = perm[i] >= 0 ? perm[i] : 0;
+            for (int a = 0; a < 3; ++a) sorted[3 * i + a] = nps[3 * (size_t)src + a];
+        }
+    }
+    const int Dp = (int)perm.size();
+    p->mma_paired = sym ? 1 : 0;
     p->Dp = Dp;
     e = cudaMalloc(&p->d_dirs_sorted, sorted.size() * 4);
     if (e != cudaSuccess) return e;
@@ -768,26 +894,38 @@ cudaError_t mma_path_prepare(Plan *p)
     if (e != cudaSuccess) return e;
     e = cudaMemcpy(p->d_dirs_sorted, sorted.data(), sorted.size() * 4, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return e;
-    return cudaMemcpy(p->d_dir_perm, perm.data(), perm.size() * 4, cudaMemcpyHostToDevice);
+    e = cudaMemcpy(p->d_dir_perm, perm.data(), perm.size() * 4, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess || !sym) return e;
+    e = cudaMalloc(&p->d_dir_perm_mirror, mirror.size() * 4);
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(p->d_dir_perm_mirror, mirror.data(), mirror.size() * 4, cudaMemcpyHostToDevice);
 }
 
 cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts, cudaStream_t st)
 {
     if (M == 0) return cudaSuccess;
     // deferred list (material points whose ROI overflows the shared ion buffer), grown on demand
-    if (M + 1 > p->cap_deferred) {
+    int nchunks = 1;                                       // one gather per material point when there are enough of them
+    const int ngroups_all = p->Dp / 32;
+    const int64_t want = (int64_t)p->sm_count * 8;
+    if (M * nchunks < want) nchunks = (int)((want + M - 1) / M);
+    if (nchunks > (ngroups_all + 1) / 2) nchunks = (ngroups_all + 1) / 2;
+    if (nchunks < 1) nchunks = 1;
+    if (nchunks > 1 && nchunks < 6 && (ngroups_all >> (nchunks + 1)) >= 2) ++nchunks;   // one more, smaller, tail chunk
+    const int64_t need_deferred = M * (nchunks + 1) + 1;   // ROIs too large (<= M) + fix-list overflows (<= 1 per CTA)
+    if (need_deferred > p->cap_deferred) {
         if (p->d_deferred) cudaFree(p->d_deferred);
         p->d_deferred = nullptr; p->cap_deferred = 0;
-        cudaError_t e = cudaMalloc(&p->d_deferred, (size_t)(M + 1) * 4);
+        cudaError_t e = cudaMalloc(&p->d_deferred, (size_t)need_deferred * 4);
         if (e != cudaSuccess) return e;
-        p->cap_deferred = M + 1;
+        p->cap_deferred = need_deferred;
     }
     cudaError_t e = cudaMemsetAsync(p->d_deferred, 0, 4, st);
     if (e != cudaSuccess) return e;
 
     MmaParams q;
     q.sorted = p->d_sorted; q.cell_start = p->d_cell_start; q.grid = p->d_grid; q.centres = centres;
-    q.dirs_sorted = p->d_dirs_sorted; q.perm = p->d_dir_perm;
+    q.dirs_sorted = p->d_dirs_sorted; q.perm = p->d_dir_perm; q.perm_mirror = p->mma_paired ? p->d_dir_perm_mirror : nullptr;
     q.table = reinterpret_cast<const uint4 *>(p->d_mma_table); q.phase = p->d_mma_phase; q.zeros = p->d_mma_zero;
     q.sig = reinterpret_cast<float2 *>(sig); q.counts = counts; q.deferred = p->d_deferred;
     q.D = p->D; q.B = p->B; q.k_lo = p->k_lo; q.W = p->W; q.N = mma_n_for(p->W);
@@ -796,16 +934,10 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.cap = mma_cap_for(p->B, q.N, p->W);
     q.cap_big = std::min(8192, q.cap + (int)((size_t)(p->B / 32) * kGroupBytes / 12));
     q.ngroups = p->Dp / 32;
-    int nchunks = 1;                                       // one gather per material point when there are enough of them
-    const int64_t want = (int64_t)p->sm_count * 8;
-    if (M * nchunks < want) nchunks = (int)((want + M - 1) / M);
-    if (nchunks > (q.ngroups + 1) / 2) nchunks = (q.ngroups + 1) / 2;
-    if (nchunks < 1) nchunks = 1;
-    if (nchunks > 1 && nchunks < 6 && (q.ngroups >> (nchunks + 1)) >= 2) ++nchunks;   // one more, smaller, tail chunk
     q.nchunks = nchunks;
     q.M = (int)M;
     q.clamp = p->need_clamp;
-    q.paired = p->mma_paired;
+    q.half = p->mma_paired;
     uint32_t cols = 32;
     while (cols < (uint32_t)(2 * q.N)) cols *= 2;
     q.tmem_cols = cols;
@@ -819,9 +951,15 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
         kern<<<(unsigned)blocks, kMmaThreads, L.total, st>>>(q);
         return cudaSuccess;
     };
-    if (p->B == 1024) e = launch(k_signature_mma<16>);
-    else if (p->B == 512) e = launch(k_signature_mma<8>);
-    else e = launch(k_signature_mma<4>);
+    if (p->mma_paired) {
+        if (p->B == 1024) e = launch(k_signature_mma<16, true>);
+        else if (p->B == 512) e = launch(k_signature_mma<8, true>);
+        else e = launch(k_signature_mma<4, true>);
+    } else {
+        if (p->B == 1024) e = launch(k_signature_mma<16, false>);
+        else if (p->B == 512) e = launch(k_signature_mma<8, false>);
+        else e = launch(k_signature_mma<4, false>);
+    }
     if (e != cudaSuccess) return e;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;

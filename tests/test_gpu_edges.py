@@ -135,31 +135,42 @@ def test_run_host_matches_device_path():
     plan.apx_plan_destroy()
 
 
-@pytest.mark.parametrize("flags", [pytest.param(0, id="paired"), pytest.param(apx.APX_FLAG_NO_PAIRING, id="unpaired")])
-def test_antipodal_pairs_with_exact_integer_projections(flags):
-    """Paired binning of (n, -n) on a symmetric grid: b(-n) = B-1-b(n) holds only while n'.d is not an integer
-    (floor(-x) = -floor(x) - 1); for an exact integer b(-n) = B - b(n).  R = 511/256 makes s = 256 exactly, so ions
-    on a 1/4 grid project to exact integers along the axis directions (+-x, +-y, +-z are vertices of the geodesic
-    grid), an ion sits exactly on every centre (x = +-0 for every direction), and a random half of the cloud does
-    not: a missed special case would shift the grid ions against the rest by one bin and change the amplitudes."""
+@pytest.mark.parametrize("centre_ions", [False, True], ids=["fixups", "overflow"])
+@pytest.mark.parametrize("flags", [pytest.param(0, id="half"), pytest.param(apx.APX_FLAG_NO_PAIRING, id="full")])
+def test_half_grid_mode_with_exact_integer_projections(flags, centre_ions):
+    """Half-grid mode on a symmetric grid: b(-n) = B-1-b(n) holds only while n'.d is not an integer
+    (floor(-x) = -floor(x) - 1); for an exact integer b(-n) = B - b(n), and the kernel must redo -n on its own.
+    R = 511/256 makes s = 256 exactly, so ions on a 1/4 grid project to exact integers along the axis directions
+    (+-x, +-y, +-z are vertices of the geodesic grid) and a random half of the cloud does not: using the mirrored
+    histogram there would shift the grid ions against the rest by one bin and change the amplitudes.  With an ion
+    exactly on each centre (x = +-0 for EVERY direction) the list of flagged pairs overflows and the material
+    points are redone by the general kernel."""
     rng = np.random.Generator(np.random.PCG64(11))
     R, B = 511.0 / 256.0, 1024
+    c2 = np.array([0.25, 0.5, -0.25])
     g = np.arange(-10, 11) / 4.0
     grid = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
     grid = grid[(grid ** 2).sum(1) <= 2.6 ** 2]
-    grid = grid[rng.random(len(grid)) < 0.25]
-    grid = np.concatenate([grid, np.zeros((1, 3)), [[0.25, 0.5, -0.25]]])          # ions exactly on both centres
+    on_centre = ((grid == 0).all(1)) | ((grid == c2).all(1))
+    grid = grid[(rng.random(len(grid)) < 0.25) & ~on_centre]
+    if centre_ions:
+        grid = np.concatenate([grid, np.zeros((1, 3)), c2[None]])
     rnd = rng.uniform(-2.6, 2.6, size=(900, 3))
     xyz = np.concatenate([grid, rnd]).astype(np.float32)
     rng.shuffle(xyz)
     dirs = apx.apx_dirs_geodesic(3)
     assert any((np.abs(d) == (1, 0, 0)).all() for d in dirs)
-    centres = np.array([[0, 0, 0], [0.25, 0.5, -0.25]], np.float32)
+    centres = np.array([[0, 0, 0], c2], np.float32)
     w = _case(xyz, np.zeros(len(xyz), np.uint8), R, B)
-    import torch
     plan = apx.Plan(R, B, dirs, k_lo=15, k_hi=34, device=0, flags=flags)
     assert plan.apx_plan_path() == 1 and plan.apx_plan_paired() == (0 if flags else 1)
     _, s, _ = plan.apx_plan_constants()
     assert s == 256.0
     plan.apx_plan_destroy()
     _check(w, dirs, centres, (15, 34), flags)
+
+
+def test_half_grid_mode_is_off_for_asymmetric_grids():
+    plan = apx.Plan(2.0, 1024, O.dirs_fibonacci(1000), k_lo=15, k_hi=34, device=0)
+    assert plan.apx_plan_path() == 1 and plan.apx_plan_paired() == 0
+    plan.apx_plan_destroy()

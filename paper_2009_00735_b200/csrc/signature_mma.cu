@@ -44,9 +44,23 @@ constexpr int kSvcWarp0 = 18;            // warps 18..25: epilogue (TMEM quarter
 constexpr int kSvcWarps = 8;             // two sets of four warps; set s takes the groups with (group & 1) == s
 constexpr int kMmaWarps = kSvcWarp0 + kSvcWarps;
 constexpr int kMmaThreads = kMmaWarps * 32;
-constexpr int kChunkBytes = 160;         // SBO: 8 directions x 8 rows x 2 B + 32 B skew
-constexpr int kBlkBytes = 640;           // 4 M-chunks: one (blk, kg) slab of 8 K rows x 32 directions
-constexpr int kGroupBytes = 2560;        // LBO: 16 M-chunks = the 4 blk slabs of one 8-row K group
+// Histogram layout, by the number NB of bin parts that sit side by side in the M dimension of the tensor-core operand:
+// b = hi3 * B/8 + NB * kg + blk (blk < NB), M row = blk * G + direction slot, K index = kg * 8 + hi3, K = B / NB.
+//   NB = 4 (B <= 1024): G = 32 slots per group, 16 words per histogram row, two ion streams (half-warps) per warp
+//   NB = 8 (B = 2048) : G = 16 slots per group,  8 words per histogram row, four ion streams (quarter-warps) per warp
+// SBO (bytes between 8-slot M chunks) = 128 + a skew that puts the words of a row on different banks for a common hi3
+// and keeps the stride of `low` (= BLK) a multiple of 128 B, i.e. bank neutral; LBO = 16 M chunks = one 8-row K group.
+template <int NB>
+struct Lay {
+    static constexpr int G = 128 / NB;
+    static constexpr int LW = G / 2;                 // lanes per ion stream = words per histogram row
+    static constexpr int NS = 32 / LW;               // ion streams per warp
+    static constexpr int SBO = NB == 4 ? 160 : 192;
+    static constexpr int BLK = (G / 8) * SBO;        // one (blk, kg) slab: 640 / 384 B
+    static constexpr int LBO = 16 * SBO;             // 2560 / 3072 B
+};
+__host__ __device__ inline int mma_nb_for(int B) { return B > 1024 ? 8 : 4; }
+__host__ __device__ inline int mma_sbo_for(int nb) { return nb == 4 ? 160 : 192; }
 constexpr int kStsClearBelow = 700;      // ROIs with fewer ions clear with plain stores instead of TMA copies from L2
 constexpr int kEpiRound = 4;             // window bins per epilogue round (one tcgen05.ld x16)
 
@@ -130,15 +144,20 @@ __host__ __device__ inline MmaSmem mma_smem_layout(int B, int N, int W, int cap)
 {
     MmaSmem s;
     uint32_t off = 0;
-    s.hist_bytes = (uint32_t)(B / 32) * kGroupBytes;             // K/8 = B/32 K groups of 2560 B
-    s.table = off; off += (uint32_t)(B / 4) * N * 2;             // (K/64) * N * 128 with K = B/4; multiple of 1024
+    const int nb = mma_nb_for(B), K = B / nb;
+    s.hist_bytes = (uint32_t)(K / 8) * 16u * (uint32_t)mma_sbo_for(nb);   // K/8 K groups of LBO bytes
+    s.table = off; off += (uint32_t)K * N * 2;                   // (K/64) * N * 128; multiple of 1024
     s.hist0 = off; off += s.hist_bytes;
-    s.exch = off; off += 2u * kEpiRound * 4 * 32 * 8;             // per set, one epilogue round: 4 bins x 4 blk x 32 slots x float2
+    s.exch = off; off += 2u * kEpiRound * 4 * 32 * 8;             // per set, one epilogue round: 4 bins x 4 warps x 32 lanes x float2
     s.cand = off; off += 8u * 32 * 8;
-    s.phase = off; off += 4u * W * 8;
+    s.phase = off; off += (uint32_t)nb * W * 8;
     s.ions = off; off += (uint32_t)cap * 12;
-    s.hist1 = off; off += s.hist_bytes;                            // directly behind the ion buffer: a ROI with more than
+    if (nb == 4) {
+        s.hist1 = off; off += s.hist_bytes;                        // directly behind the ion buffer: a ROI with more than
                                                                    // `cap` ions spills into it and runs single-buffered
+    } else {
+        s.hist1 = s.hist0;                                         // B = 2048: room for one histogram buffer only
+    }
     s.total = off + 1024;                                          // slack for 1024-byte alignment
     return s;
 }
@@ -199,7 +218,7 @@ __device__ __forceinline__ uint64_t pack2(float lo, float hi)
 }
 struct Detect;
 __device__ void flag_pair(uint32_t *flag, int *nfix, uint16_t *fix, uint32_t bit, uint32_t id);
-template <bool kClamp, bool kDetect>
+template <bool kClamp, bool kDetect, int BLK>
 __device__ __forceinline__ void bin_one(float dx, float dy, float dz, float npx, float npy, float npz, const BinConst &c,
                                         uint32_t k0, uint32_t inc, uint32_t *flag, int *nfix, uint16_t *fix, uint32_t bit, uint32_t id)
 {
@@ -208,7 +227,7 @@ __device__ __forceinline__ void bin_one(float dx, float dy, float dz, float npx,
     const uint32_t ua = __float_as_uint(__fadd_rd(x, c.magic_a));
     if (kDetect && ua == __float_as_uint(__fadd_ru(x, c.magic_a))) flag_pair(flag, nfix, fix, bit, id);
     const uint32_t va = __float_as_uint(__fmaf_rd(x, c.scl, c.magic_b));
-    red_shared_add(ua * (uint32_t)kBlkBytes + (va * c.kz + k0), inc);
+    red_shared_add(ua * (uint32_t)BLK + (va * c.kz + k0), inc);
 }
 // Half-grid mode (antipodally symmetric direction grids such as the geodesic mesh of the paper, L60): only one
 // direction v of every pair (v, -v) is binned.  x(-v) = -x(v) bit for bit (every product and sum is negated exactly), so
@@ -234,7 +253,7 @@ __device__ __noinline__ void flag_pair(uint32_t *flag, int *nfix, uint16_t *fix,
 }
 // two ions (dx0,dx1), (dy0,dy1), (dz0,dz1) for this lane's direction
 // returns (only with kDetect) the number of the two projections that are NOT exact integers
-template <bool kDetect>
+template <bool kDetect, int BLK>
 __device__ __forceinline__ uint32_t bin_pair(float dx0, float dx1, float dy0, float dy1, float dz0, float dz1, uint64_t nx2,
                                          uint64_t ny2, uint64_t nz2, uint64_t ma2, uint64_t sc2, uint64_t mb2, uint32_t kz,
                                          uint32_t k0, uint32_t inc, const Detect &dt)
@@ -246,8 +265,8 @@ __device__ __forceinline__ uint32_t bin_pair(float dx0, float dx1, float dy0, fl
     asm("add.rm.f32x2 %0, %1, %2;" : "=l"(ua) : "l"(t), "l"(ma2));
     asm("fma.rm.f32x2 %0, %1, %2, %3;" : "=l"(va) : "l"(t), "l"(sc2), "l"(mb2));
     const uint32_t ua0 = (uint32_t)ua, ua1 = (uint32_t)(ua >> 32), va0 = (uint32_t)va, va1 = (uint32_t)(va >> 32);
-    red_shared_add(ua0 * (uint32_t)kBlkBytes + (va0 * kz + k0), inc);
-    red_shared_add(ua1 * (uint32_t)kBlkBytes + (va1 * kz + k0), inc);
+    red_shared_add(ua0 * (uint32_t)BLK + (va0 * kz + k0), inc);
+    red_shared_add(ua1 * (uint32_t)BLK + (va1 * kz + k0), inc);
     if (kDetect) {                                       // RU(x + magic) - RD(x + magic) = 1, or 0 for an integer x
         uint64_t up;
         asm("add.rp.f32x2 %0, %1, %2;" : "=l"(up) : "l"(t), "l"(ma2));
@@ -263,17 +282,18 @@ struct LaneDirs {
 // ions_s = shared-space byte address of the quad-blocked ion records; i0 is a multiple of 4.  The two half-warps of a
 // warp take alternate blocks of ions (half h = lane >> 4), every lane bins each of its ions for BOTH of its directions,
 // so one ion load serves two (ion, direction) pairs.
-template <bool kClamp, bool kDetect>
+template <bool kClamp, bool kDetect, int NB>
 __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const LaneDirs &n, const BinConst &c, uint32_t k0,
                                          int h, const Detect &da, const Detect &db)
 {
+    constexpr int NS = Lay<NB>::NS, BLK = Lay<NB>::BLK;
     int ib = i0;
     if (!kClamp) {
         const uint64_t ax2 = pack2(n.ax, n.ax), ay2 = pack2(n.ay, n.ay), az2 = pack2(n.az, n.az);
         const uint64_t bx2 = pack2(n.bx, n.bx), by2 = pack2(n.by, n.by), bz2 = pack2(n.bz, n.bz);
         const uint64_t ma2 = pack2(c.magic_a, c.magic_a), sc2 = pack2(c.scl, c.scl), mb2 = pack2(c.magic_b, c.magic_b);
         uint32_t src = ions_s + (uint32_t)ib * 12u + (uint32_t)h * 96u;
-        for (; ib + 16 <= i1; ib += 16, src += 192u) {       // 8 ions per half-warp = 6 LDS.128, then 8 packed chains
+        for (; ib + 8 * NS <= i1; ib += 8 * NS, src += 96u * NS) {   // 8 ions per stream = 6 LDS.128, then 8 packed chains
             float4 q[6];
 #pragma unroll
             for (int u = 0; u < 6; ++u) q[u] = lds128(src + (uint32_t)u * 16u);
@@ -281,39 +301,39 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
 #pragma unroll
             for (int hh = 0; hh < 2; ++hh) {
                 const float4 X = q[3 * hh], Y = q[3 * hh + 1], Z = q[3 * hh + 2];
-                na += bin_pair<kDetect>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
-                na += bin_pair<kDetect>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
-                nb += bin_pair<kDetect>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
-                nb += bin_pair<kDetect>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
+                na += bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
+                na += bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
+                nb += bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
+                nb += bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
             }
             if (kDetect) {
                 if (__builtin_expect(na != 8u, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
                 if (__builtin_expect(nb != 8u, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
             }
         }
-        if (ib + 8 <= i1) {                                  // one quad per half-warp
+        if (ib + 4 * NS <= i1) {                             // one quad per stream
             const uint32_t a = ions_s + (uint32_t)ib * 12u + (uint32_t)h * 48u;
             const float4 X = lds128(a), Y = lds128(a + 16u), Z = lds128(a + 32u);
             uint32_t na = 0u, nb = 0u;
-            na += bin_pair<kDetect>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
-            na += bin_pair<kDetect>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
-            nb += bin_pair<kDetect>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
-            nb += bin_pair<kDetect>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
+            na += bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
+            na += bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
+            nb += bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
+            nb += bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
             if (kDetect) {
                 if (__builtin_expect(na != 4u, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
                 if (__builtin_expect(nb != 4u, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
             }
-            ib += 8;
+            ib += 4 * NS;
         }
     }
-    for (int i = ib + h; i < i1; i += 2) {                   // ragged tail (and every ion when the clamp is needed)
+    for (int i = ib + h; i < i1; i += NS) {                   // ragged tail (and every ion when the clamp is needed)
         const uint32_t a = ions_s + (uint32_t)(i >> 2) * 48u + (uint32_t)(i & 3) * 4u;
         float dx, dy, dz;
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dx) : "r"(a));
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dy) : "r"(a + 16u));
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(a + 32u));
-        bin_one<kClamp, kDetect>(dx, dy, dz, n.ax, n.ay, n.az, c, k0, 1u, da.flag, da.nfix, da.fix, da.bit, da.id);
-        bin_one<kClamp, kDetect>(dx, dy, dz, n.bx, n.by, n.bz, c, k0, 65536u, db.flag, db.nfix, db.fix, db.bit, db.id);
+        bin_one<kClamp, kDetect, BLK>(dx, dy, dz, n.ax, n.ay, n.az, c, k0, 1u, da.flag, da.nfix, da.fix, da.bit, da.id);
+        bin_one<kClamp, kDetect, BLK>(dx, dy, dz, n.bx, n.by, n.bz, c, k0, 65536u, db.flag, db.nfix, db.fix, db.bit, db.id);
     }
 }
 
@@ -328,7 +348,7 @@ struct EpiOut {
     uint32_t *flag;                      // mode 0, half-grid: flag word of this group (read, then reset)
     const uint16_t *fix;
 };
-template <bool kHalf>
+template <bool kHalf, int NB>
 __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc, const EpiOut &eo, int64_t m, const float2 *phase,
                                                float2 *exch_all, float2 *cand_all, int set, int q, int lane)
 {
@@ -350,8 +370,12 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
             if (w < p.W) {
                 const float re = __uint_as_float(v[4 * j]) + __uint_as_float(v[4 * j + 2]) * (1.0f / 2048.0f);
                 const float im = -(__uint_as_float(v[4 * j + 1]) + __uint_as_float(v[4 * j + 3]) * (1.0f / 2048.0f));
-                const float2 f = phase[q * p.W + w];
-                const float2 P = make_float2(f.x * re - f.y * im, f.x * im + f.y * re);
+                const float2 f = phase[(NB == 4 ? q : 2 * q + (lane >> 4)) * p.W + w];
+                float2 P = make_float2(f.x * re - f.y * im, f.x * im + f.y * re);
+                if (NB == 8) {                           // lanes l and l + 16 hold parts blk = 2q and 2q + 1 of slot l
+                    P.x += __shfl_xor_sync(0xffffffffu, P.x, 16);
+                    P.y += __shfl_xor_sync(0xffffffffu, P.y, 16);
+                }
                 if (j == q) keep = P;
                 else exch[(j * 4 + q) * 32 + lane] = P;
             }
@@ -372,7 +396,8 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
     }
     cand[q * 32 + lane] = make_float2(best, __int_as_float(kbest));
     if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
-    if (q == 0) {
+    if (q == 0 && lane < Lay<NB>::G) {                   // (NB = 8: lanes 16..31 carry copies of lanes 0..15)
+        constexpr int G = Lay<NB>::G;
         if (kHalf && lane == 0 && mode == 0) *eo.flag = 0u;             // every thread of the set has read it (barriers above)
         float bb = -1.0f;
         int kb = p.k_lo;
@@ -382,19 +407,20 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
             const int ck = __float_as_int(c2.y);
             if (c2.x > bb || (c2.x == bb && ck < kb)) { bb = c2.x; kb = ck; }
         }
-        const int slot = ((lane & 1) << 4) + ((lane >> 3) << 2) + ((lane & 7) >> 1);
+        // M row (within a part) = chunk * 8 + word * 2 + half  ->  slot = half * G/2 + chunk * 4 + word
+        const int slot = (lane & 1) * (G / 2) + ((lane >> 3) << 2) + ((lane & 7) >> 1);
         const float2 res = make_float2(16777216.0f * sqrtf(fmaxf(bb, 0.0f)), (float)kb);
         if (mode == 0) {
-            const int d = p.perm[eo.gi * 32 + slot];
+            const int d = p.perm[eo.gi * G + slot];
             if (d >= 0) p.sig[(size_t)m * p.D + d] = res;
             if (kHalf && !((mask >> slot) & 1u)) {               // the mirrored histogram has the same amplitude spectrum
-                const int d2 = p.perm_mirror[eo.gi * 32 + slot];
+                const int d2 = p.perm_mirror[eo.gi * G + slot];
                 if (d2 >= 0) p.sig[(size_t)m * p.D + d2] = res;
             }
         } else {
-            const int e = eo.f * 32 + slot;
+            const int e = eo.f * G + slot;
             if (e < eo.nfix) {
-                const int d2 = p.perm_mirror[eo.g0 * 32 + (int)eo.fix[e]];
+                const int d2 = p.perm_mirror[eo.g0 * G + (int)eo.fix[e]];
                 if (d2 >= 0) p.sig[(size_t)m * p.D + d2] = res;
             }
         }
@@ -419,7 +445,7 @@ struct PipeShared {
 
 // The warp-specialised pipeline of one (material point, chunk).  kBig: the ROI's ions have spilled into the second
 // histogram buffer, so only buffer 0 is used and bin -> transform -> clear are serial per item.
-template <int KS, bool kBig, bool kHalf>
+template <int KS, int NB, bool kBig, bool kHalf>
 __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &L, unsigned char *smem, uint32_t tmem, int n_ions,
                                              const Seq &sq, int64_t m, const float *ions, const float2 *phase,
                                              float2 *exch, float2 *cand, const PipeShared &ps)
@@ -443,22 +469,23 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         BinConst c;
         c.half_b = (float)(p.B / 2); c.magic_a = magic_for(p.B); c.magic_b = 12582912.0f + 4.0f;
         c.scl = __int_as_float((127 - p.nl) << 23);                       // 2^-nl
-        c.kz = 16u - (uint32_t)kBlkBytes * (1u << p.nl);
-        const int l = lane & 15, h = lane >> 4;
-        const uint32_t k0base = smem_u32(smem + L.hist0) + (uint32_t)(l >> 2) * kChunkBytes + (uint32_t)(l & 3) * 4u
-                                - 0x4B400000u * (uint32_t)kBlkBytes - 0x4B400000u * c.kz;
+        constexpr int G = Lay<NB>::G, LW = Lay<NB>::LW;
+        c.kz = 16u - (uint32_t)Lay<NB>::BLK * (1u << p.nl);
+        const int l = lane & (LW - 1), h = lane / LW;
+        const uint32_t k0base = smem_u32(smem + L.hist0) + (uint32_t)(l >> 2) * Lay<NB>::SBO + (uint32_t)(l & 3) * 4u
+                                - 0x4B400000u * (uint32_t)Lay<NB>::BLK - 0x4B400000u * c.kz;
         const uint32_t ions_s = smem_u32(ions);
         const bool detect = kHalf && mode == 0;
         for (int it = 0, gl = 0, pass = 0; it < nitems; ++it) {
             const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
             LaneDirs n;
             if (mode == 0) {
-                const float *da = p.dirs_sorted + (size_t)((sq.g0 + gl) * 32 + l) * 3;
-                n.ax = da[0]; n.ay = da[1]; n.az = da[2]; n.bx = da[48]; n.by = da[49]; n.bz = da[50];
+                const float *da = p.dirs_sorted + (size_t)((sq.g0 + gl) * G + l) * 3;
+                n.ax = da[0]; n.ay = da[1]; n.az = da[2]; n.bx = da[3 * LW]; n.by = da[3 * LW + 1]; n.bz = da[3 * LW + 2];
             } else {                                                     // the opposite of a flagged pair's direction
-                const int ea = gl * 32 + l, eb = ea + 16;
-                const float *da = p.dirs_sorted + (ea < sq.nfix ? (size_t)(sq.g0 * 32 + (int)ps.fix[ea]) * 3 : 0);
-                const float *db = p.dirs_sorted + (eb < sq.nfix ? (size_t)(sq.g0 * 32 + (int)ps.fix[eb]) * 3 : 0);
+                const int ea = gl * G + l, eb = ea + LW;
+                const float *da = p.dirs_sorted + (ea < sq.nfix ? (size_t)(sq.g0 * G + (int)ps.fix[ea]) * 3 : 0);
+                const float *db = p.dirs_sorted + (eb < sq.nfix ? (size_t)(sq.g0 * G + (int)ps.fix[eb]) * 3 : 0);
                 n.ax = -da[0]; n.ay = -da[1]; n.az = -da[2]; n.bx = -db[0]; n.by = -db[1]; n.bz = -db[2];
             }
             if (use >= 1) mbar_wait(&ps.free_[buf], (uint32_t)((use - 1) & 1));       // cleared after its previous use
@@ -470,13 +497,13 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             if (detect) {
                 dta.flag = dtb.flag = &ps.flag[(sq.grp_base + gl) & 3];
                 dta.nfix = dtb.nfix = ps.nfix; dta.fix = dtb.fix = ps.fix;
-                dta.bit = 1u << l; dtb.bit = 65536u << l;
-                dta.id = (uint32_t)(gl * 32 + l); dtb.id = dta.id + 16u;
-                bin_ions<false, true>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
+                dta.bit = 1u << l; dtb.bit = 1u << (LW + l);
+                dta.id = (uint32_t)(gl * G + l); dtb.id = dta.id + (uint32_t)LW;
+                bin_ions<false, true, NB>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
             } else if (p.clamp) {
-                bin_ions<true, false>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
+                bin_ions<true, false, NB>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
             } else {
-                bin_ions<false, false>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
+                bin_ions<false, false, NB>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
             __syncwarp();
@@ -487,8 +514,8 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         // ---- MMA warp: descriptors advance by adding to the 14-bit start-address field ---------------
         const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(p.N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
         const uint32_t tb = smem_u32(smem + L.table), hb = smem_u32(smem + L.hist0);
-        const uint32_t a_hi = (uint32_t)(kChunkBytes >> 4) | (1u << 14);                         // SBO, version 1, INTERLEAVE
-        const uint32_t a_lo0 = ((hb >> 4) & 0x3FFFu) | ((uint32_t)(kGroupBytes >> 4) << 16);       // LBO = 2560 B
+        const uint32_t a_hi = (uint32_t)(Lay<NB>::SBO >> 4) | (1u << 14);                        // SBO, version 1, INTERLEAVE
+        const uint32_t a_lo0 = ((hb >> 4) & 0x3FFFu) | ((uint32_t)(Lay<NB>::LBO >> 4) << 16);      // LBO
         const uint32_t b_hi = (uint32_t)(1024 >> 4) | (1u << 14) | (2u << 29);                     // SBO, version 1, SWIZZLE_128B
         const uint32_t b_lo0 = ((tb >> 4) & 0x3FFFu) | (1u << 16);
         const uint32_t kblk_step = (uint32_t)(p.N * 128) >> 4;
@@ -503,7 +530,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                 const uint32_t a_lo = a_lo0 + (uint32_t)buf * ((L.hist1 - L.hist0) >> 4);
 #pragma unroll
                 for (int ks = 0; ks < KS; ++ks) {
-                    const uint64_t ad = ((uint64_t)a_hi << 32) | (a_lo + (uint32_t)ks * ((2 * kGroupBytes) >> 4));
+                    const uint64_t ad = ((uint64_t)a_hi << 32) | (a_lo + (uint32_t)ks * ((2 * Lay<NB>::LBO) >> 4));
                     const uint64_t bd = ((uint64_t)b_hi << 32) | (b_lo0 + (uint32_t)(ks >> 2) * kblk_step + (uint32_t)(ks & 3) * 2u);
                     if (ks == 0) mma_f16_ss(acc, ad, bd, idesc, pass > 0 ? 1u : 0u);
                     else mma_f16_acc(acc, ad, bd, idesc);
@@ -550,7 +577,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             EpiOut eo;
             eo.mode = mode; eo.gi = sq.g0 + gl; eo.g0 = sq.g0; eo.f = gl; eo.nfix = sq.nfix;
             eo.flag = kHalf ? &ps.flag[gq & 3] : nullptr; eo.fix = ps.fix;
-            epilogue_group<kHalf>(p, tmem + (uint32_t)(set * p.N), eo, m, phase, exch, cand, set, q, lane);
+            epilogue_group<kHalf, NB>(p, tmem + (uint32_t)(set * p.N), eo, m, phase, exch, cand, set, q, lane);
             asm volatile("tcgen05.fence::before_thread_sync;");
             __syncwarp();
             if (lane == 0) mbar_arrive(&ps.tfree[set]);
@@ -558,7 +585,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
     }
 }
 
-template <int KS, bool kHalf>   // KS = K/16 = B/64 k-steps per group; kHalf = half-grid mode
+template <int KS, int NB, bool kHalf>   // KS = K/16 k-steps per group, NB = bin parts (layout), kHalf = half-grid mode
 __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParams p)
 {
     extern __shared__ unsigned char smem_raw[];
@@ -613,10 +640,13 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     }
     {
         uint4 *h0 = reinterpret_cast<uint4 *>(smem + L.hist0), *h1 = reinterpret_cast<uint4 *>(smem + L.hist1);
-        for (int i = tid; i < (int)(L.hist_bytes / 16); i += kMmaThreads) { h0[i] = make_uint4(0, 0, 0, 0); h1[i] = make_uint4(0, 0, 0, 0); }
+        for (int i = tid; i < (int)(L.hist_bytes / 16); i += kMmaThreads) {
+            h0[i] = make_uint4(0, 0, 0, 0);
+            if (NB == 4) h1[i] = make_uint4(0, 0, 0, 0);
+        }
         uint4 *t = reinterpret_cast<uint4 *>(smem + L.table);
         for (int i = tid; i < K * p.N / 8; i += kMmaThreads) t[i] = p.table[i];
-        for (int i = tid; i < 4 * p.W; i += kMmaThreads) phase[i] = p.phase[i];
+        for (int i = tid; i < NB * p.W; i += kMmaThreads) phase[i] = p.phase[i];
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     asm volatile("tcgen05.fence::before_thread_sync;");
@@ -637,8 +667,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
         if (chunk == 0 && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
     } else {
         auto run = [&](const Seq &sq) {
-            if (n > p.cap) run_pipeline<KS, true, kHalf>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps);
-            else run_pipeline<KS, false, kHalf>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps);
+            if (NB == 8 || n > p.cap) run_pipeline<KS, NB, true, kHalf>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps);
+            else run_pipeline<KS, NB, false, kHalf>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps);
         };
         // half-grid mode: sub-ranges of kSubGroups groups, each followed by the fix-up groups of its flagged pairs
         const int sub = kHalf ? kSubGroups : (g_end - g_begin);
@@ -654,7 +684,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
                 __syncthreads();
                 if (tid == 0) s_nfix = 0;
                 if (nf > kFixCap) overflow = true;         // pathological input: the FFT kernel redoes this material point
-                sq.mode = 1; sq.nfix = min(nf, kFixCap); sq.ngrp = (sq.nfix + 31) >> 5; sq.grp_base = grp_total;
+                sq.mode = 1; sq.nfix = min(nf, kFixCap); sq.ngrp = (sq.nfix + Lay<NB>::G - 1) / Lay<NB>::G; sq.grp_base = grp_total;
                 if (sq.ngrp) run(sq);
                 grp_total += sq.ngrp;
                 __syncthreads();                           // the list is consumed before the next sub-range appends
@@ -664,7 +694,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
         // the bulk copies that clear the buffers after their last use must land before the CTA gives up its shared memory
         if (warp == kClrWarp && grp_total > 0) {
             const int npass = n > 2048 ? (n + 2047) / 2048 : 1, items = grp_total * npass;
-            if (n > p.cap) {
+            if (NB == 8 || n > p.cap) {
                 mbar_wait(&s_free[0], (uint32_t)((items - 1) & 1));
             } else {
                 const int u0 = (items + 1) >> 1, u1 = items >> 1;
@@ -691,7 +721,7 @@ static int mma_cap_for(int B, int N, int W)
 
 bool mma_path_supported(const Plan *p)
 {
-    if (p->B > 1024) return false;                       // B = 2048, 4096 stay on the FFT kernel
+    if (p->B > 2048) return false;                       // B = 4096 stays on the FFT kernel
     const int N = mma_n_for(p->W);
     if (2 * N > 512) return false;                       // two accumulators of N TMEM columns
     return mma_cap_for(p->B, N, p->W) >= 1024;           // room for a useful ion buffer
@@ -709,14 +739,14 @@ struct FoldedDir {
     float f[3];
     int idx;
 };
-static void pair_bisect(std::vector<FoldedDir> &P, std::vector<FoldedDir> &Q, int lo, int hi)
+static void pair_bisect(std::vector<FoldedDir> &P, std::vector<FoldedDir> &Q, int lo, int hi, int leaf)
 {
     const int cnt = hi - lo;
     const int pe = std::min(hi, (int)P.size()), qe = std::min(hi, (int)Q.size());
     auto lex = [](const FoldedDir &a, const FoldedDir &b) {
         return a.f[0] != b.f[0] ? a.f[0] < b.f[0] : (a.f[1] != b.f[1] ? a.f[1] < b.f[1] : a.f[2] < b.f[2]);
     };
-    if (cnt <= 16) {                                     // leaf: same slot order on both sides (exact antipodes line up)
+    if (cnt <= leaf) {                                   // leaf: same slot order on both sides (exact antipodes line up)
         if (lo < pe) std::sort(P.begin() + lo, P.begin() + pe, lex);
         if (lo < qe) std::sort(Q.begin() + lo, Q.begin() + qe, lex);
         return;
@@ -729,16 +759,16 @@ static void pair_bisect(std::vector<FoldedDir> &P, std::vector<FoldedDir> &Q, in
     int ax = 0;
     for (int a = 1; a < 3; ++a)
         if (mx[a] - mn[a] > mx[ax] - mn[ax]) ax = a;
-    const int leaves = (cnt + 15) / 16;
-    const int mid = lo + (leaves / 2) * 16;
+    const int leaves = (cnt + leaf - 1) / leaf;
+    const int mid = lo + (leaves / 2) * leaf;
     auto cmp = [&](const FoldedDir &a, const FoldedDir &b) { return a.f[ax] != b.f[ax] ? a.f[ax] < b.f[ax] : lex(a, b); };
     if (mid < pe) std::nth_element(P.begin() + lo, P.begin() + mid, P.begin() + pe, cmp);
     if (mid < qe) std::nth_element(Q.begin() + lo, Q.begin() + mid, Q.begin() + qe, cmp);
-    pair_bisect(P, Q, lo, mid);
-    pair_bisect(P, Q, mid, hi);
+    pair_bisect(P, Q, lo, mid, leaf);
+    pair_bisect(P, Q, mid, hi, leaf);
 }
 // v = [D][3]; returns the slot order (original index per slot, -1 = padding), length = multiple of 32
-static std::vector<int> pair_order(const std::vector<float> &v, int D)
+static std::vector<int> pair_order(const std::vector<float> &v, int D, int leaf)
 {
     std::vector<FoldedDir> P, Q;
     for (int i = 0; i < D; ++i) {
@@ -760,21 +790,22 @@ static std::vector<int> pair_order(const std::vector<float> &v, int D)
     move_surplus(P, Q);
     move_surplus(Q, P);
     const int cnt = (int)std::max(P.size(), Q.size());
-    const int leaves = (cnt + 15) / 16;
-    if (leaves > 0) pair_bisect(P, Q, 0, leaves * 16);
-    std::vector<int> slots((size_t)leaves * 32, -1);
+    const int leaves = (cnt + leaf - 1) / leaf;
+    if (leaves > 0) pair_bisect(P, Q, 0, leaves * leaf, leaf);
+    std::vector<int> slots((size_t)leaves * 2 * leaf, -1);
     for (int j = 0; j < leaves; ++j)
-        for (int e = 0; e < 16; ++e) {
-            const int i = j * 16 + e;
-            if (i < (int)P.size()) slots[(size_t)j * 32 + e] = P[i].idx;
-            if (i < (int)Q.size()) slots[(size_t)j * 32 + 16 + e] = Q[i].idx;
+        for (int e = 0; e < leaf; ++e) {
+            const int i = j * leaf + e;
+            if (i < (int)P.size()) slots[(size_t)j * 2 * leaf + e] = P[i].idx;
+            if (i < (int)Q.size()) slots[(size_t)j * 2 * leaf + leaf + e] = Q[i].idx;
         }
     return slots;
 }
 
 cudaError_t mma_path_prepare(Plan *p)
 {
-    const int B = p->B, K = B / 4, W = p->W, N = mma_n_for(W);
+    const int B = p->B, nb = mma_nb_for(B), K = B / nb, W = p->W, N = mma_n_for(W);
+    const int G = 128 / nb, leaf = G / 2;               // slots per group, directions per patch
     int nl = 0;
     while ((8 << nl) < B) ++nl;                          // B = 8 * 2^nl
     // twiddle table: K index k = kg*8 + hi3 stands for the bin part hi3*(B/8) + 4*kg
@@ -784,7 +815,7 @@ cudaError_t mma_path_prepare(Plan *p)
             const int w = n / 4, c = n % 4;
             __half val = __float2half(0.0f);
             if (w < W) {
-                const int64_t binpart = (int64_t)(r & 7) * (B / 8) + 4 * (r >> 3);
+                const int64_t binpart = (int64_t)(r & 7) * (B / 8) + nb * (r >> 3);
                 const double th = 2.0 * M_PI * (double)((binpart * (p->k_lo + w)) % B) / (double)B;
                 const double v = (c & 1) ? std::sin(th) : std::cos(th);
                 const __half hi = __float2half((float)v);
@@ -799,8 +830,8 @@ cudaError_t mma_path_prepare(Plan *p)
     e = cudaMemcpy(p->d_mma_table, img.data(), img.size() * 2, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return e;
     // recombination phases exp(-2 pi i blk k / B), blk = 0..3
-    std::vector<float2> ph((size_t)4 * W);
-    for (int pb = 0; pb < 4; ++pb)
+    std::vector<float2> ph((size_t)nb * W);
+    for (int pb = 0; pb < nb; ++pb)
         for (int w = 0; w < W; ++w) {
             const int64_t off = pb;
             const double th = 2.0 * M_PI * (double)((off * (p->k_lo + w)) % B) / (double)B;
@@ -811,9 +842,10 @@ cudaError_t mma_path_prepare(Plan *p)
     e = cudaMemcpy(p->d_mma_phase, ph.data(), ph.size() * sizeof(float2), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return e;
 
-    e = cudaMalloc(&p->d_mma_zero, (size_t)(B / 32) * kGroupBytes);
+    const size_t hist_bytes = mma_smem_layout(B, N, W, 0).hist_bytes;
+    e = cudaMalloc(&p->d_mma_zero, hist_bytes);
     if (e != cudaSuccess) return e;
-    e = cudaMemset(p->d_mma_zero, 0, (size_t)(B / 32) * kGroupBytes);
+    e = cudaMemset(p->d_mma_zero, 0, hist_bytes);
     if (e != cudaSuccess) return e;
     std::vector<float> nps((size_t)3 * p->D);
     e = cudaMemcpy(nps.data(), p->d_dirs_scaled, nps.size() * 4, cudaMemcpyDeviceToHost);
@@ -860,15 +892,15 @@ cudaError_t mma_path_prepare(Plan *p)
         }
         if ((int)P.size() * 2 != D) sym = false;
         else {
-            const int npairs = (int)P.size(), leaves = (npairs + 15) / 16, ngroups = (leaves + 1) / 2;
-            pair_bisect(P, Q, 0, leaves * 16);
-            perm.assign((size_t)ngroups * 32, -1);
-            mirror.assign((size_t)ngroups * 32, -1);
-            sorted.assign((size_t)ngroups * 32 * 3, 0.0f);
-            for (int sl = 0; sl < ngroups * 32; ++sl)          // padding: any valid vector
+            const int npairs = (int)P.size(), leaves = (npairs + leaf - 1) / leaf, ngroups = (leaves + 1) / 2;
+            pair_bisect(P, Q, 0, leaves * leaf, leaf);
+            perm.assign((size_t)ngroups * G, -1);
+            mirror.assign((size_t)ngroups * G, -1);
+            sorted.assign((size_t)ngroups * G * 3, 0.0f);
+            for (int sl = 0; sl < ngroups * G; ++sl)           // padding: any valid vector
                 for (int a = 0; a < 3; ++a) sorted[3 * (size_t)sl + a] = nps[a];
             for (int i = 0; i < npairs; ++i) {
-                const int j = i / 16, e = i % 16, sl = (j / 2) * 32 + (j & 1) * 16 + e;
+                const int j = i / leaf, e = i % leaf, sl = (j / 2) * G + (j & 1) * leaf + e;
                 const int own = (j & 1) ? partner[P[i].idx] : P[i].idx;
                 perm[sl] = own; mirror[sl] = partner[own];
                 for (int a = 0; a < 3; ++a) sorted[3 * (size_t)sl + a] = nps[3 * (size_t)own + a];
@@ -877,7 +909,7 @@ cudaError_t mma_path_prepare(Plan *p)
     }
     if (!sym) {
         // paired patch order, padded to a multiple of 32 (padding slots repeat direction 0, perm = -1)
-        perm = pair_order(nps, p->D);
+        perm = pair_order(nps, p->D, leaf);
         mirror.clear();
         sorted.assign(perm.size() * 3, 0.0f);
         for (size_t i = 0; i < perm.size(); ++i) {
@@ -906,7 +938,8 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     if (M == 0) return cudaSuccess;
     // deferred list (material points whose ROI overflows the shared ion buffer), grown on demand
     int nchunks = 1;                                       // one gather per material point when there are enough of them
-    const int ngroups_all = p->Dp / 32;
+    const int slots_per_group = 128 / mma_nb_for(p->B);
+    const int ngroups_all = p->Dp / slots_per_group;
     const int64_t want = (int64_t)p->sm_count * 8;
     if (M * nchunks < want) nchunks = (int)((want + M - 1) / M);
     if (nchunks > (ngroups_all + 1) / 2) nchunks = (ngroups_all + 1) / 2;
@@ -932,8 +965,9 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.nl = 0;
     while ((8 << q.nl) < p->B) ++q.nl;
     q.cap = mma_cap_for(p->B, q.N, p->W);
-    q.cap_big = std::min(8192, q.cap + (int)((size_t)(p->B / 32) * kGroupBytes / 12));
-    q.ngroups = p->Dp / 32;
+    const MmaSmem L0 = mma_smem_layout(p->B, q.N, p->W, q.cap);
+    q.cap_big = L0.hist1 == L0.hist0 ? q.cap : std::min(8192, q.cap + (int)(L0.hist_bytes / 12));
+    q.ngroups = p->Dp / slots_per_group;
     q.nchunks = nchunks;
     q.M = (int)M;
     q.clamp = p->need_clamp;
@@ -952,13 +986,15 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
         return cudaSuccess;
     };
     if (p->mma_paired) {
-        if (p->B == 1024) e = launch(k_signature_mma<16, true>);
-        else if (p->B == 512) e = launch(k_signature_mma<8, true>);
-        else e = launch(k_signature_mma<4, true>);
+        if (p->B == 2048) e = launch(k_signature_mma<16, 8, true>);
+        else if (p->B == 1024) e = launch(k_signature_mma<16, 4, true>);
+        else if (p->B == 512) e = launch(k_signature_mma<8, 4, true>);
+        else e = launch(k_signature_mma<4, 4, true>);
     } else {
-        if (p->B == 1024) e = launch(k_signature_mma<16, false>);
-        else if (p->B == 512) e = launch(k_signature_mma<8, false>);
-        else e = launch(k_signature_mma<4, false>);
+        if (p->B == 2048) e = launch(k_signature_mma<16, 8, false>);
+        else if (p->B == 1024) e = launch(k_signature_mma<16, 4, false>);
+        else if (p->B == 512) e = launch(k_signature_mma<8, 4, false>);
+        else e = launch(k_signature_mma<4, 4, false>);
     }
     if (e != cudaSuccess) return e;
     e = cudaGetLastError();

@@ -135,18 +135,19 @@ def test_run_host_matches_device_path():
     plan.apx_plan_destroy()
 
 
+@pytest.mark.parametrize("B", [1024, 2048])
 @pytest.mark.parametrize("centre_ions", [False, True], ids=["fixups", "overflow"])
 @pytest.mark.parametrize("flags", [pytest.param(0, id="half"), pytest.param(apx.APX_FLAG_NO_PAIRING, id="full")])
-def test_half_grid_mode_with_exact_integer_projections(flags, centre_ions):
+def test_half_grid_mode_with_exact_integer_projections(flags, centre_ions, B):
     """Half-grid mode on a symmetric grid: b(-n) = B-1-b(n) holds only while n'.d is not an integer
     (floor(-x) = -floor(x) - 1); for an exact integer b(-n) = B - b(n), and the kernel must redo -n on its own.
-    R = 511/256 makes s = 256 exactly, so ions on a 1/4 grid project to exact integers along the axis directions
+    R = (B/2-1)/(B/4) makes s = B/4 exactly, so ions on a 1/4 grid project to exact integers along the axis directions
     (+-x, +-y, +-z are vertices of the geodesic grid) and a random half of the cloud does not: using the mirrored
     histogram there would shift the grid ions against the rest by one bin and change the amplitudes.  With an ion
     exactly on each centre (x = +-0 for EVERY direction) the list of flagged pairs overflows and the material
     points are redone by the general kernel."""
     rng = np.random.Generator(np.random.PCG64(11))
-    R, B = 511.0 / 256.0, 1024
+    R = (B / 2 - 1) / (B / 4)
     c2 = np.array([0.25, 0.5, -0.25])
     g = np.arange(-10, 11) / 4.0
     grid = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
@@ -165,7 +166,7 @@ def test_half_grid_mode_with_exact_integer_projections(flags, centre_ions):
     plan = apx.Plan(R, B, dirs, k_lo=15, k_hi=34, device=0, flags=flags)
     assert plan.apx_plan_path() == 1 and plan.apx_plan_paired() == (0 if flags else 1)
     _, s, _ = plan.apx_plan_constants()
-    assert s == 256.0
+    assert s == B / 4
     plan.apx_plan_destroy()
     _check(w, dirs, centres, (15, 34), flags)
 
@@ -174,3 +175,22 @@ def test_half_grid_mode_is_off_for_asymmetric_grids():
     plan = apx.Plan(2.0, 1024, O.dirs_fibonacci(1000), k_lo=15, k_hi=34, device=0)
     assert plan.apx_plan_path() == 1 and plan.apx_plan_paired() == 0
     plan.apx_plan_destroy()
+
+
+@pytest.mark.parametrize("flags", [pytest.param(0, id="half"), pytest.param(apx.APX_FLAG_NO_PAIRING, id="full")])
+def test_b2048_tensor_path_multipass_and_deferred(flags):
+    """B = 2048 on the tensor-core kernel (16 direction slots per group, one histogram buffer): a ROI of ~2700 ions is
+    binned in two passes of <= 2048 ions, a ROI of more than 4096 ions is left to the general kernel, a partial ROI
+    and an empty one ride along; whole symmetric grid, so the half-grid mode and its fix-up groups run as well."""
+    xyz, types = _ball(3.4)
+    dirs = apx.apx_dirs_geodesic(3)
+    w = _case(xyz, types, 2.2, 2048)
+    centres = np.array([[0, 0, 0], [0.3, -0.2, 0.1], [3.0, 0, 0], [9.0, 9.0, 9.0]], np.float32)
+    plan = apx.Plan(2.2, 2048, dirs, k_lo=23, k_hi=51, device=0, flags=flags)
+    assert plan.apx_plan_path() == 1 and plan.apx_plan_paired() == (0 if flags else 1)
+    plan.apx_plan_destroy()
+    path, cnt = _check(w, dirs, centres, (23, 51), flags)
+    assert path == 1 and cnt[0] > 2048 and cnt[3] == 0
+    w = _case(xyz, types, 2.7, 2048)
+    path, cnt = _check(w, dirs, centres[:2], window_for(2.7, 2048), flags)
+    assert path == 1 and cnt.min() > 4096

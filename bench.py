@@ -35,10 +35,16 @@ FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 # issue-slot peak: 148 SMs x 4 schedulers x 32 lanes x 1.965 GHz thread-instructions/s
 ISSUE_PEAK_TINST = 148 * 4 * 32 * 1.965e9
 PAIR_FLOP = 6.0          # FMUL + 2 FFMA + round-down FADD of Eq. 1's projection and floor, per (ion, direction) pair
-PAIR_SLOTS_MMA = 8.0     # + FFMA.RD (hi3) + 2 IMAD (address) + 1 shared atomic: issue slots per pair, MMA kernel
+# issue slots per pair in the MMA kernel's binning loop: 100 instructions per 8 ions x 2 directions of a lane
+# (6 LDS.128, 20 packed FP32x2 for projection / floor / hi3, 32 IMAD, 16 ATOMS, loop control)
+PAIR_SLOTS_MMA = 6.25
+# shared-memory (LSU data pipe) ceiling: one wavefront per SM and clock
+LSU_PEAK_WAVEFRONTS = 148 * 1.965e9
 # traffic (dram__bytes_read.sum + dram__bytes_write.sum per launch) of the dominant kernel from the committed
 # ncu --set full capture (profiles/), config 2; None for a kernel/config that was not captured
 NCU_TRAFFIC = {"k_signature_mma": 25.6e6, "k_signature_fft": 28.4e6}
+# shared-memory wavefronts per launch (l1tex__data_pipe_lsu_wavefronts_mem_shared.sum) from the same captures
+NCU_LSU_WAVEFRONTS = {"k_signature_mma": 1.08e9}
 
 
 def algorithmic_flops(n_pairs, n_hist, B, path):
@@ -267,6 +273,10 @@ def run_ours(args, rank, world, local_rank):
                      "model": "6 flop per (ion,direction) pair" + ("" if path == "mma" else " + 2.5 B log2 B flop per histogram"),
                      "pairs_per_launch": pairs,
                      "issue_slot_frac": (PAIR_SLOTS_MMA * pairs / q_s / ISSUE_PEAK_TINST) if path == "mma" else None,
+                     # what actually bounds the binning: the shared-memory data pipe (atomics + ion loads), one
+                     # wavefront per SM and clock; wavefronts per launch from the committed ncu capture
+                     "lsu_wavefront_frac": (NCU_LSU_WAVEFRONTS[kname] / q_s / LSU_PEAK_WAVEFRONTS)
+                     if kname in NCU_LSU_WAVEFRONTS else None,
                      "tensor_tflops": tensor_flops / q_s / 1e12 if path == "mma" else None},
     }
     if not args.no_cpu_baseline:

@@ -488,7 +488,18 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                 const float *db = p.dirs_sorted + (eb < sq.nfix ? (size_t)(sq.g0 * G + (int)ps.fix[eb]) * 3 : 0);
                 n.ax = -da[0]; n.ay = -da[1]; n.az = -da[2]; n.bx = -db[0]; n.by = -db[1]; n.bz = -db[2];
             }
-            if (use >= 1) mbar_wait(&ps.free_[buf], (uint32_t)((use - 1) & 1));       // cleared after its previous use
+            if (kBig) {
+                // single-buffered: the shared-memory pipe is idle while the tensor core transforms the buffer, so the 16
+                // binning warps clear it themselves as soon as it has been read (a few STS.128 per thread)
+                if (use >= 1) {
+                    mbar_wait(&ps.done[0], (uint32_t)((use - 1) & 1));
+                    uint4 *hb = reinterpret_cast<uint4 *>(smem + L.hist0);
+                    for (int i = tid; i < (int)(L.hist_bytes / 16); i += kBinWarps * 32) hb[i] = make_uint4(0, 0, 0, 0);
+                    asm volatile("bar.sync 5, %0;" ::"n"(kBinWarps * 32) : "memory");
+                }
+            } else if (use >= 1) {
+                mbar_wait(&ps.free_[buf], (uint32_t)((use - 1) & 1));                  // cleared after its previous use
+            }
             const int a0 = pass * 2048, a1 = min(n_ions, a0 + 2048);
             const int nq = (a1 - a0 + 3) >> 2;                                       // quads of this pass, split evenly
             const int i0 = a0 + 4 * ((warp * nq) / kBinWarps), i1 = min(a1, a0 + 4 * (((warp + 1) * nq) / kBinWarps));
@@ -547,7 +558,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
     } else if (warp == kClrWarp) {
         // ---- clear warp: once the tensor core has read a buffer, clear it with bulk copies of zeros (TMA engine, no
         //      LSU work); free(buf) completes when all bytes have landed
-        for (int it = 0; it < nitems; ++it) {
+        for (int it = 0; it < (kBig ? 0 : nitems); ++it) {           // (single-buffered: the binning warps clear)
             const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
             mbar_wait<100>(&ps.done[buf], (uint32_t)(use & 1));
             if (n < kStsClearBelow) {
@@ -695,7 +706,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
         if (warp == kClrWarp && grp_total > 0) {
             const int npass = n > 2048 ? (n + 2047) / 2048 : 1, items = grp_total * npass;
             if (NB == 8 || n > p.cap) {
-                mbar_wait(&s_free[0], (uint32_t)((items - 1) & 1));
+                // single-buffered: cleared with plain stores by the binning warps, nothing in flight
             } else {
                 const int u0 = (items + 1) >> 1, u1 = items >> 1;
                 if (u0) mbar_wait(&s_free[0], (uint32_t)((u0 - 1) & 1));

@@ -42,9 +42,9 @@ PAIR_SLOTS_MMA = 6.25
 LSU_PEAK_WAVEFRONTS = 148 * 1.965e9
 # traffic (dram__bytes_read.sum + dram__bytes_write.sum per launch) of the dominant kernel from the committed
 # ncu --set full capture (profiles/), config 2; None for a kernel/config that was not captured
-NCU_TRAFFIC = {"k_signature_mma": 25.6e6, "k_signature_fft": 28.4e6}
+NCU_TRAFFIC = {"k_signature_mma": 180.4e6, "k_signature_fft": 29.7e6}
 # shared-memory wavefronts per launch (l1tex__data_pipe_lsu_wavefronts_mem_shared.sum) from the same captures
-NCU_LSU_WAVEFRONTS = {"k_signature_mma": 1.08e9}
+NCU_LSU_WAVEFRONTS = {"k_signature_mma": 1.0856e9, "k_signature_fft": 3.619e9}
 
 
 def algorithmic_flops(n_pairs, n_hist, B, path):

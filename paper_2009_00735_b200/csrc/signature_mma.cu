@@ -1,12 +1,14 @@
 // signature_mma.cu -- windowed-DFT signature kernel: shared-memory histograms feed the tcgen05 tensor
-// cores directly (steps a2, a4-a7 for narrow spectral windows, B <= 1024).
+// cores directly (steps a2, a4-a7 for narrow spectral windows, B <= 2048).
 //
-// Per CTA: one material point x a chunk of direction groups; a group = 32 directions.
+// Per CTA: one material point x a chunk of direction groups; a group = G direction slots (32 for B <= 1024, 16 for
+// B = 2048; struct Lay).  Described for B = 1024:
 //   binning  : lane l (0..15) of a half-warp owns ONE 32-bit word per histogram row: two u16 counters, the
 //              low half for direction l (set A) and the high half for direction l + 16 (set B) of the group
-//              (Eq. 1).  The two half-warps of a warp work on different ions.  The u16 bit
-//              pattern c is the fp16 number c * 2^-24 (subnormal / first binade, exact for c <= 2048), so the
-//              histogram IS a valid fp16 tensor-core operand and is never converted or copied.
+//              (Eq. 1).  The two half-warps of a warp work on different ions, every lane bins its
+//              ions for both of its directions.  The u16 bit pattern c is the fp16 number c * 2^-24 (subnormal /
+//              first binade, exact for c <= 2048), so the histogram IS a valid fp16 tensor-core operand and is never
+//              converted or copied.
 //   layout   : byte address of (bin b, lane l) = (l/4)*160 + (l%4)*4 + 16*hi3 + 640*low,
 //              hi3 = b >> (log2 B - 3), low = b & (B/8 - 1).  Bank = 8*(l/4) + 4*hi3 + l%4 (mod 32): the 16 lanes
 //              of a half-warp hit 16 different banks whenever their bins agree in the top three bits (hi3) -- the
@@ -24,7 +26,10 @@
 // Two histogram buffers and two TMEM accumulators: while the 16 binning warps fill buffer (g+1)&1, the tensor
 // core transforms buffer g&1, a TMA bulk copy clears it and one of two sets of four service warps runs the epilogue
 // of group g.  A ROI with more ions than the ion buffer spills into the second histogram buffer and runs
-// single-buffered; only ROIs beyond that are appended to a deferred list for the general FFT kernel.
+// single-buffered (so does every ROI at B = 2048, where only one buffer fits); only ROIs beyond that are appended to
+// a deferred list for the general FFT kernel.
+// Half-grid mode (antipodally symmetric direction grids, L60): one member of every pair (n, -n) is binned and its peak
+// serves both; see the comment above struct Detect.
 #include <algorithm>
 #include <array>
 #include <cstring>

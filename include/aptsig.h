@@ -115,6 +115,11 @@ int apx_dirs_fibonacci(int32_t D, float *out /* D x 3 */);
 /* Geodesic sphere: icosahedron subdivided `level` times (level 6 = the paper's 40 962 nodes, L60).
  * out may be NULL to query *D_out = 10*4^level + 2 only; level 0..8. */
 int apx_dirs_geodesic(int32_t level, float *out, int32_t *D_out);
+/* Antipodal partners of a direction grid (HOST, no GPU): partner[i] = j with dirs[j] == -dirs[i] component by
+ * component (+0 and -0 are the same), or -1.  Returns 1 if every direction has a partner other than itself and no
+ * direction occurs twice (the grid is antipodally symmetric: the tensor-core kernel's half-grid mode applies to it,
+ * see apx_plan_paired), 0 if not, APX_EINVAL for bad arguments.  `partner` (D ints) may be NULL. */
+int apx_dirs_antipodes(const float *dirs /* D x 3 */, int32_t D, int32_t *partner);
 
 const char *apx_strerror(int status);
 const char *apx_version(void);

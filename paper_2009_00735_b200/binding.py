@@ -17,7 +17,7 @@ APX_FLAG_FORCE_FFT, APX_FLAG_FORCE_MMA, APX_FLAG_NO_PAIRING = 1, 2, 4
 
 EXPORTS = ["apx_plan_create", "apx_plan_destroy", "apx_plan_constants", "apx_plan_path", "apx_plan_paired", "apx_last_cuda_error",
            "apx_ingest", "apx_query", "apx_run", "apx_run_host", "apx_debug_histograms",
-           "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_strerror", "apx_version"]
+           "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_dirs_antipodes", "apx_strerror", "apx_version"]
 
 
 class apx_plan_desc(C.Structure):
@@ -59,6 +59,7 @@ def _lib():
         L.apx_debug_histograms.argtypes = [vp, C.POINTER(C.c_float), i32, i32, vp, vp]
         L.apx_dirs_fibonacci.argtypes = [i32, vp]
         L.apx_dirs_geodesic.argtypes = [i32, vp, C.POINTER(i32)]
+        L.apx_dirs_antipodes.argtypes = [vp, i32, vp]
         L.apx_strerror.argtypes = [C.c_int]
         L.apx_strerror.restype = C.c_char_p
         L.apx_version.restype = C.c_char_p
@@ -101,6 +102,16 @@ def apx_dirs_geodesic(level: int) -> np.ndarray:
     if rc:
         raise ApxError(rc, "apx_dirs_geodesic")
     return out
+
+
+def apx_dirs_antipodes(dirs: np.ndarray):
+    """(symmetric, partner): partner[i] = index of the direction -dirs[i], or -1 (host only)."""
+    d = np.ascontiguousarray(dirs, np.float32)
+    partner = np.empty(len(d), np.int32)
+    rc = _lib().apx_dirs_antipodes(d.ctypes.data, len(d), partner.ctypes.data)
+    if rc < 0:
+        raise ApxError(rc, "apx_dirs_antipodes")
+    return bool(rc), partner
 
 
 def _ptr(t, dtype=None):

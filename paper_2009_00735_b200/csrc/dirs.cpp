@@ -2,7 +2,10 @@
 // Fibonacci sphere: BASELINE.json configs 1-2 (not in the paper).  Geodesic sphere: the paper's
 // "geodesic sphere finite element mesh" with N_v = 40 962 nodes = level 6.
 #include <cmath>
+#include <array>
 #include <cstdint>
+#include <cstring>
+#include <map>
 #include <unordered_map>
 #include <vector>
 #include "../../include/aptsig.h"
@@ -76,4 +79,29 @@ extern "C" int apx_dirs_geodesic(int32_t level, float *out, int32_t *D_out)
         out[3 * i + 2] = (float)v[i].z;
     }
     return APX_OK;
+}
+
+extern "C" int apx_dirs_antipodes(const float *dirs, int32_t D, int32_t *partner)
+{
+    if (!dirs || D < 1) return APX_EINVAL;
+    auto key = [&](int32_t i, float sgn) {
+        std::array<uint32_t, 3> k;
+        for (int a = 0; a < 3; ++a) {
+            float v = sgn * dirs[3 * (size_t)i + a];
+            if (v == 0.0f) v = 0.0f;                             // -0 and +0 are the same component
+            std::memcpy(&k[a], &v, 4);
+        }
+        return k;
+    };
+    std::map<std::array<uint32_t, 3>, int32_t> index;
+    bool sym = true;
+    for (int32_t i = 0; i < D; ++i)
+        if (!index.emplace(key(i, 1.0f), i).second) sym = false;  // duplicate direction
+    for (int32_t i = 0; i < D; ++i) {
+        auto it = index.find(key(i, -1.0f));
+        const int32_t j = (it == index.end() || it->second == i) ? -1 : it->second;
+        if (j < 0) sym = false;
+        if (partner) partner[i] = j;
+    }
+    return sym ? 1 : 0;
 }

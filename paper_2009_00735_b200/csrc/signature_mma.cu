@@ -871,25 +871,7 @@ cudaError_t mma_path_prepare(Plan *p)
     const int D = p->D;
     std::vector<int> partner((size_t)D, -1);
     bool sym = !p->need_clamp && !(p->desc.flags & APX_FLAG_NO_PAIRING) && D >= 2 && D % 2 == 0;
-    if (sym) {
-        auto key = [&](int i, float sgn) {
-            std::array<uint32_t, 3> k;
-            for (int a = 0; a < 3; ++a) {
-                float v = sgn * nps[3 * (size_t)i + a];
-                if (v == 0.0f) v = 0.0f;                         // -0 and +0 are the same direction component
-                std::memcpy(&k[a], &v, 4);
-            }
-            return k;
-        };
-        std::map<std::array<uint32_t, 3>, int> index;
-        for (int i = 0; i < D && sym; ++i)
-            if (!index.emplace(key(i, 1.0f), i).second) sym = false;      // duplicate direction
-        for (int i = 0; i < D && sym; ++i) {
-            auto it = index.find(key(i, -1.0f));
-            if (it == index.end() || it->second == i) sym = false;
-            else partner[i] = it->second;
-        }
-    }
+    if (sym) sym = apx_dirs_antipodes(nps.data(), D, partner.data()) == 1;   // scaling by s keeps n' = -(-n)'
     std::vector<int> perm, mirror;
     std::vector<float> sorted;
     if (sym) {

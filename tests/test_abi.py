@@ -61,3 +61,23 @@ def test_plan_create_rejects_bad_arguments_before_touching_cuda():
         with pytest.raises(apx.ApxError) as ei:
             apx.Plan(dirs=d, **kw)
         assert ei.value.status == apx.APX_EINVAL
+
+
+def test_antipodal_partners_of_direction_grids():
+    """The geodesic grid (the paper's mesh, L60) is antipodally symmetric bit for bit -- what the half-grid mode of the
+    tensor-core kernel relies on; a Fibonacci grid is not; duplicates and self-partners are rejected."""
+    for level in (0, 1, 3):
+        d = apx.apx_dirs_geodesic(level)
+        sym, partner = apx.apx_dirs_antipodes(d)
+        assert sym and (partner >= 0).all() and (partner[partner] == np.arange(len(d))).all()
+        assert (d[partner] == -d).all()                       # numerically: -0.0 == +0.0
+    sym, partner = apx.apx_dirs_antipodes(O.dirs_fibonacci(1000))
+    assert not sym and (partner == -1).all()
+    d = apx.apx_dirs_geodesic(1)
+    sym, _ = apx.apx_dirs_antipodes(np.concatenate([d, d[:1]]))          # a duplicate
+    assert not sym
+    sym, partner = apx.apx_dirs_antipodes(np.array([[0, 0, 0], [1, 0, 0], [-1, 0, 0]], np.float32))
+    assert not sym and partner[0] == -1 and partner[1] == 2 and partner[2] == 1
+    # scaling by the plan's s (one fp32 multiply per component) keeps the pairs exact
+    sym, _ = apx.apx_dirs_antipodes((apx.apx_dirs_geodesic(4) * np.float32(255.5)).astype(np.float32))
+    assert sym

@@ -148,6 +148,49 @@ def run_reference(args, rank, world):
     }))
 
 
+def run_ingest(args):
+    """--ingest-ions N: step a1 alone (HBM-bound counting sort) on N uniform random ions in config 4's 60^3 nm box;
+    not the default bench line -- the roofline evidence for the ingest kernels."""
+    import torch
+    import paper_2009_00735_b200 as apx
+    dev = torch.device("cuda:0")
+    N = args.ingest_ions
+    rng = np.random.Generator(np.random.PCG64(200900735))
+    xyz_np = (rng.random((N, 3), dtype=np.float32) * np.float32(60.0))
+    types_np = np.zeros(N, np.uint8)
+    plan = apx.Plan(2.0, 1024, apx.apx_dirs_fibonacci(64), k_lo=15, k_hi=34, device=0)
+    xyz, types = torch.from_numpy(xyz_np).to(dev), torch.from_numpy(types_np).to(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    for _ in range(max(args.warmup, 3)):
+        plan.apx_ingest(xyz, types)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in ev:
+        flush.fill_(1)
+        a.record(); plan.apx_ingest(xyz, types); b.record()
+    torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in ev) / args.steps
+    # algorithmic bytes per ion: xyz + type read by k_bounds and k_count (2 x 13), cell id written and read (2 x 4),
+    # xyz read again and the 16-byte record written by k_scatter (12 + 16)
+    bytes_per_ion = 2 * 13 + 2 * 4 + 12 + 16
+    try:
+        peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        src = "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        peak, src = 6550.0, "fallback (B200_PROFILING.md)"
+    achieved = bytes_per_ion * N / (ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "ingested ions/s", "value": N / (ms * 1e-3), "unit": "ions/s", "n_gpus": 1,
+                      "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+                      "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": f"ingest only: {N} uniform random ions in a 60^3 nm box, R = 2.0 (cell edge 1 nm)",
+                                 "l2": "flushed between timed steps (256 MiB fill, untimed)"},
+                      "gpu_launches": 8 * args.steps,
+                      "roofline": {"bound": "hbm", "kernel": "ingest (8 kernels)", "achieved": achieved, "peak": peak,
+                                   "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": src,
+                                   "model": f"{bytes_per_ion} B per ion"}}))
+    plan.apx_plan_destroy()
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import paper_2009_00735_b200 as apx
@@ -261,9 +304,9 @@ def run_ours(args, rank, world, local_rank):
         "clocks": clocks,
         "e2e": {"value": n_hist * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "entry": "apx_run_host", "steps": e2e_steps},
-        # 7 ingest kernels (k_reset, k_bounds, k_grid_params, k_zero_cells, k_count, k_scan, k_scatter)
+        # 8 ingest kernels (k_reset, k_bounds, k_grid_params, k_zero_cells, k_count, k_scan_local, k_scan_add, k_scatter)
         # + k_signature_mma + k_signature_fft over the deferred list (or k_signature_fft alone) per step
-        "gpu_launches": (9 if path == "mma" else 8) * args.steps,
+        "gpu_launches": (10 if path == "mma" else 9) * args.steps,
         "roofline": {"bound": "alu", "kernel": kname,
                      "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                      "frac": achieved / FP32_PEAK_TFLOPS, "traffic": NCU_TRAFFIC.get(kname),
@@ -301,11 +344,15 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--path", default="auto", choices=["auto", "fft"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ingest-ions", type=int, default=0, help="time step a1 (ingest) alone on this many ions")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.ingest_ions > 0:
+        if rank == 0:
+            run_ingest(args)
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
         run_ours(args, rank, world, local_rank)

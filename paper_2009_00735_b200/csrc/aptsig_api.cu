@@ -49,7 +49,7 @@ extern "C" int apx_plan_destroy(apx_plan *p)
     if (!p) return APX_OK;
     cudaSetDevice(p->device);
     void *bufs[] = {p->d_dirs_scaled, p->d_twiddle, p->d_mma_table, p->d_mma_zero, p->d_mma_phase, p->d_dirs_sorted, p->d_dir_perm, p->d_dir_perm_mirror, p->d_type_mask, p->d_grid, p->d_cell_start,
-                    p->d_cell_cursor, p->d_cell_of_ion, p->d_sorted, p->d_deferred, p->h2d_xyz, p->h2d_types, p->h2d_centres,
+                    p->d_cell_cursor, p->d_scan_tiles, p->d_cell_of_ion, p->d_sorted, p->d_deferred, p->h2d_xyz, p->h2d_types, p->h2d_centres,
                     p->d2h_sig, p->d2h_counts};
     for (void *b : bufs)
         if (b) cudaFree(b);
@@ -113,6 +113,7 @@ extern "C" int apx_plan_create(const apx_plan_desc *desc, apx_plan **out)
     CUF(cudaMalloc(&p->d_grid, sizeof(GridParams)));
     CUF(cudaMalloc(&p->d_cell_start, (size_t)(kMaxCells + 1) * sizeof(uint32_t)));
     CUF(cudaMalloc(&p->d_cell_cursor, (size_t)kMaxCells * sizeof(uint32_t)));
+    CUF(cudaMalloc(&p->d_scan_tiles, (size_t)(kMaxCells / 8192) * sizeof(uint32_t)));
     CUF(cudaMemcpy(p->d_dirs_scaled, nps.data(), nps.size() * sizeof(float), cudaMemcpyHostToDevice));
     CUF(cudaMemcpy(p->d_twiddle, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice));
     CUF(cudaMemcpy(p->d_type_mask, mask, 32, cudaMemcpyHostToDevice));

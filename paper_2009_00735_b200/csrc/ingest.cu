@@ -54,10 +54,25 @@ __global__ void __launch_bounds__(256) k_bounds(const float *__restrict__ xyz, c
         }
         cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
     }
+    // block-level reduction in shared memory, then one set of global atomics per block
+    __shared__ int s_mn[3], s_mx[3];
+    __shared__ unsigned s_cnt;
+    if (threadIdx.x == 0) {
+        s_mn[0] = s_mn[1] = s_mn[2] = 0x7FFFFFFF;
+        s_mx[0] = s_mx[1] = s_mx[2] = (int)0x80000000;
+        s_cnt = 0;
+    }
+    __syncthreads();
     if ((threadIdx.x & 31) == 0 && cnt) {
-        atomicMin(&g->minx, mn[0]); atomicMin(&g->miny, mn[1]); atomicMin(&g->minz, mn[2]);
-        atomicMax(&g->maxx, mx[0]); atomicMax(&g->maxy, mx[1]); atomicMax(&g->maxz, mx[2]);
-        atomicAdd(&g->n_accepted, cnt);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { atomicMin(&s_mn[a], mn[a]); atomicMax(&s_mx[a], mx[a]); }
+        atomicAdd(&s_cnt, cnt);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && s_cnt) {
+        atomicMin(&g->minx, s_mn[0]); atomicMin(&g->miny, s_mn[1]); atomicMin(&g->minz, s_mn[2]);
+        atomicMax(&g->maxx, s_mx[0]); atomicMax(&g->maxy, s_mx[1]); atomicMax(&g->maxz, s_mx[2]);
+        atomicAdd(&g->n_accepted, s_cnt);
     }
 }
 
@@ -113,43 +128,81 @@ __global__ void __launch_bounds__(256) k_count(const float *__restrict__ xyz, co
     }
 }
 
-// exclusive scan of cell_count[0..ncells) in place, total at [ncells]; one 1024-thread block walks chunks.
-__global__ void __launch_bounds__(1024) k_scan(uint32_t *cell, uint32_t *cursor, const GridParams *g)
+// Exclusive scan of cell_count[0..ncells) in place, total at [ncells], in two fully parallel launches over tiles of 8192
+// cells (8 consecutive cells per thread; the grid has at most 2^21 cells = 256 tiles):
+//   k_scan_local: exclusive scan inside every tile, tile totals to tile_sum
+//   k_scan_add  : every tile adds the sum of the totals of the tiles before it (<= 255 values, one block reduce)
+constexpr int kScanItems = 8, kScanTile = 1024 * kScanItems;
+__device__ __forceinline__ uint32_t block_exclusive(uint32_t tot, uint32_t *warp_sum, uint32_t *block_total)
 {
-    __shared__ uint32_t warp_sum[32];
-    __shared__ uint32_t carry;
-    const int n = g->ncells;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry = 0;
+    uint32_t inc = tot;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) warp_sum[wid] = inc;
     __syncthreads();
-    for (int base = 0; base < n; base += 1024) {
-        int i = base + threadIdx.x;
-        uint32_t v = i < n ? cell[i] : 0u;
-        uint32_t inc = v;
+    if (wid == 0) {
+        uint32_t w = warp_sum[lane], wi = w;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
+            uint32_t t = __shfl_up_sync(0xffffffffu, wi, o);
+            if (lane >= o) wi += t;
         }
-        if (lane == 31) warp_sum[wid] = inc;
-        __syncthreads();
-        if (wid == 0) {
-            uint32_t w = warp_sum[lane], wi = w;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                uint32_t t = __shfl_up_sync(0xffffffffu, wi, o);
-                if (lane >= o) wi += t;
-            }
-            warp_sum[lane] = wi - w;   // exclusive
-        }
-        __syncthreads();
-        uint32_t excl = carry + warp_sum[wid] + inc - v;
-        if (i < n) { cell[i] = excl; cursor[i] = excl; }
-        __syncthreads();
-        if (threadIdx.x == 1023) carry = excl + v;
-        __syncthreads();
+        warp_sum[lane] = wi - w;   // exclusive
+        if (lane == 31) *block_total = wi;
     }
-    if (threadIdx.x == 0) cell[n] = carry;
+    __syncthreads();
+    return warp_sum[wid] + inc - tot;
+}
+__global__ void __launch_bounds__(1024) k_scan_local(uint32_t *cell, uint32_t *tile_sum, const GridParams *g)
+{
+    __shared__ uint32_t warp_sum[32], total;
+    const int n = g->ncells, i0 = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
+    if (blockIdx.x * kScanTile >= n) return;
+    uint32_t v[kScanItems];
+    const bool full = i0 + kScanItems <= n;                      // cell_start is 16-byte aligned and i0 a multiple of 8
+    if (full) {
+        const uint4 a = *reinterpret_cast<const uint4 *>(cell + i0), b4 = *reinterpret_cast<const uint4 *>(cell + i0 + 4);
+        v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b4.x; v[5] = b4.y; v[6] = b4.z; v[7] = b4.w;
+    } else {
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k) v[k] = i0 + k < n ? cell[i0 + k] : 0u;
+    }
+    uint32_t tot = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) { const uint32_t t = v[k]; v[k] = tot; tot += t; }   // exclusive within the thread
+    const uint32_t excl = block_exclusive(tot, warp_sum, &total);
+    if (full) {
+        *reinterpret_cast<uint4 *>(cell + i0) = make_uint4(excl + v[0], excl + v[1], excl + v[2], excl + v[3]);
+        *reinterpret_cast<uint4 *>(cell + i0 + 4) = make_uint4(excl + v[4], excl + v[5], excl + v[6], excl + v[7]);
+    } else {
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k)
+            if (i0 + k < n) cell[i0 + k] = excl + v[k];
+    }
+    if (threadIdx.x == 0) tile_sum[blockIdx.x] = total;
+}
+__global__ void __launch_bounds__(1024) k_scan_add(uint32_t *cell, uint32_t *cursor, const uint32_t *tile_sum, const GridParams *g)
+{
+    __shared__ uint32_t warp_sum[32], before;
+    const int n = g->ncells, tile = blockIdx.x, i0 = tile * kScanTile + threadIdx.x * kScanItems;
+    if (tile * kScanTile >= n) return;
+    block_exclusive((int)threadIdx.x < tile ? tile_sum[threadIdx.x] : 0u, warp_sum, &before);   // sum of the earlier tiles
+    const uint32_t off = before;
+    if (i0 + kScanItems <= n) {
+        uint4 a = *reinterpret_cast<const uint4 *>(cell + i0), b4 = *reinterpret_cast<const uint4 *>(cell + i0 + 4);
+        a.x += off; a.y += off; a.z += off; a.w += off; b4.x += off; b4.y += off; b4.z += off; b4.w += off;
+        *reinterpret_cast<uint4 *>(cell + i0) = a; *reinterpret_cast<uint4 *>(cell + i0 + 4) = b4;
+        *reinterpret_cast<uint4 *>(cursor + i0) = a; *reinterpret_cast<uint4 *>(cursor + i0 + 4) = b4;
+    } else {
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k)
+            if (i0 + k < n) { const uint32_t val = cell[i0 + k] + off; cell[i0 + k] = val; cursor[i0 + k] = val; }
+    }
+    if (threadIdx.x == 0 && (tile + 1) * kScanTile >= n) cell[n] = off + tile_sum[tile];   // the last tile: grand total
 }
 
 __global__ void __launch_bounds__(256) k_scatter(const float *__restrict__ xyz, int64_t N,
@@ -173,7 +226,8 @@ cudaError_t launch_ingest(Plan *p, const float *xyz, const uint8_t *types, int64
     k_zero_cells<<<blocks, 256, 0, st>>>(p->d_cell_start, p->d_grid);
     if (N > 0)
         k_count<<<blocks, 256, 0, st>>>(xyz, types, N, p->d_type_mask, p->d_grid, p->d_cell_start, p->d_cell_of_ion);
-    k_scan<<<1, 1024, 0, st>>>(p->d_cell_start, p->d_cell_cursor, p->d_grid);
+    k_scan_local<<<kMaxCells / kScanTile, 1024, 0, st>>>(p->d_cell_start, p->d_scan_tiles, p->d_grid);
+    k_scan_add<<<kMaxCells / kScanTile, 1024, 0, st>>>(p->d_cell_start, p->d_cell_cursor, p->d_scan_tiles, p->d_grid);
     if (N > 0) k_scatter<<<blocks, 256, 0, st>>>(xyz, N, p->d_cell_of_ion, p->d_cell_cursor, p->d_sorted);
     return cudaGetLastError();
 }

@@ -101,14 +101,15 @@ def test_every_bin_count(flags, B):
         _check(w, dirs[:40], centres, None, flags)                 # full window [1, B/2]
 
 
+@pytest.mark.parametrize("B", [512, 2048])
 @pytest.mark.parametrize("flags", PATHS)
-def test_pad0_and_non_unit_directions_clamp(flags):
+def test_pad0_and_non_unit_directions_clamp(flags, B):
     """pad = 0 (north_star's [-R, R]) puts ions on the last bin edge, and directions 3 % longer than unit push
     projections past +-R: the bin clamp of Eq. 1 (reading #5) must act on both paths."""
     xyz, types = _ball(1.6, eta=0.7, sigma=0.03, seed=13)
     dirs = (O.dirs_fibonacci(64).astype(np.float64) * 1.03).astype(np.float32)
     centres = np.array([[0, 0, 0]], np.float32)
-    w = _case(xyz, types, 1.2, 512)
+    w = _case(xyz, types, 1.2, B)
     _check(w, dirs, centres, (5, 20), flags, pad=0)
     _check(w, dirs, centres, (5, 20), flags, pad=1)
 

@@ -27,6 +27,14 @@ METRIC = "direction-histograms/s"
 UNIT = "histograms/s"
 WORKLOAD = ("cfg2_single_crystal: fcc Al 20^3 nm (~241k ions), 1000 material points x 10000 Fibonacci directions, "
             "R=2.0 nm, B=1024, window [15,34]")
+OTHER_WORKLOADS = {
+    3: "cfg3_bicrystal: 30^3 nm fcc Al | bcc W (~832k ions), 27000 material points x 40962 geodesic directions, R=2.0 nm, "
+       "B=1024, window [15,34], Al filter run",
+    4: "cfg4_nanocrystal: 64 Voronoi grains in 60^3 nm fcc Al (~4.8M ions), 175616 material points x 40962 geodesic "
+       "directions, R=2.0 nm, B=1024, window [15,34]",
+    5: "cfg5_dilute_alloy: 40^3 nm fcc Al-3%Sc + 5% background (~1.5M ions), 64000 material points x 40962 geodesic "
+       "directions, R=3.0 nm, B=2048, window [23,51], Al filter",
+}
 # nominal FP32 peak used as the "alu" roofline denominator (B200_PROFILING.md: 148 SMs, 1965 MHz max SM clock;
 # 128 FP32 lanes per SM, FFMA = 2 flop): derived in DESIGN.md "Roofline".
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
@@ -204,13 +212,16 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.set_device(local_rank)
     dev = torch.device(f"cuda:{local_rank}")
 
-    w = make_config(2)
-    dirs = apx.apx_dirs_fibonacci(w.D)                      # step a3 through the library
+    w = make_config(args.config)
+    # step a3 through the library
+    dirs = apx.apx_dirs_geodesic(w.grid[1]) if w.grid[0] == "geodesic" else apx.apx_dirs_fibonacci(w.D)
+    accepted = {0} if args.config in (3, 5) else None       # configs 3 and 5: the Al filter run
+    workload = WORKLOAD if args.config == 2 else OTHER_WORKLOADS[args.config]
     # weak scaling: every rank processes the full config-2 centre list of its own replica shard
     # (material points are independent); ions are replicated, no collective on the data path.
     centres_np = w.centres
-    M, D, B = len(centres_np), w.D, w.B
-    plan = apx.Plan(w.R, B, dirs, k_lo=w.window[0], k_hi=w.window[1], device=local_rank,
+    M, D, B = len(centres_np), len(dirs), w.B
+    plan = apx.Plan(w.R, B, dirs, k_lo=w.window[0], k_hi=w.window[1], accepted_types=accepted, device=local_rank,
                     flags=apx.APX_FLAG_FORCE_FFT if args.path == "fft" else 0)
     xyz = torch.from_numpy(w.xyz).to(dev)
     types = torch.from_numpy(w.types).to(dev)
@@ -254,21 +265,24 @@ def run_ours(args, rank, world, local_rank):
     ms_query = sum(a.elapsed_time(b) for a, b in qev)
     n_c = counts.cpu().numpy().astype(np.int64)
 
-    # end to end through the host-pointer entry (pinned buffers; H2D + D2H inside the timed region)
-    h_xyz = torch.from_numpy(w.xyz).pin_memory()
-    h_types = torch.from_numpy(w.types).pin_memory()
-    h_centres = torch.from_numpy(centres_np).pin_memory()
-    h_sig = torch.empty((M, D, 2), dtype=torch.float32).pin_memory()
-    h_counts = torch.empty(M, dtype=torch.int32).pin_memory()
-    e2e_steps = max(1, min(args.steps, 5))
-    plan.apx_run_host(h_xyz, h_types, h_centres, h_sig, h_counts)
-    barrier()
-    te = time.perf_counter()
-    for _ in range(e2e_steps):
+    # end to end through the host-pointer entry (pinned buffers; H2D + D2H inside the timed region); the headline config
+    # only: configs 3-5 would pin up to 57 GB of host memory for their signatures
+    e2e_s, e2e_steps = 0.0, 0
+    if args.config == 2:
+        h_xyz = torch.from_numpy(w.xyz).pin_memory()
+        h_types = torch.from_numpy(w.types).pin_memory()
+        h_centres = torch.from_numpy(centres_np).pin_memory()
+        h_sig = torch.empty((M, D, 2), dtype=torch.float32).pin_memory()
+        h_counts = torch.empty(M, dtype=torch.int32).pin_memory()
+        e2e_steps = max(1, min(args.steps, 5))
         plan.apx_run_host(h_xyz, h_types, h_centres, h_sig, h_counts)
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - te
-    assert torch.equal(h_sig, sig.cpu()), "host-path result differs from device-path result"
+        barrier()
+        te = time.perf_counter()
+        for _ in range(e2e_steps):
+            plan.apx_run_host(h_xyz, h_types, h_centres, h_sig, h_counts)
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - te
+        assert torch.equal(h_sig, sig.cpu()), "host-path result differs from device-path result"
 
     tt = torch.tensor([ms, ms_query, e2e_s], dtype=torch.float64, device=dev)
     if dist is not None:
@@ -288,7 +302,11 @@ def run_ours(args, rank, world, local_rank):
     q_s = ms_query * 1e-3 / args.steps
     achieved = flops / q_s / 1e12
     W = w.window[1] - w.window[0] + 1
-    tensor_flops = 2.0 * 64 * ((4 * W + 15) // 16 * 16) * B * ((D + 63) // 64) * M if path == "mma" else 0.0
+    # executed MMA flops: 2 * 128 * N * K per direction group (N = 4W rounded up to 16, K = B / bin parts, G slots per group;
+    # half-grid mode bins one direction per antipodal pair)
+    nb, n_slots = (4 if B <= 1024 else 8), (D // 2 if plan.apx_plan_paired() else D)
+    groups = -(-n_slots // (128 // nb))
+    tensor_flops = 2.0 * 128 * ((4 * W + 15) // 16 * 16) * (B // nb) * groups * M if path == "mma" else 0.0
     h2d = w.xyz.nbytes + w.types.nbytes + centres_np.nbytes
     d2h = M * D * 8 + M * 4
     out = {
@@ -296,20 +314,21 @@ def run_ours(args, rank, world, local_rank):
         "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "material_points_per_s": value / D,
-        "config": {"workload": WORKLOAD,
+        "config": {"workload": workload,
                    "kernel_path": "mma" if plan.apx_plan_path() == 1 else "fft",
+                   "half_grid_mode": bool(plan.apx_plan_paired()),
                    "l2": "flushed between timed steps (256 MiB fill, untimed)",
                    "ions": int(len(w.xyz)), "mean_ions_per_roi": float(n_c.mean()),
                    "multi_gpu": "material points sharded per rank, ions replicated, no collective"},
         "clocks": clocks,
-        "e2e": {"value": n_hist * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-                "d2h_bytes_per_step": int(d2h), "entry": "apx_run_host", "steps": e2e_steps},
+        "e2e": ({"value": n_hist * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                 "d2h_bytes_per_step": int(d2h), "entry": "apx_run_host", "steps": e2e_steps} if e2e_steps else None),
         # 8 ingest kernels (k_reset, k_bounds, k_grid_params, k_zero_cells, k_count, k_scan_local, k_scan_add, k_scatter)
         # + k_signature_mma + k_signature_fft over the deferred list (or k_signature_fft alone) per step
         "gpu_launches": (10 if path == "mma" else 9) * args.steps,
         "roofline": {"bound": "alu", "kernel": kname,
                      "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                     "frac": achieved / FP32_PEAK_TFLOPS, "traffic": NCU_TRAFFIC.get(kname),
+                     "frac": achieved / FP32_PEAK_TFLOPS, "traffic": NCU_TRAFFIC.get(kname) if args.config == 2 else None,
                      "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md); "
                                     "MEASURED_PEAKS.json has no FP32 figure",
                      "ms_per_launch": ms_query / args.steps,
@@ -319,10 +338,10 @@ def run_ours(args, rank, world, local_rank):
                      # what actually bounds the binning: the shared-memory data pipe (atomics + ion loads), one
                      # wavefront per SM and clock; wavefronts per launch from the committed ncu capture
                      "lsu_wavefront_frac": (NCU_LSU_WAVEFRONTS[kname] / q_s / LSU_PEAK_WAVEFRONTS)
-                     if kname in NCU_LSU_WAVEFRONTS else None,
+                     if kname in NCU_LSU_WAVEFRONTS and args.config == 2 else None,
                      "tensor_tflops": tensor_flops / q_s / 1e12 if path == "mma" else None},
     }
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and args.config == 2:
         # bounded sample: batches of 64 material points until >= 10 s of CPU work
         dt, nh, cores, npts = 0.0, 0, 1, 0
         while dt < 10.0 and npts < M:
@@ -344,6 +363,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--path", default="auto", choices=["auto", "fft"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5],
+                    help="BASELINE.json config to time at full size (default 2 = the bench line; 3-5: device-timed only)")
     ap.add_argument("--ingest-ions", type=int, default=0, help="time step a1 (ingest) alone on this many ions")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

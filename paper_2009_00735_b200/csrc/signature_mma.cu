@@ -93,6 +93,21 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         }
     } while (!done);
 }
+// The same wait without the trap guard, for the two waits that poll most (binning warps on `free`, service warps on
+// `epi`): three instructions fewer per attempt.  A lost arrival would still be caught by the guarded waits of the MMA and
+// clear warps that feed these barriers.
+template <unsigned kSleepNs = 64>
+__device__ __forceinline__ void mbar_wait_lean(uint64_t *bar, uint32_t parity)
+{
+    asm volatile("{\n .reg .pred p;\n"
+                 "WAIT_LOOP:\n"
+                 " mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
+                 " @p bra WAIT_DONE;\n"
+                 " nanosleep.u32 %3;\n"
+                 " bra WAIT_LOOP;\n"
+                 "WAIT_DONE:\n}"
+                 ::"r"(smem_u32(bar)), "r"(parity), "r"(1000000u), "n"(kSleepNs) : "memory");
+}
 __device__ __forceinline__ void mma_f16_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc)
 {
     asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}"
@@ -503,7 +518,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                     asm volatile("bar.sync 5, %0;" ::"n"(kBinWarps * 32) : "memory");
                 }
             } else if (use >= 1) {
-                mbar_wait(&ps.free_[buf], (uint32_t)((use - 1) & 1));                  // cleared after its previous use
+                mbar_wait_lean(&ps.free_[buf], (uint32_t)((use - 1) & 1));             // cleared after its previous use
             }
             const int a0 = pass * 2048, a1 = min(n_ions, a0 + 2048);
             const int nq = (a1 - a0 + 3) >> 2;                                       // quads of this pass, split evenly
@@ -588,7 +603,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         const int q = warp & 3, set = (warp - kSvcWarp0) >> 2;
         for (int gl = (set ^ sq.grp_base) & 1; gl < sq.ngrp; gl += 2) {
             const int gq = sq.grp_base + gl;
-            mbar_wait<200>(&ps.epi[set], (uint32_t)((gq >> 1) & 1));
+            mbar_wait_lean<200>(&ps.epi[set], (uint32_t)((gq >> 1) & 1));
             asm volatile("tcgen05.fence::after_thread_sync;");
             EpiOut eo;
             eo.mode = mode; eo.gi = sq.g0 + gl; eo.g0 = sq.g0; eo.f = gl; eo.nfix = sq.nfix;

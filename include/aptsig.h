@@ -78,9 +78,12 @@ int apx_last_cuda_error(const apx_plan *plan);
 
 /* Step a1: ingest an ion cloud: drop ions of rejected types and non-finite coordinates, bucket the
  * rest into a uniform cell grid (cell edge ~R/2) by a counting sort on the device.
- *   xyz   DEVICE float32[N][3]     types DEVICE uint8[N] or NULL (NULL = every ion is type 0)
+ *   xyz   DEVICE float32[N][3]     types DEVICE uint8[N] or NULL (NULL = no type information: every
+ *                                  ion is accepted, the plan's type mask is not applied)
  * The plan keeps the sorted copy (16 B per ion) until the next ingest; xyz/types are not referenced
- * after the enqueued work completed.  N = 0 is valid (all ROIs empty). */
+ * after the enqueued work completed.  N = 0 is valid (all ROIs empty).  The first call with a larger N
+ * than any before grows the plan's buffers (cudaMalloc: synchronises the device); apx_plan_reserve
+ * sizes them ahead of time. */
 int apx_ingest(apx_plan *plan, const float *xyz, const uint8_t *types, int64_t N, void *cuda_stream);
 
 /* Steps a2-a7 for M material points against the ingested cloud.
@@ -88,24 +91,37 @@ int apx_ingest(apx_plan *plan, const float *xyz, const uint8_t *types, int64_t N
  *   sig     DEVICE float32[M][D][2]: sig[m][d] = (A*, (float)k*), A* = max_{k in window} |X_k|
  *           (unnormalised, A_0 would be the ion count), k* the smallest such k.  Empty ROI: (0, k_lo).
  *   counts  DEVICE uint32[M] or NULL: number of ions in each ROI (N_c) for caller-side normalisation.
- * M = 0 is valid.  Requires a prior apx_ingest (else APX_ESTATE). */
+ * M = 0 is valid.  Requires a prior apx_ingest (else APX_ESTATE).  Asynchronous, except that the
+ * tensor-core path grows its list of deferred material points (4 B per point and chunk) the first
+ * time a larger M is seen; apx_plan_reserve avoids that. */
 int apx_query(apx_plan *plan, const float *centres, int64_t M, float *sig, uint32_t *counts,
               void *cuda_stream);
+
+/* Pre-allocate every internal buffer for clouds of up to N_max ions and queries of up to M_max material
+ * points, so that later apx_ingest / apx_query / apx_run calls never allocate (and never synchronise).
+ * Optional: without it buffers grow on demand. */
+int apx_plan_reserve(apx_plan *plan, int64_t N_max, int64_t M_max);
 
 /* apx_ingest followed by apx_query on the same stream (north_star's run()). */
 int apx_run(apx_plan *plan, const float *xyz, const uint8_t *types, int64_t N,
             const float *centres, int64_t M, float *sig, uint32_t *counts, void *cuda_stream);
 
 /* Same as apx_run but every array is a HOST pointer (pinned memory makes the copies asynchronous): inputs are
- * copied in on an internal stream, the material points are processed in up to four slabs, and the signatures of a
- * slab travel back on a second internal stream while the next slab is computed.  Synchronises before returning
- * (the end-to-end entry bench.py's "e2e" figure is timed through). */
+ * copied in on an internal stream, the material points are processed in slabs (at least four when M > 128, each
+ * at most 1 GiB of signatures), and the signatures of a slab travel back on a second internal stream while the
+ * next slab is computed into the other of two device staging buffers (so the device never holds more than 2 GiB
+ * of output, whatever M).  Synchronises both internal streams before returning, also on errors (the end-to-end
+ * entry bench.py's "e2e" figure is timed through). */
 int apx_run_host(apx_plan *plan, const float *xyz, const uint8_t *types, int64_t N,
                  const float *centres, int64_t M, float *sig, uint32_t *counts);
 
 /* Test hook: integer histograms (Eq. 1) of ONE material point for directions [d0, d0+nd):
- *   centre3 HOST float32[3],  out DEVICE uint32[nd][B] (overwritten).  Uses the same gather and the
- *   same binning arithmetic as the production kernels. */
+ *   centre3 HOST float32[3],  out DEVICE uint32[nd][B] (overwritten).
+ * Runs the plan's PRODUCTION kernel (the one apx_query launches for this plan: tensor-core or FFT path, with its
+ * gather, packed binning arithmetic, half-grid mirroring and fix-up groups, spill / multi-pass / deferred handling)
+ * on that one material point with an export switched on: the kernel copies every group's shared-memory histogram --
+ * the very buffer the DFT then reads -- to `out`, decoding the tensor-core path's interleaved u16 counters; in
+ * half-grid mode the direction opposite to a binned one receives the reversed histogram, as the kernel assumes. */
 int apx_debug_histograms(apx_plan *plan, const float *centre3, int32_t d0, int32_t nd, uint32_t *out,
                          void *cuda_stream);
 

@@ -4,11 +4,11 @@ The product is the CUDA library `libaptsig.so` (sources in csrc/, ABI in include
 package is its ctypes binding.  Importing the package does not load the library; the first call does,
 and raises if it has not been built (there is no CPU fallback).
 """
-from .binding import (Plan, ApxError, apx_dirs_fibonacci, apx_dirs_geodesic, apx_dirs_antipodes, apx_version, EXPORTS, LIB_PATH,
+from .binding import (Plan, ApxError, apx_peak_name, apx_peak_measure, PEAK_EXPORTS, apx_dirs_fibonacci, apx_dirs_geodesic, apx_dirs_antipodes, apx_version, EXPORTS, LIB_PATH,
                       APX_FLAG_FORCE_FFT, APX_FLAG_FORCE_MMA, APX_FLAG_NO_PAIRING, APX_OK, APX_EINVAL, APX_ENOMEM, APX_ECUDA,
                       APX_ESTATE, APX_ERANGE)
 
 from .parallel import shard_range, run_sharded, gather_counts
 
-__all__ = ["shard_range", "run_sharded", "gather_counts", "Plan", "ApxError", "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_dirs_antipodes", "apx_version", "EXPORTS", "LIB_PATH",
+__all__ = ["apx_peak_name", "apx_peak_measure", "PEAK_EXPORTS", "shard_range", "run_sharded", "gather_counts", "Plan", "ApxError", "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_dirs_antipodes", "apx_version", "EXPORTS", "LIB_PATH",
            "APX_FLAG_FORCE_FFT", "APX_FLAG_FORCE_MMA", "APX_FLAG_NO_PAIRING"]

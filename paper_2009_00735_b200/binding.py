@@ -16,8 +16,9 @@ APX_OK, APX_EINVAL, APX_ENOMEM, APX_ECUDA, APX_ESTATE, APX_ERANGE = 0, -1, -2, -
 APX_FLAG_FORCE_FFT, APX_FLAG_FORCE_MMA, APX_FLAG_NO_PAIRING = 1, 2, 4
 
 EXPORTS = ["apx_plan_create", "apx_plan_destroy", "apx_plan_constants", "apx_plan_path", "apx_plan_paired", "apx_last_cuda_error",
-           "apx_ingest", "apx_query", "apx_run", "apx_run_host", "apx_debug_histograms",
+           "apx_plan_reserve", "apx_ingest", "apx_query", "apx_run", "apx_run_host", "apx_debug_histograms",
            "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_dirs_antipodes", "apx_strerror", "apx_version"]
+PEAK_EXPORTS = ["apx_peak_name", "apx_peak_measure"]          # include/aptsig_peaks.h
 
 
 class apx_plan_desc(C.Structure):
@@ -26,10 +27,19 @@ class apx_plan_desc(C.Structure):
                 ("device", C.c_int32), ("flags", C.c_int32)]
 
 
+class apx_peak_result(C.Structure):
+    _fields_ = [("sm_count", C.c_int), ("ms", C.c_float), ("median_cycles", C.c_double), ("warp_inst_per_s", C.c_double),
+                ("warp_inst_per_clk_per_sm", C.c_double), ("sm_mhz_effective", C.c_double)]
+
+
 class ApxError(RuntimeError):
     def __init__(self, status, where, cuda=None):
         self.status = status
-        msg = f"{where}: {_lib().apx_strerror(status).decode()} ({status})"
+        try:
+            text = _lib().apx_strerror(status).decode()
+        except Exception:
+            text = "error"
+        msg = f"{where}: {text} ({status})"
         if cuda is not None:
             msg += f" [cudaError {cuda}]"
         super().__init__(msg)
@@ -52,6 +62,7 @@ def _lib():
         L.apx_plan_path.argtypes = [vp]
         L.apx_plan_paired.argtypes = [vp]
         L.apx_last_cuda_error.argtypes = [vp]
+        L.apx_plan_reserve.argtypes = [vp, i64, i64]
         L.apx_ingest.argtypes = [vp, vp, vp, i64, vp]
         L.apx_query.argtypes = [vp, vp, i64, vp, vp, vp]
         L.apx_run.argtypes = [vp, vp, vp, i64, vp, i64, vp, vp, vp]
@@ -63,6 +74,10 @@ def _lib():
         L.apx_strerror.argtypes = [C.c_int]
         L.apx_strerror.restype = C.c_char_p
         L.apx_version.restype = C.c_char_p
+        L.apx_peak_name.argtypes = [C.c_int]
+        L.apx_peak_name.restype = C.c_char_p
+        L.apx_peak_measure.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(apx_peak_result)]
+        L.apx_peak_measure.restype = C.c_int
         for name in EXPORTS:
             if name not in ("apx_strerror", "apx_version"):
                 getattr(L, name).restype = C.c_int
@@ -114,20 +129,56 @@ def apx_dirs_antipodes(dirs: np.ndarray):
     return bool(rc), partner
 
 
-def _ptr(t, dtype=None):
-    """device (or host) pointer of a torch tensor / numpy array / None, after layout checks."""
+def apx_peak_name(test: int):
+    n = _lib().apx_peak_name(int(test))
+    return None if n is None else n.decode()
+
+
+def apx_peak_measure(device: int, test: int, iters: int) -> dict:
+    """One on-chip peak microbenchmark (include/aptsig_peaks.h) -> dict of the result struct's fields."""
+    r = apx_peak_result()
+    rc = _lib().apx_peak_measure(int(device), int(test), int(iters), C.byref(r))
+    if rc:
+        raise ApxError(rc, "apx_peak_measure")
+    return {k: getattr(r, k) for k, _ in apx_peak_result._fields_}
+
+
+def _is_np(t):
+    return isinstance(t, np.ndarray)
+
+
+def _arg(t, name, dtype, shape, device=None, optional=False):
+    """Pointer of a torch tensor / numpy array after checking dtype, shape, contiguity and placement.
+    device = CUDA ordinal the array must live on, or None for a HOST array (numpy or CPU tensor)."""
     if t is None:
-        return None
-    if isinstance(t, np.ndarray):
-        assert t.flags.c_contiguous and (dtype is None or t.dtype == dtype)
-        return t.ctypes.data
-    assert t.is_contiguous(), "tensor must be contiguous"
-    return t.data_ptr()
-
-
-def _stream(stream=None):
-    import torch
-    return (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+        if optional:
+            return None
+        raise ApxError(APX_EINVAL, f"{name}: missing")
+    want = np.dtype(dtype)
+    if _is_np(t):
+        if device is not None:
+            raise ApxError(APX_EINVAL, f"{name}: expected a tensor on cuda:{device}, got a numpy array")
+        have, contiguous, ptr = t.dtype, t.flags.c_contiguous, t.ctypes.data
+    else:
+        try:
+            have = np.dtype(str(t.dtype).replace("torch.", ""))
+        except TypeError:
+            raise ApxError(APX_EINVAL, f"{name}: dtype {t.dtype}, expected {want}") from None
+        contiguous, ptr = t.is_contiguous(), t.data_ptr()
+        if device is None:
+            if t.device.type != "cpu":
+                raise ApxError(APX_EINVAL, f"{name}: expected a host array, got {t.device}")
+        elif t.device.type != "cuda" or t.device.index != device:
+            raise ApxError(APX_EINVAL, f"{name}: expected a tensor on cuda:{device}, got {t.device}")
+    # 4-byte integer outputs may be int32 or uint32 (torch has no full uint32 support)
+    same = have == want or (want == np.uint32 and have == np.int32)
+    if not same:
+        raise ApxError(APX_EINVAL, f"{name}: dtype {have}, expected {want}")
+    if tuple(t.shape) != tuple(shape):
+        raise ApxError(APX_EINVAL, f"{name}: shape {tuple(t.shape)}, expected {tuple(shape)}")
+    if not contiguous:
+        raise ApxError(APX_EINVAL, f"{name}: must be contiguous")
+    return ptr
 
 
 class Plan:
@@ -164,26 +215,49 @@ class Plan:
     def apx_plan_paired(self) -> int:
         return _lib().apx_plan_paired(self._h)
 
+    def _stream(self, stream=None):
+        import torch
+        return (torch.cuda.current_stream(self.device) if stream is None else stream).cuda_stream
+
+    def apx_plan_reserve(self, N_max, M_max):
+        self._check(_lib().apx_plan_reserve(self._h, int(N_max), int(M_max)), "apx_plan_reserve")
+
     def apx_ingest(self, xyz, types=None, stream=None):
-        self._check(_lib().apx_ingest(self._h, _ptr(xyz), _ptr(types), xyz.shape[0], _stream(stream)), "apx_ingest")
+        N, dev = int(xyz.shape[0]), self.device
+        self._check(_lib().apx_ingest(self._h, _arg(xyz, "xyz", np.float32, (N, 3), dev),
+                                      _arg(types, "types", np.uint8, (N,), dev, optional=True), N,
+                                      self._stream(stream)), "apx_ingest")
 
     def apx_query(self, centres, sig, counts=None, stream=None):
-        self._check(_lib().apx_query(self._h, _ptr(centres), centres.shape[0], _ptr(sig), _ptr(counts),
-                                     _stream(stream)), "apx_query")
+        M, dev = int(centres.shape[0]), self.device
+        self._check(_lib().apx_query(self._h, _arg(centres, "centres", np.float32, (M, 3), dev), M,
+                                     _arg(sig, "sig", np.float32, (M, self.D, 2), dev),
+                                     _arg(counts, "counts", np.uint32, (M,), dev, optional=True),
+                                     self._stream(stream)), "apx_query")
 
     def apx_run(self, xyz, types, centres, sig, counts=None, stream=None):
-        self._check(_lib().apx_run(self._h, _ptr(xyz), _ptr(types), xyz.shape[0], _ptr(centres), centres.shape[0],
-                                   _ptr(sig), _ptr(counts), _stream(stream)), "apx_run")
+        N, M, dev = int(xyz.shape[0]), int(centres.shape[0]), self.device
+        self._check(_lib().apx_run(self._h, _arg(xyz, "xyz", np.float32, (N, 3), dev),
+                                   _arg(types, "types", np.uint8, (N,), dev, optional=True), N,
+                                   _arg(centres, "centres", np.float32, (M, 3), dev), M,
+                                   _arg(sig, "sig", np.float32, (M, self.D, 2), dev),
+                                   _arg(counts, "counts", np.uint32, (M,), dev, optional=True),
+                                   self._stream(stream)), "apx_run")
 
     def apx_run_host(self, xyz, types, centres, sig, counts=None):
         """All arguments are HOST arrays (numpy, or pinned CPU torch tensors)."""
-        self._check(_lib().apx_run_host(self._h, _ptr(xyz), _ptr(types), xyz.shape[0], _ptr(centres),
-                                        centres.shape[0], _ptr(sig), _ptr(counts)), "apx_run_host")
+        N, M = int(xyz.shape[0]), int(centres.shape[0])
+        self._check(_lib().apx_run_host(self._h, _arg(xyz, "xyz", np.float32, (N, 3)),
+                                        _arg(types, "types", np.uint8, (N,), optional=True), N,
+                                        _arg(centres, "centres", np.float32, (M, 3)), M,
+                                        _arg(sig, "sig", np.float32, (M, self.D, 2)),
+                                        _arg(counts, "counts", np.uint32, (M,), optional=True)), "apx_run_host")
 
     def apx_debug_histograms(self, centre3, d0, nd, out, stream=None):
         c = (C.c_float * 3)(*[float(v) for v in centre3])
-        self._check(_lib().apx_debug_histograms(self._h, c, d0, nd, _ptr(out), _stream(stream)),
-                    "apx_debug_histograms")
+        self._check(_lib().apx_debug_histograms(self._h, c, int(d0), int(nd),
+                                                _arg(out, "out", np.uint32, (int(nd), self.B), self.device),
+                                                self._stream(stream)), "apx_debug_histograms")
 
     def apx_plan_destroy(self):
         if self._h:

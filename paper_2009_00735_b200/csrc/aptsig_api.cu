@@ -21,6 +21,23 @@ struct apx_plan : public apx::Plan {};
         }                                             \
     } while (0)
 
+// Entry points run on the plan's device and leave the caller's current device as they found it.
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err;
+    explicit DeviceGuard(int dev)
+    {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != dev) err = cudaSetDevice(dev);
+    }
+    ~DeviceGuard()
+    {
+        int cur = -1;
+        if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+    }
+};
+#define ON_DEVICE(p) DeviceGuard guard__((p)->device); CU(p, guard__.err)
+
 static int ensure_capacity(apx_plan *p, int64_t N)
 {
     if (N <= p->capacity) return APX_OK;
@@ -47,16 +64,18 @@ static int grow(apx_plan *p, void **buf, int64_t *cap, int64_t bytes)
 extern "C" int apx_plan_destroy(apx_plan *p)
 {
     if (!p) return APX_OK;
-    cudaSetDevice(p->device);
-    void *bufs[] = {p->d_dirs_scaled, p->d_twiddle, p->d_mma_table, p->d_mma_zero, p->d_mma_phase, p->d_dirs_sorted, p->d_dir_perm, p->d_dir_perm_mirror, p->d_type_mask, p->d_grid, p->d_cell_start,
+    DeviceGuard guard(p->device);
+    void *bufs[] = {p->dbg_centre, p->dbg_sig, p->d_dirs_scaled, p->d_twiddle, p->d_mma_table, p->d_mma_zero, p->d_mma_phase, p->d_dirs_sorted, p->d_dir_perm, p->d_dir_perm_mirror, p->d_type_mask, p->d_grid, p->d_cell_start,
                     p->d_cell_cursor, p->d_scan_tiles, p->d_cell_of_ion, p->d_sorted, p->d_deferred, p->h2d_xyz, p->h2d_types, p->h2d_centres,
                     p->d2h_sig, p->d2h_counts};
     for (void *b : bufs)
         if (b) cudaFree(b);
     if (p->own_stream) cudaStreamDestroy(p->own_stream);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
-    for (int i = 0; i < 2; ++i)
+    for (int i = 0; i < 2; ++i) {
         if (p->slab_done[i]) cudaEventDestroy(p->slab_done[i]);
+        if (p->copy_done[i]) cudaEventDestroy(p->copy_done[i]);
+    }
     delete p;
     return APX_OK;
 }
@@ -88,8 +107,8 @@ extern "C" int apx_plan_create(const apx_plan_desc *desc, apx_plan **out)
     p->s = (float)((double)(B / 2 - desc->pad) / (double)desc->R);             // fp64, rounded once
 
     auto fail = [&](int code) { apx_plan_destroy(p); return code; };
-    cudaError_t e = cudaSetDevice(p->device);
-    if (e != cudaSuccess) { delete p; return APX_ECUDA; }
+    DeviceGuard guard(p->device);
+    if (guard.err != cudaSuccess) { delete p; return APX_ECUDA; }
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) { delete p; return APX_ECUDA; }
     p->sm_count = prop.multiProcessorCount;
@@ -121,6 +140,9 @@ extern "C" int apx_plan_create(const apx_plan_desc *desc, apx_plan **out)
     CUF(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
     CUF(cudaEventCreateWithFlags(&p->slab_done[0], cudaEventDisableTiming));
     CUF(cudaEventCreateWithFlags(&p->slab_done[1], cudaEventDisableTiming));
+    CUF(cudaEventCreateWithFlags(&p->copy_done[0], cudaEventDisableTiming));
+    CUF(cudaEventCreateWithFlags(&p->copy_done[1], cudaEventDisableTiming));
+    CUF(cudaMalloc(&p->dbg_centre, 16));
 
     // the clamp of Eq. 1's bin index can be skipped when it provably never triggers: paper padding (pad = 1) and
     // directions that are unit vectors to fp32 accuracy => |x| <= (B/2-1)(1+2e-5) < B/2 - 0.25
@@ -163,7 +185,7 @@ extern "C" int apx_ingest(apx_plan *p, const float *xyz, const uint8_t *types, i
 {
     if (!p || N < 0 || (N > 0 && !xyz)) return APX_EINVAL;
     if (N >= (1LL << 31)) return APX_ERANGE;
-    CU(p, cudaSetDevice(p->device));
+    ON_DEVICE(p);
     int rc = ensure_capacity(p, N);
     if (rc) return rc;
     CU(p, launch_ingest(p, xyz, types, N, (cudaStream_t)stream));
@@ -176,7 +198,7 @@ extern "C" int apx_query(apx_plan *p, const float *centres, int64_t M, float *si
     if (!p || M < 0 || (M > 0 && (!centres || !sig))) return APX_EINVAL;
     if (!p->ingested) return APX_ESTATE;
     if ((double)M * (double)p->D >= 1099511627776.0) return APX_ERANGE;
-    CU(p, cudaSetDevice(p->device));
+    ON_DEVICE(p);
     if (p->path == 1) CU(p, launch_signature_mma(p, centres, M, sig, counts, (cudaStream_t)stream));
     else CU(p, launch_signature_fft(p, centres, M, sig, counts, (cudaStream_t)stream));
     return APX_OK;
@@ -190,51 +212,95 @@ extern "C" int apx_run(apx_plan *p, const float *xyz, const uint8_t *types, int6
     return apx_query(p, centres, M, sig, counts, stream);
 }
 
+extern "C" int apx_plan_reserve(apx_plan *p, int64_t N_max, int64_t M_max)
+{
+    if (!p || N_max < 0 || M_max < 0) return APX_EINVAL;
+    if (N_max >= (1LL << 31)) return APX_ERANGE;
+    ON_DEVICE(p);
+    int rc = ensure_capacity(p, N_max);
+    if (rc) return rc;
+    if (p->path == 1) CU(p, mma_reserve_for(p, M_max));
+    return APX_OK;
+}
+
+// Output staging of apx_run_host: two device slabs of at most kSlabBytes each, used alternately (slab i in buffer
+// i & 1): the signatures of slab i travel to the host on the copy stream while slab i + 1 is computed.
+static const int64_t kSlabBytes = 1LL << 30;
+
 extern "C" int apx_run_host(apx_plan *p, const float *xyz, const uint8_t *types, int64_t N, const float *centres,
                             int64_t M, float *sig, uint32_t *counts)
 {
     if (!p || N < 0 || M < 0 || (N > 0 && !xyz) || (M > 0 && (!centres || !sig))) return APX_EINVAL;
-    CU(p, cudaSetDevice(p->device));
+    if (N >= (1LL << 31)) return APX_ERANGE;
+    ON_DEVICE(p);
     cudaStream_t st = p->own_stream;
+    const int64_t row_bytes = (int64_t)p->D * 8;
+    // material points per slab: bounded by the staging size, and at most a quarter of the job so that copies overlap
+    int64_t slab = kSlabBytes / row_bytes;
+    if (slab < 1) slab = 1;
+    if (M > 128 && slab > (M + 3) / 4) slab = (M + 3) / 4;
+    if (slab > M) slab = M > 0 ? M : 1;
+    const int64_t nslab = M > 0 ? (M + slab - 1) / slab : 0;
     int rc;
-    const int64_t sig_bytes = M * (int64_t)p->D * 8;
     if ((rc = grow(p, &p->h2d_xyz, &p->cap_xyz, N * 12 + 16))) return rc;
     if (types && (rc = grow(p, &p->h2d_types, &p->cap_types, N + 16))) return rc;
     if ((rc = grow(p, &p->h2d_centres, &p->cap_centres, M * 12 + 16))) return rc;
-    if ((rc = grow(p, &p->d2h_sig, &p->cap_sig, sig_bytes + 16))) return rc;
+    if ((rc = grow(p, &p->d2h_sig, &p->cap_sig, (nslab > 1 ? 2 : 1) * slab * row_bytes + 16))) return rc;
     if (counts && (rc = grow(p, &p->d2h_counts, &p->cap_counts, M * 4 + 16))) return rc;
-    if (N) CU(p, cudaMemcpyAsync(p->h2d_xyz, xyz, (size_t)N * 12, cudaMemcpyHostToDevice, st));
-    if (N && types) CU(p, cudaMemcpyAsync(p->h2d_types, types, (size_t)N, cudaMemcpyHostToDevice, st));
-    if (M) CU(p, cudaMemcpyAsync(p->h2d_centres, centres, (size_t)M * 12, cudaMemcpyHostToDevice, st));
-    // ingest once, then the material points in slabs: while slab i+1 is computed on the compute stream the signatures
-    // of slab i travel to the host on the copy stream (the 8 B per histogram of output dominate the PCIe traffic)
+    if ((rc = ensure_capacity(p, N))) return rc;
+    if (p->path == 1) CU(p, mma_reserve_for(p, slab));
+    // from here on work is in flight on the two internal streams: never return before both have drained, the copies
+    // read and write the caller's host buffers
+    auto drain = [&](int code) {
+        cudaStreamSynchronize(p->copy_stream);
+        cudaStreamSynchronize(st);
+        return code;
+    };
+#define CUD(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { p->last_cuda = (int)e__; \
+        return drain(e__ == cudaErrorMemoryAllocation ? APX_ENOMEM : APX_ECUDA); } } while (0)
+    if (N) CUD(cudaMemcpyAsync(p->h2d_xyz, xyz, (size_t)N * 12, cudaMemcpyHostToDevice, st));
+    if (N && types) CUD(cudaMemcpyAsync(p->h2d_types, types, (size_t)N, cudaMemcpyHostToDevice, st));
+    if (M) CUD(cudaMemcpyAsync(p->h2d_centres, centres, (size_t)M * 12, cudaMemcpyHostToDevice, st));
     rc = apx_ingest(p, (const float *)p->h2d_xyz, types ? (const uint8_t *)p->h2d_types : nullptr, N, st);
-    if (rc) return rc;
-    const int64_t slab = M <= 128 ? (M > 0 ? M : 1) : (M + 3) / 4;
+    if (rc) return drain(rc);
     for (int64_t m0 = 0, i = 0; m0 < M; m0 += slab, ++i) {
         const int64_t mc = (M - m0 < slab) ? M - m0 : slab;
-        float *dsig = (float *)p->d2h_sig + m0 * (int64_t)p->D * 2;
+        float *dsig = (float *)p->d2h_sig + (i & 1) * slab * (int64_t)p->D * 2;
         uint32_t *dcnt = counts ? (uint32_t *)p->d2h_counts + m0 : nullptr;
+        if (i >= 2) CUD(cudaStreamWaitEvent(st, p->copy_done[i & 1], 0));       // the buffer's previous slab has left
         rc = apx_query(p, (const float *)p->h2d_centres + 3 * m0, mc, dsig, dcnt, st);
-        if (rc) return rc;
-        CU(p, cudaEventRecord(p->slab_done[i & 1], st));
-        CU(p, cudaStreamWaitEvent(p->copy_stream, p->slab_done[i & 1], 0));
-        CU(p, cudaMemcpyAsync(sig + m0 * (int64_t)p->D * 2, dsig, (size_t)(mc * (int64_t)p->D * 8), cudaMemcpyDeviceToHost, p->copy_stream));
-        if (counts) CU(p, cudaMemcpyAsync(counts + m0, dcnt, (size_t)mc * 4, cudaMemcpyDeviceToHost, p->copy_stream));
+        if (rc) return drain(rc);
+        CUD(cudaEventRecord(p->slab_done[i & 1], st));
+        CUD(cudaStreamWaitEvent(p->copy_stream, p->slab_done[i & 1], 0));
+        CUD(cudaMemcpyAsync(sig + m0 * (int64_t)p->D * 2, dsig, (size_t)(mc * row_bytes), cudaMemcpyDeviceToHost, p->copy_stream));
+        if (counts) CUD(cudaMemcpyAsync(counts + m0, dcnt, (size_t)mc * 4, cudaMemcpyDeviceToHost, p->copy_stream));
+        CUD(cudaEventRecord(p->copy_done[i & 1], p->copy_stream));
     }
+#undef CUD
     CU(p, cudaStreamSynchronize(p->copy_stream));
     CU(p, cudaStreamSynchronize(st));
     return APX_OK;
 }
 
+// Test hook: ONE material point through the plan's production kernel (the one apx_query launches: tensor-core or FFT
+// path, half-grid mode, spill / multi-pass / deferred handling included) with the histogram export switched on.
 extern "C" int apx_debug_histograms(apx_plan *p, const float *centre3, int32_t d0, int32_t nd, uint32_t *out,
                                     void *stream)
 {
     if (!p || !centre3 || d0 < 0 || nd < 0 || d0 + nd > p->D || (nd > 0 && !out)) return APX_EINVAL;
     if (!p->ingested) return APX_ESTATE;
-    CU(p, cudaSetDevice(p->device));
-    CU(p, launch_debug_hist(p, centre3, d0, nd, out, (cudaStream_t)stream));
-    return APX_OK;
+    if (nd == 0) return APX_OK;
+    ON_DEVICE(p);
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    int64_t cap = p->dbg_sig ? (int64_t)p->D * 8 : 0;
+    if ((rc = grow(p, (void **)&p->dbg_sig, &cap, (int64_t)p->D * 8))) return rc;
+    CU(p, cudaMemcpyAsync(p->dbg_centre, centre3, 12, cudaMemcpyHostToDevice, st));
+    CU(p, cudaMemsetAsync(out, 0, (size_t)nd * p->B * sizeof(uint32_t), st));
+    p->dbg_hist_out = out; p->dbg_d0 = d0; p->dbg_nd = nd;
+    rc = apx_query(p, p->dbg_centre, 1, p->dbg_sig, nullptr, st);
+    p->dbg_hist_out = nullptr; p->dbg_d0 = 0; p->dbg_nd = 0;
+    return rc;
 }
 
 extern "C" const char *apx_strerror(int s)

@@ -43,6 +43,10 @@ struct Plan {
     int need_clamp;                // 1 = the bin clamp of Eq. 1 can trigger and must stay in the kernels' inner loops
     uint32_t *d_deferred;          // [0] count, [1..] material points the MMA kernel left to the FFT kernel
     int64_t cap_deferred;
+    uint32_t *dbg_hist_out;        // non-null only inside apx_debug_histograms: the kernels also export their histograms
+    int dbg_d0, dbg_nd;
+    float *dbg_centre;             // [3] device copy of the debug centre
+    float *dbg_sig;                // [D][2] scratch signature output of the debug run
     uint32_t *d_type_mask;         // [8] words
     GridParams *d_grid;
     uint32_t *d_cell_start;        // [kMaxCells + 1]
@@ -53,7 +57,7 @@ struct Plan {
     int64_t capacity;              // ions the sorted buffers can hold
     // host staging for apx_run_host
     cudaStream_t own_stream, copy_stream;
-    cudaEvent_t slab_done[2];
+    cudaEvent_t slab_done[2], copy_done[2];
     void *h2d_xyz, *h2d_types, *h2d_centres, *d2h_sig, *d2h_counts;   // device-side staging
     int64_t cap_xyz, cap_types, cap_centres, cap_sig, cap_counts;
 };
@@ -112,8 +116,9 @@ cudaError_t launch_signature_fft_list(Plan *p, const float *centres, const uint3
                                       uint32_t *counts, cudaStream_t st);
 cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts,
                                  cudaStream_t st);
-cudaError_t launch_debug_hist(Plan *p, const float *centre3, int d0, int nd, uint32_t *out, cudaStream_t st);
 bool mma_path_supported(const Plan *p);
 cudaError_t mma_path_prepare(Plan *p);   // builds d_mma_table
+cudaError_t mma_reserve_deferred(Plan *p, int64_t need);   // deferred list of at least `need` words
+cudaError_t mma_reserve_for(Plan *p, int64_t M);           // ... sized for any apx_query of up to M material points
 
 }  // namespace apx

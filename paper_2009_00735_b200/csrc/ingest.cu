@@ -18,10 +18,15 @@ __device__ __forceinline__ float ord2f(int i) { return __int_as_float(i >= 0 ? i
 __device__ __forceinline__ bool accepted(const uint32_t *mask, const uint8_t *types, int64_t i,
                                          float x, float y, float z)
 {
-    unsigned t = types ? types[i] : 0u;
-    bool ok = (mask[t >> 5] >> (t & 31)) & 1u;
-    // finite test: |v| < inf  (NaN compares false)
-    return ok && fabsf(x) < 3.0e38f && fabsf(y) < 3.0e38f && fabsf(z) < 3.0e38f;
+    // no type array = no type information = no filter (the oracle's reading of L52 "selected atom types")
+    bool ok = true;
+    if (types) {
+        const unsigned t = types[i];
+        ok = (mask[t >> 5] >> (t & 31)) & 1u;
+    }
+    // finite test: |v| < inf  (NaN compares false; every finite float passes)
+    const float inf = __int_as_float(0x7f800000);
+    return ok && fabsf(x) < inf && fabsf(y) < inf && fabsf(z) < inf;
 }
 
 __global__ void k_reset(GridParams *g)

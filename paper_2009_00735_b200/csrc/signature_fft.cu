@@ -32,6 +32,8 @@ struct FftParams {
     float2 *sig;
     uint32_t *counts;
     const uint32_t *list;      // nullptr = direct mode; else list[0] = count, list[1..] = material point ids
+    uint32_t *hist_out;        // test hook (apx_debug_histograms, M = 1): uint32[hist_nd][B] histograms of the directions
+    int hist_d0, hist_nd;      // [hist_d0, hist_d0 + hist_nd), copied from the shared counters the FFT is about to read
     int D, k_lo, k_hi, cap, nchunks, ngroups, clamp;
     float R, R2;
 };
@@ -241,6 +243,15 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const FftParam
                 }
             }
             __syncthreads();
+            if (p.hist_out) {                                    // test hook: the counters are complete, the FFT has not started
+                const uint32_t *ub = reinterpret_cast<const uint32_t *>(buf);
+                for (int i = tid; i < B * G; i += kFftThreads) {
+                    const int b = i / G, dg = gi * G + i % G;
+                    if (dg < p.D && dg >= p.hist_d0 && dg < p.hist_d0 + p.hist_nd)
+                        p.hist_out[(size_t)(dg - p.hist_d0) * B + b] = ub[i];
+                }
+                __syncthreads();
+            }
             // ---- packed real FFT (step a5): radix-8 DIF passes in place, then the remaining radix 2 / 4 ----
             fft_pass<B, G, 8, true>(buf, s_tw, d, t, N);
             __syncthreads();
@@ -308,6 +319,7 @@ static cudaError_t launch_fft_common(Plan *p, const float *centres, int64_t M, c
     FftParams q;
     q.sorted = p->d_sorted; q.cell_start = p->d_cell_start; q.grid = p->d_grid; q.centres = centres;
     q.dirs_scaled = p->d_dirs_scaled; q.tw = p->d_twiddle; q.sig = reinterpret_cast<float2 *>(sig); q.counts = counts;
+    q.hist_out = p->dbg_hist_out; q.hist_d0 = p->dbg_d0; q.hist_nd = p->dbg_nd;
     q.list = list; q.D = p->D; q.k_lo = p->k_lo; q.k_hi = p->k_hi; q.cap = fft_cap_for(B);
     q.ngroups = (p->D + G - 1) / G;
     // enough CTAs to fill the machine a few times over, but at least a handful of groups per CTA (one gather each)

@@ -150,6 +150,8 @@ struct MmaParams {
     float2 *sig;
     uint32_t *counts;
     uint32_t *deferred;        // [0] = count, [1..] = material point ids left to the FFT kernel
+    uint32_t *hist_out;        // test hook (apx_debug_histograms, M = 1): uint32[hist_nd][B] histograms of the directions
+    int hist_d0, hist_nd;      // [hist_d0, hist_d0 + hist_nd), decoded from the shared-memory buffers the tensor core reads
     int D, B, nl, k_lo, W, N, cap, cap_big, nchunks, ngroups, clamp, M;
     int half;                  // 1 = half-grid mode: one direction per antipodal pair is binned (perm_mirror != nullptr)
     uint32_t tmem_cols;
@@ -448,6 +450,41 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
     // the set's cand is rewritten only after the barriers of the rounds of its next epilogue
 }
 
+// Test hook behind apx_debug_histograms: the MMA warp copies the group's histogram out of the shared-memory buffer the
+// binning warps have just filled (and the tensor core is about to read) into uint32[nd][B], un-interleaving the u16
+// halves: (bin b, slot) lives in half (slot / LW) of word (slot % LW) at byte (w/4)*SBO + (w%4)*4 + 16*hi3 + BLK*low.
+// Pass 0 of a group stores, later passes of a ROI with more than 2048 ions add.  Half-grid mode: the mirrored direction
+// gets the histogram reversed (b -> B-1-b) unless the pair is flagged; flagged pairs are stored by their fix-up group.
+template <int NB, bool kHalf>
+__device__ __noinline__ void export_hist(const MmaParams &p, const unsigned char *hist, int mode, int gi, int g0, int f, int nfix,
+                                         const uint16_t *fix, uint32_t mask, int pass, int lane)
+{
+    constexpr int G = Lay<NB>::G, LW = Lay<NB>::LW, SBO = Lay<NB>::SBO, BLK = Lay<NB>::BLK;
+    const int B = p.B, lowmask = (B >> 3) - 1;
+    for (int idx = lane; idx < B * G; idx += 32) {
+        const int b = idx / G, slot = idx % G, w = slot % LW, hf = slot / LW;
+        const int hi3 = b >> p.nl, low = b & lowmask;
+        const uint32_t v = *reinterpret_cast<const uint16_t *>(hist + (w >> 2) * SBO + (w & 3) * 4 + 16 * hi3 + BLK * low + 2 * hf);
+        int d = -1, d2 = -1;
+        if (mode == 0) {
+            d = p.perm[gi * G + slot];
+            if (kHalf && !((mask >> slot) & 1u)) d2 = p.perm_mirror[gi * G + slot];
+        } else {
+            const int e = f * G + slot;
+            if (e < nfix) d = p.perm_mirror[g0 * G + (int)fix[e]];      // binned as the direction opposite to the listed slot's
+        }
+        if (d >= p.hist_d0 && d < p.hist_d0 + p.hist_nd) {
+            uint32_t *o = p.hist_out + (size_t)(d - p.hist_d0) * B + b;
+            *o = pass ? *o + v : v;
+        }
+        if (d2 >= p.hist_d0 && d2 < p.hist_d0 + p.hist_nd) {
+            uint32_t *o = p.hist_out + (size_t)(d2 - p.hist_d0) * B + (B - 1 - b);
+            *o = pass ? *o + v : v;
+        }
+    }
+    __syncwarp();
+}
+
 // A sequence of direction groups for run_pipeline.  mode 0: the ordinary groups [g0, g0 + ngrp) of the plan's slot
 // order.  mode 1: fix-up groups of the half-grid mode, built from the list of flagged pairs of the sub-range that
 // starts at group g0 (slot s of fix-up group f = list entry 32 f + s, binned as the direction OPPOSITE to the
@@ -556,6 +593,9 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             mbar_wait<100>(&ps.full[buf], (uint32_t)(use & 1));
             if (pass == 0 && gq >= 2) mbar_wait(&ps.tfree[gq & 1], (uint32_t)(((gq >> 1) - 1) & 1));
             asm volatile("tcgen05.fence::after_thread_sync;");
+            if (p.hist_out)                                      // test hook: the buffer is complete (all binning warps arrived)
+                export_hist<NB, kHalf>(p, smem + (buf ? L.hist1 : L.hist0), mode, sq.g0 + gl, sq.g0, gl, sq.nfix, ps.fix,
+                                       (kHalf && mode == 0) ? ps.flag[gq & 3] : 0u, pass, lane);
             const uint32_t acc = tmem + (uint32_t)((gq & 1) * p.N);
             if (lane == 0) {
                 const uint32_t a_lo = a_lo0 + (uint32_t)buf * ((L.hist1 - L.hist0) >> 4);
@@ -946,11 +986,10 @@ cudaError_t mma_path_prepare(Plan *p)
     return cudaMemcpy(p->d_dir_perm_mirror, mirror.data(), mirror.size() * 4, cudaMemcpyHostToDevice);
 }
 
-cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts, cudaStream_t st)
+// chunks of direction groups per material point: one gather per material point when there are enough of them
+static int mma_nchunks_for(const Plan *p, int64_t M)
 {
-    if (M == 0) return cudaSuccess;
-    // deferred list (material points whose ROI overflows the shared ion buffer), grown on demand
-    int nchunks = 1;                                       // one gather per material point when there are enough of them
+    int nchunks = 1;
     const int slots_per_group = 128 / mma_nb_for(p->B);
     const int ngroups_all = p->Dp / slots_per_group;
     const int64_t want = (int64_t)p->sm_count * 8;
@@ -958,15 +997,40 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     if (nchunks > (ngroups_all + 1) / 2) nchunks = (ngroups_all + 1) / 2;
     if (nchunks < 1) nchunks = 1;
     if (nchunks > 1 && nchunks < 6 && (ngroups_all >> (nchunks + 1)) >= 2) ++nchunks;   // one more, smaller, tail chunk
-    const int64_t need_deferred = M * (nchunks + 1) + 1;   // ROIs too large (<= M) + fix-list overflows (<= 1 per CTA)
-    if (need_deferred > p->cap_deferred) {
-        if (p->d_deferred) cudaFree(p->d_deferred);
-        p->d_deferred = nullptr; p->cap_deferred = 0;
-        cudaError_t e = cudaMalloc(&p->d_deferred, (size_t)need_deferred * 4);
-        if (e != cudaSuccess) return e;
-        p->cap_deferred = need_deferred;
-    }
-    cudaError_t e = cudaMemsetAsync(p->d_deferred, 0, 4, st);
+    return nchunks;
+}
+
+cudaError_t mma_reserve_deferred(Plan *p, int64_t need)
+{
+    if (need <= p->cap_deferred) return cudaSuccess;
+    if (p->d_deferred) cudaFree(p->d_deferred);
+    p->d_deferred = nullptr; p->cap_deferred = 0;
+    cudaError_t e = cudaMalloc(&p->d_deferred, (size_t)need * 4);
+    if (e != cudaSuccess) return e;
+    p->cap_deferred = need;
+    return cudaSuccess;
+}
+
+cudaError_t mma_reserve_for(Plan *p, int64_t M)
+{
+    if (M <= 0) return cudaSuccess;
+    // M * (nchunks(M) + 1) + 1 is not monotone in M below sm_count * 8 (where nchunks drops to 1): take the maximum
+    int64_t need = M * (mma_nchunks_for(p, M) + 1) + 1;
+    for (int64_t m = 1; m <= std::min<int64_t>(M, (int64_t)p->sm_count * 8); ++m)
+        need = std::max(need, m * (mma_nchunks_for(p, m) + 1) + 1);
+    return mma_reserve_deferred(p, need);
+}
+
+cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts, cudaStream_t st)
+{
+    if (M == 0) return cudaSuccess;
+    const int nchunks = mma_nchunks_for(p, M);
+    const int slots_per_group = 128 / mma_nb_for(p->B);
+    // deferred list: ROIs too large (<= M) + fix-list overflows (<= 1 per CTA).  Grown here only when apx_plan_reserve
+    // has not sized it already (cudaFree / cudaMalloc synchronise the device: reserve first to keep apx_query asynchronous)
+    cudaError_t e = mma_reserve_deferred(p, M * (nchunks + 1) + 1);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(p->d_deferred, 0, 4, st);
     if (e != cudaSuccess) return e;
 
     MmaParams q;
@@ -974,6 +1038,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.dirs_sorted = p->d_dirs_sorted; q.perm = p->d_dir_perm; q.perm_mirror = p->mma_paired ? p->d_dir_perm_mirror : nullptr;
     q.table = reinterpret_cast<const uint4 *>(p->d_mma_table); q.phase = p->d_mma_phase; q.zeros = p->d_mma_zero;
     q.sig = reinterpret_cast<float2 *>(sig); q.counts = counts; q.deferred = p->d_deferred;
+    q.hist_out = p->dbg_hist_out; q.hist_d0 = p->dbg_d0; q.hist_nd = p->dbg_nd;
     q.D = p->D; q.B = p->B; q.k_lo = p->k_lo; q.W = p->W; q.N = mma_n_for(p->W);
     q.nl = 0;
     while ((8 << q.nl) < p->B) ++q.nl;

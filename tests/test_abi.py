@@ -21,12 +21,13 @@ def lib():
 
 
 def test_every_declared_symbol_is_exported(lib):
-    hdr = open(os.path.join(ROOT, "include", "aptsig.h")).read()
-    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(apx_[a-z_0-9]+)\s*\(", hdr))
-    assert declared == set(apx.EXPORTS), declared ^ set(apx.EXPORTS)
-    for name in declared:
-        assert getattr(lib, name) is not None
+    for header, exports in (("aptsig.h", apx.EXPORTS), ("aptsig_peaks.h", apx.PEAK_EXPORTS)):
+        hdr = open(os.path.join(ROOT, "include", header)).read()
+        hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+        declared = set(re.findall(r"\b(apx_[a-z_0-9]+)\s*\(", hdr))
+        assert declared == set(exports), declared ^ set(exports)
+        for name in declared:
+            assert getattr(lib, name) is not None
 
 
 def test_strerror_and_version():
@@ -81,3 +82,20 @@ def test_antipodal_partners_of_direction_grids():
     # scaling by the plan's s (one fp32 multiply per component) keeps the pairs exact
     sym, _ = apx.apx_dirs_antipodes((apx.apx_dirs_geodesic(4) * np.float32(255.5)).astype(np.float32))
     assert sym
+
+
+def test_binding_argument_checks_host_side():
+    """binding._arg: dtype / shape / contiguity / placement checks (the host-array half runs without a GPU)."""
+    from paper_2009_00735_b200.binding import _arg
+    a = np.zeros((5, 3), np.float32)
+    assert _arg(a, "xyz", np.float32, (5, 3)) == a.ctypes.data
+    assert _arg(None, "types", np.uint8, (5,), optional=True) is None
+    assert _arg(np.zeros(4, np.int32), "counts", np.uint32, (4,)) is not None      # int32 storage for uint32 counts
+    for bad in (lambda: _arg(a.astype(np.float64), "xyz", np.float32, (5, 3)),
+                lambda: _arg(a, "xyz", np.float32, (6, 3)),
+                lambda: _arg(a[:, ::-1], "xyz", np.float32, (5, 3)),
+                lambda: _arg(a, "xyz", np.float32, (5, 3), device=0),
+                lambda: _arg(None, "xyz", np.float32, (5, 3))):
+        with pytest.raises(apx.ApxError) as ei:
+            bad()
+        assert ei.value.status == apx.APX_EINVAL

@@ -58,7 +58,8 @@ def test_empty_cloud_and_no_centres(flags):
 @pytest.mark.parametrize("flags", PATHS)
 def test_dense_roi_overflows_mma_ion_buffer(flags):
     """Noiseless full-density fcc Al, R = 2.2 nm: ~2700 ions per ROI > the MMA kernel's shared ion buffer at
-    B = 1024, so the auto path defers these material points to the FFT kernel."""
+    B = 1024 (1152 ions), so on the auto path these ROIs spill into the second histogram buffer, run single-buffered
+    and are binned in two passes of <= 2048 ions."""
     xyz, types = _ball(3.0)
     dirs = O.dirs_fibonacci(200)
     centres = np.array([[0, 0, 0], [0.3, -0.2, 0.1], [2.5, 0, 0]], np.float32)    # the last one is a partial ROI
@@ -114,8 +115,9 @@ def test_pad0_and_non_unit_directions_clamp(flags, B):
     _check(w, dirs, centres, (5, 20), flags, pad=1)
 
 
-def test_run_host_matches_device_path():
-    """apx_run_host (host pointers, slabbed and pipelined copies) returns exactly what apx_run leaves on the device."""
+def test_run_host_against_oracle_and_device_path():
+    """apx_run_host (host pointers, ring of two staging slabs, pipelined copies): every output element against the
+    ORACLE, and bit for bit what apx_run leaves on the device."""
     import torch
     xyz, types = _ball(2.4, eta=0.5, sigma=0.05, seed=17)
     rng = np.random.default_rng(3)
@@ -127,13 +129,83 @@ def test_run_host_matches_device_path():
     cnt_d = torch.empty(301, dtype=torch.int32, device=dev)
     plan.apx_run(torch.from_numpy(xyz).to(dev), torch.from_numpy(types).to(dev), torch.from_numpy(centres).to(dev), sig_d, cnt_d)
     torch.cuda.synchronize()
-    sig_h = torch.empty((301, 96, 2), dtype=torch.float32).pin_memory()
-    cnt_h = torch.empty(301, dtype=torch.int32).pin_memory()
+    sig_h = torch.full((301, 96, 2), -7.0, dtype=torch.float32).pin_memory()
+    cnt_h = torch.full((301,), -1, dtype=torch.int32).pin_memory()
     plan.apx_run_host(torch.from_numpy(xyz), torch.from_numpy(types), torch.from_numpy(centres), sig_h, cnt_h)
     assert torch.equal(sig_h, sig_d.cpu()) and torch.equal(cnt_h, cnt_d.cpu())
-    ref, rc = O.signatures(xyz, types, centres[:5], dirs, 1.0, 256, k_lo=7, k_hi=17)
-    assert (cnt_h[:5].numpy().astype(np.uint32) == rc).all()
+    ref, rc, win = O.signatures(xyz, types, centres, dirs, 1.0, 256, k_lo=7, k_hi=17, want_window=True)
+    assert_parity(sig_h.numpy(), cnt_h.numpy().astype(np.uint32), ref, rc, win, 7)
+    # pageable numpy buffers, no counts, no types: same numbers
+    sig_n = np.full((301, 96, 2), -7.0, np.float32)
+    plan.apx_run_host(xyz, None, centres, sig_n, None)
+    assert np.array_equal(sig_n, sig_h.numpy())
     plan.apx_plan_destroy()
+
+
+def test_run_host_ring_reuses_two_slabs():
+    """More slabs than staging buffers: D = 40 962 directions make a material point 328 KB, so 20 000 points are 6.5 GB of
+    signatures = 7 slabs of <= 1 GiB through the two device staging buffers; sampled against the oracle."""
+    import torch
+    xyz, types = _ball(3.2, eta=0.3, sigma=0.05, seed=23)
+    rng = np.random.default_rng(9)
+    M = 20000
+    centres = ((rng.random((M, 3)) - 0.5) * 3.0).astype(np.float32)
+    dirs = O.dirs_geodesic(6)
+    plan = apx.Plan(1.0, 256, dirs, k_lo=7, k_hi=17, device=0)
+    sig_h = torch.full((M, len(dirs), 2), -7.0, dtype=torch.float32)
+    cnt_h = torch.full((M,), -1, dtype=torch.int32)
+    free0 = torch.cuda.mem_get_info()[0]
+    plan.apx_run_host(xyz, types, centres, sig_h.numpy(), cnt_h.numpy())
+    assert free0 - torch.cuda.mem_get_info()[0] < (3 << 30)              # two 1 GiB slabs, not 6.5 GB, live on the device
+    idx = np.array([0, 3276, 3277, 6553, 9999, 13107, 16383, 19660, M - 1])       # around the slab seams
+    ref, rc, win = O.signatures(xyz, types, centres[idx], dirs, 1.0, 256, k_lo=7, k_hi=17, want_window=True)
+    assert_parity(sig_h.numpy()[idx], cnt_h.numpy().astype(np.uint32)[idx], ref, rc, win, 7)
+    assert bool((sig_h[..., 1] >= 7).all())                               # nothing left unwritten
+    plan.apx_plan_destroy()
+
+
+def _hist_check(plan, w, dirs, centre, d0, nd, accepted=None, pad=1):
+    import torch
+    out = torch.full((nd, w.B), -1, dtype=torch.int32, device="cuda")
+    plan.apx_debug_histograms(centre, d0, nd, out)
+    torch.cuda.synchronize()
+    ref, n = O.histograms(w.xyz, w.types, np.asarray(centre, np.float32), dirs, w.R, w.B, pad=pad, accepted=accepted, d0=d0, nd=nd)
+    got = out.cpu().numpy().astype(np.uint32)
+    assert (got == ref).all(), np.argwhere(got != ref)[:4]
+    return n
+
+
+@pytest.mark.parametrize("flags", PATHS)
+def test_histograms_bit_exact_multipass_spill_deferred(flags):
+    """The production kernels' histograms (export of apx_debug_histograms) against the oracle on the ROI sizes that take
+    the special routes: B = 256 two-pass (> 2048 ions, partial counts added), B = 1024 spilled into the second buffer
+    (1152 < n), B = 1024 beyond 8192 ions (deferred to the FFT kernel / streaming), B = 2048 two-pass single-buffered."""
+    import torch
+    xyz, types = _ball(4.0)
+    X, T = torch.from_numpy(xyz).cuda(), torch.from_numpy(types).cuda()
+    for R, B, window, lo in ((2.2, 256, window_for(2.2, 256), 2049), (2.2, 1024, window_for(2.2, 1024), 2049),
+                             (3.3, 1024, (20, 39), 8193), (2.2, 2048, (23, 51), 2049)):
+        dirs = O.dirs_fibonacci(200)
+        w = _case(xyz, types, R, B)
+        plan = apx.Plan(R, B, dirs, k_lo=window[0], k_hi=window[1], device=0, flags=flags)
+        plan.apx_ingest(X, T)
+        for c in ((0.0, 0.0, 0.0), (0.3, -0.2, 0.1)):
+            n = _hist_check(plan, w, dirs, c, 3, 197)
+            assert n >= lo
+        plan.apx_plan_destroy()
+
+
+@pytest.mark.parametrize("flags", PATHS)
+def test_histograms_bit_exact_pad0_clamp(flags):
+    xyz, types = _ball(1.6, eta=0.7, sigma=0.03, seed=13)
+    dirs = (O.dirs_fibonacci(64).astype(np.float64) * 1.03).astype(np.float32)
+    import torch
+    for B in (512, 2048):
+        w = _case(xyz, types, 1.2, B)
+        plan = apx.Plan(1.2, B, dirs, pad=0, k_lo=5, k_hi=20, device=0, flags=flags)
+        plan.apx_ingest(torch.from_numpy(xyz).cuda(), torch.from_numpy(types).cuda())
+        _hist_check(plan, w, dirs, (0.0, 0.0, 0.0), 0, 64, pad=0)
+        plan.apx_plan_destroy()
 
 
 @pytest.mark.parametrize("B", [1024, 2048])
@@ -168,6 +240,12 @@ def test_half_grid_mode_with_exact_integer_projections(flags, centre_ions, B):
     assert plan.apx_plan_path() == 1 and plan.apx_plan_paired() == (0 if flags else 1)
     _, s, _ = plan.apx_plan_constants()
     assert s == B / 4
+    # bit-exact histograms of every direction: mirrored ones (reversed), flagged pairs (binned again on their own in the
+    # fix-up groups) and, with an ion on the centre, the fix-list overflow that sends the point to the FFT kernel
+    import torch
+    plan.apx_ingest(torch.from_numpy(w.xyz).cuda(), torch.from_numpy(w.types).cuda())
+    for c in centres:
+        _hist_check(plan, w, dirs, c, 0, len(dirs))
     plan.apx_plan_destroy()
     _check(w, dirs, centres, (15, 34), flags)
 
@@ -195,3 +273,71 @@ def test_b2048_tensor_path_multipass_and_deferred(flags):
     w = _case(xyz, types, 2.7, 2048)
     path, cnt = _check(w, dirs, centres[:2], window_for(2.7, 2048), flags)
     assert path == 1 and cnt.min() > 4096
+
+
+def test_large_roi_deferred_from_tensor_path_b1024():
+    """B = 1024 on the auto path: more than 8192 ions exceed even the spill mode of the tensor-core kernel, the material
+    point goes to the deferred list and the general kernel (streaming its cell rows) serves it in the same stream."""
+    xyz, types = _ball(4.0)
+    dirs = O.dirs_fibonacci(64)
+    centres = np.array([[0, 0, 0], [3.9, 0, 0]], np.float32)             # the second one is a partial ROI on the tensor path
+    w = _case(xyz, types, 3.3, 1024)
+    path, cnt = _check(w, dirs, centres, (20, 39), 0)
+    assert path == 1 and cnt[0] > 8192 and cnt[1] < 8192
+
+
+def test_multipass_roi_run_to_run():
+    """A ROI with more than 2048 ions is binned in passes of 2048 whose partial spectra accumulate in fp32 (TMEM).  Which
+    ions fall into which pass depends on the order the counting sort's atomics and the gather's warp appends happen to
+    take, so the last bits of the amplitude may differ from run to run.  Bound it: counts and peak
+    bins identical (up to oracle-level ties), amplitudes within 4 fp32 ulps of N_c; single-pass ROIs are bit-identical."""
+    import torch
+    xyz, types = _ball(3.0)
+    dirs = O.dirs_fibonacci(512)
+    dev = torch.device("cuda:0")
+    centres = torch.tensor([[0.0, 0.0, 0.0], [0.3, -0.2, 0.1], [2.6, 0.0, 0.0]], dtype=torch.float32, device=dev)
+    plan = apx.Plan(2.2, 256, dirs, k_lo=12, k_hi=40, device=0)
+    runs = []
+    for _ in range(3):
+        sig = torch.empty((3, 512, 2), dtype=torch.float32, device=dev)
+        cnt = torch.empty(3, dtype=torch.int32, device=dev)
+        plan.apx_run(torch.from_numpy(xyz).to(dev), torch.from_numpy(types).to(dev), centres, sig, cnt)
+        torch.cuda.synchronize()
+        runs.append((sig.cpu().numpy(), cnt.cpu().numpy()))
+    n = runs[0][1].astype(np.float64)
+    assert n[0] > 2048 and n[2] <= 2048
+    for s, c in runs[1:]:
+        assert (c == runs[0][1]).all()
+        assert np.array_equal(s[2], runs[0][0][2])                              # single pass: bit-identical
+        assert (np.abs(s[..., 0] - runs[0][0][..., 0]) <= 4 * 2.0 ** -23 * n[:, None]).all()
+        assert (s[..., 1] == runs[0][0][..., 1]).mean() > 0.999
+    plan.apx_plan_destroy()
+
+
+def test_binding_rejects_wrong_dtype_shape_device():
+    """The Python binding checks dtype, shape, contiguity and placement of every array before a raw pointer crosses the ABI."""
+    import torch
+    dev = torch.device("cuda:0")
+    dirs = O.dirs_fibonacci(32)
+    plan = apx.Plan(1.0, 256, dirs, k_lo=7, k_hi=17, device=0)
+    xyz = torch.zeros((10, 3), dtype=torch.float32, device=dev)
+    types = torch.zeros(10, dtype=torch.uint8, device=dev)
+    centres = torch.zeros((2, 3), dtype=torch.float32, device=dev)
+    sig = torch.zeros((2, 32, 2), dtype=torch.float32, device=dev)
+    bad = [
+        lambda: plan.apx_ingest(xyz.double(), types),                           # float64 coordinates
+        lambda: plan.apx_ingest(xyz, types[:5]),                                # too few types
+        lambda: plan.apx_ingest(xyz.cpu(), types),                              # host tensor where a device tensor is due
+        lambda: plan.apx_ingest(xyz.t().contiguous().t(), types),               # not contiguous
+        lambda: plan.apx_run(xyz, types, centres, sig[:1]),                     # signature buffer too small
+        lambda: plan.apx_run(xyz, types, centres, sig, torch.zeros(1, dtype=torch.int32, device=dev)),   # counts too small
+        lambda: plan.apx_run(xyz, types, centres, sig.half()),                  # wrong output dtype
+        lambda: plan.apx_run_host(xyz, types, centres, sig),                    # device tensors into the host entry
+    ]
+    for f in bad:
+        with pytest.raises(apx.ApxError) as ei:
+            f()
+        assert ei.value.status == apx.APX_EINVAL
+    plan.apx_run(xyz, types, centres, sig)                                       # the well-formed call still works
+    torch.cuda.synchronize()
+    plan.apx_plan_destroy()

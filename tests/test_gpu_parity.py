@@ -1,5 +1,7 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
 same seeded inputs.  Run with -m gpu on a B200."""
+import functools
+
 import numpy as np
 import pytest
 
@@ -33,7 +35,7 @@ def test_cfg1_exhaustive(flags, window):
 
 @pytest.mark.parametrize("flags", PATHS)
 def test_cfg2_sampled_points_all_directions(flags):
-    w = make_config(2)
+    w = _config(2)
     dirs = O.dirs_fibonacci(w.D)
     idx = np.array([0, 9, 99, 455, 500, 555, 901, 999])       # corners, faces, interior
     got, cnt, path = run_gpu(apx, w, dirs, w.centres[idx], window=w.window, flags=flags, split=True)
@@ -50,18 +52,55 @@ def test_cfg2_full_window_sample():
     assert_parity(got, cnt, ref, rc, rwin, klo)
 
 
-def test_histograms_bit_exact_cfg2():
+@functools.lru_cache(maxsize=2)
+def _config(cfg):
+    return make_config(cfg)
+
+
+def _dirs_for(w):
+    return O.dirs_geodesic(w.grid[1]) if w.grid[0] == "geodesic" else O.dirs_fibonacci(w.D)
+
+
+def _hist_points(w, cfg, n=8):
+    """Seeded material points for the histogram check: first / last centre (box corners), one off-grid point on a box
+    face, and for config 3 the two grid planes next to the phase boundary."""
+    M = len(w.centres)
+    rng = np.random.default_rng(100 + cfg)
+    pts = [w.centres[0], w.centres[M - 1]] if M > 1 else [w.centres[0]]
+    if cfg == 3:
+        g = w.centres.reshape(30, 30, 30, 3)
+        pts += [g[14, 11, 7], g[15, 11, 7]]
+    if M > 1:
+        hi = w.centres.max(0)
+        pts.append(np.array([hi[0] + 0.45, 0.5 * hi[1], 0.31 * hi[2]], np.float32))
+        pts += [w.centres[i] for i in rng.choice(M, n - len(pts), replace=False)]
+    return pts
+
+
+@pytest.mark.parametrize("flags", PATHS)
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_histograms_bit_exact_production_kernels(cfg, flags):
+    """north_star: histogram counts bit-exact.  apx_debug_histograms runs the plan's PRODUCTION kernel
+    (k_signature_mma incl. half-grid mirroring / fix-ups, or k_signature_fft) with its export switched on: the
+    shared-memory histogram the DFT reads, against the oracle's Eq. 1, 8 material points x 512 directions per config."""
     import torch
-    w = make_config(2)
-    dirs = O.dirs_fibonacci(w.D)
-    plan = apx.Plan(w.R, w.B, dirs, device=0)
+    w = _config(cfg)
+    dirs = _dirs_for(w)
+    accepted = {0} if cfg in (3, 5) else None
+    plan = apx.Plan(w.R, w.B, dirs, k_lo=w.window[0], k_hi=w.window[1], accepted_types=accepted, device=0, flags=flags)
+    if flags == 0:
+        assert plan.apx_plan_path() == 1 and plan.apx_plan_paired() == (1 if w.grid[0] == "geodesic" else 0)
     plan.apx_ingest(torch.from_numpy(w.xyz).cuda(), torch.from_numpy(w.types).cuda())
-    for c in (w.centres[555], w.centres[0], np.array([19.5, 10.0, 0.3], np.float32)):
-        out = torch.empty((512, w.B), dtype=torch.int32, device="cuda")
-        plan.apx_debug_histograms(c, 1000, 512, out)
+    nd = min(512, len(dirs))
+    for j, c in enumerate(_hist_points(w, cfg)):
+        d0 = (j * 4999) % (len(dirs) - nd + 1)
+        out = torch.full((nd, w.B), -1, dtype=torch.int32, device="cuda")
+        plan.apx_debug_histograms(c, d0, nd, out)
         torch.cuda.synchronize()
-        ref, n = O.histograms(w.xyz, w.types, c, dirs, w.R, w.B, d0=1000, nd=512)
-        assert (out.cpu().numpy().astype(np.uint32) == ref).all()
+        ref, n = O.histograms(w.xyz, w.types, c, dirs, w.R, w.B, accepted=accepted, d0=d0, nd=nd)
+        got = out.cpu().numpy().astype(np.uint32)
+        assert (got.sum(1) == n).all(), f"cfg {cfg} point {j}: histogram totals differ from N_c = {n}"
+        assert (got == ref).all(), f"cfg {cfg} point {j}: {np.argwhere(got != ref)[:4]}"
     plan.apx_plan_destroy()
 
 
@@ -97,11 +136,14 @@ def test_cfg4_sample(flags):
     assert_parity(got, cnt, ref, rc, rwin, klo)
 
 
-def _full_launch(w, dirs, accepted=None):
+def _full_launch(w, dirs, accepted=None, expect_paired=None):
     """The whole config in ONE apx_run (the launch configuration bench.py times); results stay on the device."""
     import torch
     dev = torch.device("cuda:0")
     plan = apx.Plan(w.R, w.B, dirs, k_lo=w.window[0], k_hi=w.window[1], accepted_types=accepted, device=0)
+    assert plan.apx_plan_path() == 1
+    if expect_paired is not None:
+        assert plan.apx_plan_paired() == expect_paired            # half-grid mode is what runs on the geodesic grid
     xyz = torch.from_numpy(w.xyz).to(dev)
     types = torch.from_numpy(w.types).to(dev)
     c = torch.from_numpy(w.centres).to(dev)
@@ -116,58 +158,78 @@ def _full_launch(w, dirs, accepted=None):
 
 def _check_full(w, dirs, sig, counts, idx, accepted=None, count_all=True):
     import torch
-    M = len(w.centres)
     cnt = counts.cpu().numpy().astype(np.uint32)
-    if count_all:
-        # every material point: ROI ion count against the oracle's brute force (one direction is enough for counts)
-        _, rc_all = O.signatures(w.xyz, w.types, w.centres, dirs[:1], w.R, w.B, k_lo=w.window[0], k_hi=w.window[1],
-                                 accepted=accepted)
-        assert (cnt == rc_all).all()
+    # ROI ion counts against the oracle's brute force (one direction is enough for counts): every material point, or
+    # -- where N x M makes that take the oracle an hour -- a seeded sample of 2048
+    cidx = np.arange(len(cnt)) if count_all else np.sort(np.random.default_rng(len(cnt)).choice(len(cnt), 2048, replace=False))
+    _, rc_all = O.signatures(w.xyz, w.types, w.centres[cidx], dirs[:1], w.R, w.B, k_lo=w.window[0], k_hi=w.window[1],
+                             accepted=accepted)
+    assert (cnt[cidx] == rc_all).all()
     # properties that hold for every output: 0 <= A <= N_c (P4), k inside the window, nothing left unwritten
-    amp, k = sig[..., 0], sig[..., 1]
-    assert bool((amp >= 0).all()) and bool((amp <= counts.to(torch.float32)[:, None] * (1 + 1e-5) + 1e-3).all())
-    assert bool((k >= w.window[0]).all()) and bool((k <= w.window[1]).all())
+    ok = torch.ones((), dtype=torch.bool, device=sig.device)
+    for m0 in range(0, sig.shape[0], 8192):                                  # in slabs: no 57 GB temporaries
+        blk, cb = sig[m0:m0 + 8192], counts[m0:m0 + 8192].to(torch.float32)[:, None]
+        amp, k = blk[..., 0], blk[..., 1]
+        ok &= (amp >= 0).all() & (amp <= cb * (1 + 1e-5) + 1e-3).all() & (k >= w.window[0]).all() & (k <= w.window[1]).all()
+    assert bool(ok)
     # sampled material points x all directions, element by element
+    idx = np.unique(np.asarray(idx))
     got = sig[torch.from_numpy(idx).cuda()].cpu().numpy()
     ref, rc, rwin = O.signatures(w.xyz, w.types, w.centres[idx], dirs, w.R, w.B, k_lo=w.window[0], k_hi=w.window[1],
                                  accepted=accepted, want_window=True)
     assert_parity(got, cnt[idx], ref, rc, rwin, w.window[0])
 
 
+def _sample64(M, seed, extra=()):
+    """64 seeded material points (SURVEY 8(c) parity protocol): the given special points plus random ones."""
+    rng = np.random.default_rng(seed)
+    extra = [int(e) for e in extra]
+    return np.unique(np.concatenate([extra, rng.choice(M, 64 - len(extra), replace=False)]).astype(np.int64))
+
+
 def test_cfg2_full_size_bench_launch():
-    w = make_config(2)
+    w = _config(2)
     dirs = O.dirs_fibonacci(w.D)
-    sig, counts = _full_launch(w, dirs)
+    sig, counts = _full_launch(w, dirs, expect_paired=0)
     _check_full(w, dirs, sig, counts, np.array([0, 99, 137, 455, 500, 555, 900, 999]))
 
 
-def test_cfg3_full_size_al_filter():
-    """Config 3 at full size (27 000 material points x 40 962 geodesic directions, 8.85 GB of signatures), Al filter."""
-    w = make_config(3)
+@pytest.mark.parametrize("mask", [{0}, {1}], ids=["Al", "W"])
+def test_cfg3_full_size_per_phase_filter(mask):
+    """Config 3 at full size (27 000 material points x 40 962 geodesic directions, 8.85 GB of signatures), one run per
+    phase filter; 64 sampled points include the box corners / faces and both grid planes next to the phase plane."""
+    w = _config(3)
     dirs = O.dirs_geodesic(6)
-    sig, counts = _full_launch(w, dirs, accepted={0})
+    sig, counts = _full_launch(w, dirs, accepted=mask, expect_paired=1)
     g = np.arange(27000).reshape(30, 30, 30)
-    idx = np.array([g[14, 10, 10], g[15, 10, 10], g[0, 0, 0], g[29, 15, 3], g[3, 20, 20], g[7, 7, 29]])
-    _check_full(w, dirs, sig, counts, idx, accepted={0})
+    special = [g[14, 10, 10], g[15, 10, 10], g[14, 0, 29], g[15, 29, 0], g[0, 0, 0], g[29, 29, 29], g[29, 15, 3],
+               g[3, 20, 20], g[7, 7, 29], g[13, 13, 13], g[16, 16, 16]]
+    _check_full(w, dirs, sig, counts, _sample64(27000, 3, special), accepted=mask)
 
 
 def test_cfg4_full_size():
     """Config 4 at full size (175 616 material points x 40 962 directions, 57.5 GB of signatures, half-grid mode):
-    properties on every output, sampled material points x all directions element by element (the brute-force count
-    of every ROI would take the oracle minutes, so counts are checked on the sample)."""
-    w = make_config(4)
+    properties on every output, ROI counts of 2048 sampled material points against the oracle's brute force, 64 sampled
+    material points x all directions element by element (box corners / faces and the points nearest to grain
+    boundaries -- smallest gap between the two nearest Voronoi seeds -- included)."""
+    w = _config(4)
     dirs = O.dirs_geodesic(6)
-    sig, counts = _full_launch(w, dirs)
-    rng = np.random.default_rng(4)
-    idx = np.sort(np.concatenate([[0, len(w.centres) - 1], rng.choice(len(w.centres), 10, replace=False)]))
-    _check_full(w, dirs, sig, counts, idx, count_all=False)
+    sig, counts = _full_launch(w, dirs, expect_paired=1)
+    M = len(w.centres)
+    seeds = w.meta["seeds"]
+    dist = np.sort(np.linalg.norm(w.centres[:, None, :].astype(np.float64) - seeds[None], axis=2), axis=1)
+    gb = np.argsort(dist[:, 1] - dist[:, 0])[:12]                           # on grain boundaries
+    g = np.arange(M).reshape(56, 56, 56)
+    special = [0, M - 1, g[0, 28, 28], g[55, 0, 31], g[28, 55, 55], *gb]
+    _check_full(w, dirs, sig, counts, _sample64(M, 4, special), count_all=False)
 
 
 def test_cfg5_full_size_al_filter():
     """Config 5 at full size (64 000 x 40 962, B = 2048, Al filter) on the tensor-core kernel in half-grid mode."""
-    w = make_config(5)
+    w = _config(5)
     dirs = O.dirs_geodesic(6)
-    sig, counts = _full_launch(w, dirs, accepted={0})
-    rng = np.random.default_rng(5)
-    idx = np.sort(np.concatenate([[0, len(w.centres) - 1], rng.choice(len(w.centres), 6, replace=False)]))
-    _check_full(w, dirs, sig, counts, idx, accepted={0}, count_all=False)
+    sig, counts = _full_launch(w, dirs, accepted={0}, expect_paired=1)
+    M = len(w.centres)
+    g = np.arange(M).reshape(40, 40, 40)
+    special = [0, M - 1, g[0, 20, 20], g[39, 0, 17], g[20, 39, 39], g[20, 20, 20]]
+    _check_full(w, dirs, sig, counts, _sample64(M, 5, special), accepted={0}, count_all=False)

@@ -1,6 +1,7 @@
-"""N > 1 path on CPU: world_size-2 gloo processes shard the material points exactly as bench.py / run_sharded do,
-each rank computes its slab (with the oracle standing in for the GPU here) and the gathered result must equal the
-single-rank result.  No collective touches the signature data itself."""
+"""N > 1 path on CPU: world_size-2 gloo processes run parallel.run_sharded -- the very function bench.py --gpus N calls --
+on a stand-in plan object whose apx_run is served by the oracle (there is no GPU here): each rank computes its slab of
+the centre list and the gathered result must equal the single-rank result.  No collective touches the signature data
+itself."""
 import os
 import socket
 import numpy as np
@@ -9,7 +10,7 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_2009_00735_b200.parallel import shard_range, gather_counts
+from paper_2009_00735_b200.parallel import shard_range, gather_counts, run_sharded
 
 
 def test_shard_range_partitions():
@@ -30,6 +31,23 @@ def _free_port():
         return s.getsockname()[1]
 
 
+class _OraclePlan:
+    """Stands in for binding.Plan on a box without a GPU: same apx_run signature, CPU tensors, the oracle inside.
+    Records what run_sharded handed it."""
+
+    def __init__(self, w, dirs):
+        self.w, self.dirs, self.calls = w, dirs, []
+
+    def apx_run(self, xyz, types, centres, sig, counts=None, stream=None):
+        from oracle import oracle as O
+        self.calls.append(tuple(centres.shape))
+        s, c = O.signatures(xyz.numpy(), types.numpy(), centres.numpy(), self.dirs, self.w.R, self.w.B,
+                            k_lo=self.w.window[0], k_hi=self.w.window[1])
+        sig.copy_(torch.from_numpy(s))
+        if counts is not None:
+            counts.copy_(torch.from_numpy(c.astype(np.int64)))
+
+
 def _worker(rank, world, port, q):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     dist.init_process_group("gloo", rank=rank, world_size=world)
@@ -39,9 +57,15 @@ def _worker(rank, world, port, q):
     rng = np.random.default_rng(5)
     centres = (rng.random((7, 3)) - 0.5).astype(np.float32)          # 7 material points over 2 ranks: 4 + 3
     dirs = O.dirs_fibonacci(64)
-    b, e = shard_range(len(centres), rank, world)
-    sig, cnt = O.signatures(w.xyz, w.types, centres[b:e], dirs, w.R, w.B, k_lo=w.window[0], k_hi=w.window[1])
-    allc = gather_counts(torch.from_numpy(cnt.astype(np.int64)), len(centres), rank, world)
+    b0, e0 = shard_range(len(centres), rank, world)
+    plan = _OraclePlan(w, dirs)
+    sig_t = torch.full((e0 - b0, len(dirs), 2), -7.0)
+    cnt_t = torch.full((e0 - b0,), -1, dtype=torch.int64)
+    b, e = run_sharded(plan, torch.from_numpy(w.xyz), torch.from_numpy(w.types), torch.from_numpy(centres), sig_t, cnt_t,
+                       rank=rank, world=world)
+    assert (b, e) == (b0, e0) and plan.calls == [(e0 - b0, 3)]        # one apx_run on exactly this rank's slab
+    sig = sig_t.numpy()
+    allc = gather_counts(cnt_t, len(centres), rank, world)
     # signatures stay sharded; for the check only, rank 0 collects them as python objects
     parts = [None] * world
     dist.all_gather_object(parts, (b, e, sig))

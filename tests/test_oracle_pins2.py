@@ -150,3 +150,59 @@ def test_fibonacci_grid_pins():
     np.testing.assert_allclose(np.diff(ang) % (2 * math.pi), (math.pi * (3 - math.sqrt(5))) % (2 * math.pi),
                                atol=1e-4)
     assert abs(f.mean(axis=0)).max() < 2e-3                                           # balanced
+
+
+# ---- single-rounded fma order of the projection (reading #15) ---------------------
+def _rn32(fr):
+    """Fraction -> nearest binary32 (ties to even), exact integer arithmetic; normal range only."""
+    from fractions import Fraction
+    if fr == 0:
+        return Fraction(0)
+    sgn, a = (1 if fr > 0 else -1), abs(fr)
+    e = 0
+    while a >= 2 ** 24:
+        a /= 2; e += 1
+    while a < 2 ** 23:
+        a *= 2; e -= 1
+    q, r = divmod(a.numerator, a.denominator)
+    twice = 2 * r
+    if twice > a.denominator or (twice == a.denominator and (q & 1)):
+        q += 1
+    return sgn * Fraction(q) * (Fraction(2) ** e)
+
+
+def test_projection_uses_single_rounded_fma_not_mul_add():
+    """Eq. 1 in the contract's operation order: x = fma(n'z, dz, fma(n'y, dy, n'x*dx)), every fma ONE rounding.
+    An oracle built with two-rounding a*b+c passes every pin whose inputs are dyadic; here (ion, direction) pairs are
+    searched (seeded) whose bin differs between the two evaluation orders, in exact rational arithmetic, and the
+    oracle must land on the fma bin for every one of them."""
+    from fractions import Fraction
+    rng = _rng(77)
+    B, R = 1024, 2.0
+    R2, s = O.constants(R, B, pad=1)
+    found = 0
+    for _ in range(400000):
+        if found >= 6:
+            break
+        d = rng.standard_normal(3)
+        d /= np.linalg.norm(d)
+        n32 = d.astype(np.float32)
+        npr = (n32 * np.float32(s)).astype(np.float32)                  # one fp32 multiply each (exact in numpy float32)
+        # an ion whose projection sits within ~1e-5 of an integer: start from a random point and move it along n
+        p = rng.uniform(-1.0, 1.0, 3)
+        t = float(np.dot(npr.astype(np.float64), p))
+        p = p + d * ((round(t) - t + rng.uniform(-3e-5, 3e-5)) / float(s))
+        p32 = p.astype(np.float32)
+        if float(np.dot(p32.astype(np.float64), p32.astype(np.float64))) > 3.9:
+            continue
+        F = [Fraction(float(v)) for v in npr]
+        Dv = [Fraction(float(v)) for v in p32]                          # centre = origin: d = p exactly
+        x_fma = _rn32(F[2] * Dv[2] + _rn32(F[1] * Dv[1] + _rn32(F[0] * Dv[0])))
+        x_two = _rn32(_rn32(F[2] * Dv[2]) + _rn32(_rn32(F[1] * Dv[1]) + _rn32(F[0] * Dv[0])))
+        b_fma, b_two = B // 2 + math.floor(x_fma), B // 2 + math.floor(x_two)
+        if b_fma == b_two:
+            continue
+        found += 1
+        h, n = O.histograms(p32[None, :], None, np.zeros(3, np.float32), n32[None, :], R, B)
+        assert n == 1 and h[0, b_fma] == 1 and h[0, b_two] == 0, (b_fma, b_two, np.nonzero(h[0]))
+    assert found >= 3, "search did not find pairs that separate fma from mul+add"

@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_peak(int iters, float seed, flo
                 if (TEST == APX_PEAK_LDS32_BROADCAST || TEST == APX_PEAK_LDS32_CONFLICT_FREE) {
                     const uint32_t off = TEST == APX_PEAK_LDS32_BROADCAST ? row : row + (uint32_t)lane * 4u;
                     float v;
-                    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(wbase + off));
+                    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(wbase + off) : "memory");
                     acc += v;
                 } else {
                     uint32_t off;
@@ -103,7 +103,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_peak(int iters, float seed, flo
                     else if (TEST == APX_PEAK_LDS128_BROADCAST_4) off = row + (uint32_t)(lane >> 3) * 16u;     // four (quarter-warps)
                     else off = (uint32_t)(u % 3) * 512u + (uint32_t)lane * 16u;                          // 512 B per instruction
                     float x, y, z, w;
-                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(wbase + off));
+                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(wbase + off) : "memory");
                     acc += x + y + z + w;
                 }
             }

@@ -245,6 +245,96 @@ def run_ingest(args):
     plan.apx_plan_destroy()
 
 
+def _time_steps(torch, fn, steps, warmup, flush):
+    for _ in range(max(warmup, 3)):
+        fn()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in ev:
+        flush.fill_(1)
+        a.record(); fn(); b.record()
+    torch.cuda.synchronize()
+    return sum(a.elapsed_time(b) for a, b in ev) / steps
+
+
+def run_index(args):
+    """--index: Eq. 3 -- M synthetic normalised images on the paper's 40 962-node mesh against every
+    orientation of the stand-in orientation set, N_hat = 1000 strongest nodes (L369, L416).  L2-bound gather: algorithmic
+    traffic = 4 B (one fp32 image value) per (material point, orientation, node) triple."""
+    import torch
+    import paper_2009_00735_b200 as apx
+    dev = torch.device("cuda:0")
+    rng = np.random.Generator(np.random.PCG64(200900735 + 11))
+    dirs = apx.apx_dirs_geodesic(6)
+    G = apx.apx_so3_grid_cubic(args.index_spacing)
+    D, Ng, n_hat, M, K = len(dirs), len(G), 1000, args.index_points, 4
+    # reference: smooth image with <100> poles; measured: the same rotated by random grid orientations + noise
+    ref = np.exp(-(1.0 - np.max(np.abs(dirs), axis=1)) / 0.01).astype(np.float32)
+    t0 = time.perf_counter()
+    ix = apx.Indexer(dirs, G, ref, n_hat, device=0)
+    t_pre = time.perf_counter() - t0
+    sig = torch.zeros((M, D, 2), dtype=torch.float32, device=dev)
+    sig[..., 0] = torch.from_numpy(rng.random((M, D), dtype=np.float32)).to(dev)
+    bd = torch.empty((M, K), dtype=torch.float32, device=dev)
+    bg = torch.empty((M, K), dtype=torch.int32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ms = _time_steps(torch, lambda: ix.apx_index(sig, None, bd, bg), args.steps, args.warmup, flush)
+    gathers = float(M) * Ng * n_hat
+    try:
+        lts = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except Exception:
+        lts = 6550.0
+    # L2 ceiling: ~6300 B/clk full chip (B200_PROFILING.md "LTS throughput cap") at the maximum SM clock
+    l2_peak = 6300.0 * SM_MAX_GHZ
+    achieved = gathers * 4.0 / (ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "indexed (material point, orientation) pairs/s", "value": float(M) * Ng / (ms * 1e-3),
+                      "unit": "pairs/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms,
+                      "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": f"indexing: {M} images x {Ng} orientations ({args.index_spacing} deg Rodrigues grid, m-3m) x "
+                                             f"{n_hat} strongest nodes of {D} (geodesic level 6)", "K": K,
+                                 "preprocessing_s": t_pre, "l2": "flushed between timed steps"},
+                      "gpu_launches": 3 * args.steps * ((M + 8191) // 8192),
+                      "roofline": {"bound": "l2", "kernel": "k_index", "achieved": achieved, "peak": l2_peak, "unit": "GB/s",
+                                   "frac": achieved / l2_peak, "traffic": None,
+                                   "peak_source": "B200_PROFILING.md LTS throughput cap ~6300 B/clk x 1.965 GHz (HBM copy peak "
+                                                  f"{lts:.0f} GB/s for scale)",
+                                   "model": "4 B per (material point, orientation, node) gather; one 128-B line serves 32 material points",
+                                   "gathers_per_s": gathers / (ms * 1e-3)}}))
+    ix.apx_indexer_destroy()
+
+
+def run_fsp(args):
+    """--fsp: Eq. 2 on config 2's cloud: M ROIs x L^3 reciprocal-space points, k_max = 2 pi / nm.
+    A dense complex contraction per z-slice on the FP32 pipe: 8 flop per (ion, k point)."""
+    import torch
+    import paper_2009_00735_b200 as apx
+    from workloads import make_config
+    dev = torch.device("cuda:0")
+    w = make_config(2)
+    M, L = args.fsp_points, args.fsp_L
+    plan = apx.Plan(w.R, w.B, apx.apx_dirs_fibonacci(64), k_lo=15, k_hi=34, device=0)
+    plan.apx_ingest(torch.from_numpy(w.xyz).to(dev), torch.from_numpy(w.types).to(dev))
+    centres = torch.from_numpy(np.ascontiguousarray(w.centres[np.arange(M) % len(w.centres)])).to(dev)
+    out = torch.empty((M, L, L, L), dtype=torch.float32, device=dev)
+    cnt = torch.empty(M, dtype=torch.int32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ms = _time_steps(torch, lambda: plan.apx_fsp(centres, 2.0 * np.pi, L, out, cnt), args.steps, args.warmup, flush)
+    nw = float(cnt.cpu().numpy().astype(np.int64).sum())
+    flops = 8.0 * nw * L ** 3
+    pk = load_peaks()
+    achieved = flops / (ms * 1e-3) / 1e12
+    print(json.dumps({"metric": "FSP k-points/s", "value": float(M) * L ** 3 / (ms * 1e-3), "unit": "k-points/s", "n_gpus": 1,
+                      "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+                      "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": f"FSP (Eq. 2): {M} ROIs of config 2 (R = 2.0 nm, mean {nw / M:.0f} ions) x {L}^3 k points, "
+                                             "k_max = 2 pi / nm", "rois_per_s": M / (ms * 1e-3)},
+                      "gpu_launches": args.steps,
+                      "roofline": {"bound": "alu", "kernel": "k_fsp", "achieved": achieved, "peak": pk["fp32_tflops"],
+                                   "unit": "TFLOP/s", "frac": achieved / pk["fp32_tflops"], "traffic": None,
+                                   "peak_source": pk["source"], "model": "8 flop (one complex multiply-add) per (ion, k point)"}}))
+    plan.apx_plan_destroy()
+
+
 def host_buffer(shape, dtype, torch):
     """Pinned host tensor when the box can pin that much, else pageable (said in the line)."""
     t = torch.empty(shape, dtype=dtype)
@@ -281,6 +371,8 @@ def run_ours(args, rank, world, local_rank):
     w = make_config(cfg)
     dirs = apx.apx_dirs_geodesic(w.grid[1]) if w.grid[0] == "geodesic" else apx.apx_dirs_fibonacci(w.D)   # step a3
     accepted = accepted_for(cfg)
+    if args.points:                                            # profiling aid: a leading part of the centre list (said in the line)
+        w.centres = np.ascontiguousarray(w.centres[:args.points])
     M_all, D, B = len(w.centres), len(dirs), w.B
     # multi-GPU: strong scaling, rank r owns the contiguous slab shard_range(M, r, world) of the centre list
     # (material points are independent; ions replicated; signatures stay sharded; no collective)
@@ -349,6 +441,8 @@ def run_ours(args, rank, world, local_rank):
         Me = min(Me, M)
         frac_note = f"host memory holds {Me} of this rank's {M} material points: e2e timed on that leading part"
     e2e_steps = max(1, min(args.steps, 5 if cfg == 2 else 2))
+    if args.no_e2e:
+        Me = min(Me, 2)
     h_sig, pinned = host_buffer((Me, D, 2), torch.float32, torch)
     h_xyz = torch.from_numpy(w.xyz).pin_memory()
     h_types = torch.from_numpy(w.types).pin_memory()
@@ -414,7 +508,7 @@ def run_ours(args, rank, world, local_rank):
         "vs_baseline": None, "dtype": "f32 (DFT operands fp16 hi+lo, fp32 accumulate)" if path == "mma" else "f32",
         "data": "synthetic",
         "material_points_per_s": value / D,
-        "config": {"workload": WORKLOADS[cfg],
+        "config": {"workload": WORKLOADS[cfg] + (f" -- ONLY the first {args.points} material points (--points)" if args.points else ""),
                    "kernel_path": path, "half_grid_mode": half,
                    "l2": "flushed between timed steps (256 MiB fill, untimed)",
                    "ions": int(len(w.xyz)), "mean_ions_per_roi": nc_tot / M_tot,
@@ -474,8 +568,16 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--config", type=int, default=4, choices=[2, 3, 4, 5],
                     help="BASELINE.json config, at full size (default 4 = the largest single-GPU configuration)")
+    ap.add_argument("--points", type=int, default=0, help="profiling aid: only the first N material points of the config")
+    ap.add_argument("--no-e2e", action="store_true", help="profiling aid: skip the end-to-end leg")
     ap.add_argument("--replicas", action="store_true", help="multi-GPU: every rank runs the whole workload (weak scaling)")
     ap.add_argument("--ingest-ions", type=int, default=0, help="time step a1 (ingest) alone on this many ions")
+    ap.add_argument("--index", action="store_true", help="time the indexing step (Eq. 3, NEXT-1)")
+    ap.add_argument("--index-points", type=int, default=1024)
+    ap.add_argument("--index-spacing", type=float, default=1.0, help="orientation grid spacing in degrees")
+    ap.add_argument("--fsp", action="store_true", help="time the reciprocal space method (Eq. 2, NEXT-3)")
+    ap.add_argument("--fsp-points", type=int, default=1000)
+    ap.add_argument("--fsp-L", type=int, default=64)
     ap.add_argument("--peaks", action="store_true", help="run the on-chip peak microbenchmarks and write --peaks-out")
     ap.add_argument("--peaks-out", default=PEAKS_JSON)
     ap.add_argument("--peak-iters", type=int, default=20000)
@@ -489,6 +591,12 @@ def main():
     elif args.ingest_ions > 0:
         if rank == 0:
             run_ingest(args)
+    elif args.index:
+        if rank == 0:
+            run_index(args)
+    elif args.fsp:
+        if rank == 0:
+            run_fsp(args)
     elif args.impl == "reference":
         run_reference(args, rank, world)
     else:

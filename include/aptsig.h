@@ -38,8 +38,17 @@ typedef enum {
 #define APX_FLAG_FORCE_FFT 1   /* always use the general FFT kernel, even for a narrow window */
 #define APX_FLAG_FORCE_MMA 2   /* fail with APX_EINVAL instead of falling back when the tensor-core
                                   windowed-DFT kernel cannot serve the plan (window too wide) */
+#define APX_FLAG_NORMALISE 8   /* apx_plan_create: write A / N_c instead of A (apx_sig_spec.normalise of the one signature) */
+#define APX_FLAG_LOCAL_MAX 16  /* apx_plan_create: APX_PEAK_LOCAL_MAX for the one signature (general FFT kernel) */
 #define APX_FLAG_NO_PAIRING 4  /* tensor-core kernel: no half-grid mode even when the grid is antipodally
                                   symmetric (test hook; results are identical either way) */
+
+/* peak modes (L75 "particular bins"; L149-151 "second strongest peak") */
+#define APX_PEAK_MAX 0         /* highest amplitude of the window (default; L416 "the highest amplitude ... in the bin interval") */
+#define APX_PEAK_LOCAL_MAX 1   /* highest LOCAL maximum of the window: bin k with A_k > A_{k-1} and A_k >= A_{k+1} (A_{B/2+1} =
+                                  A_{B/2-1}); lowest k on ties; (0, k_lo) when the window has none.  The ROI-shape envelope that
+                                  dominates low bins falls monotonically and is never picked.  General FFT kernel only. */
+#define APX_MAX_SIGNATURES 4   /* signatures (apx_sig_spec) per plan */
 
 typedef struct apx_plan apx_plan; /* opaque */
 
@@ -58,9 +67,29 @@ typedef struct {
     int32_t flags;        /* APX_FLAG_*                                                                  */
 } apx_plan_desc;
 
+/* One signature of a multi-signature plan: "at least one [...] signature is computed from the positions of selected atom
+ * types in the ROI [...] multiple signatures (for different atom types) are computed per ROI" (L52); "Signatures were
+ * processed for several lattice plane families {002}, {220}, and {111}" (L208), each from "the peaks of the same bins"
+ * (L214) of the amplitude spectrum. */
+typedef struct {
+    uint8_t type_mask[32];   /* accepted ion types, as in apx_plan_desc                                              */
+    int32_t k_lo, k_hi;      /* inclusive spectral-bin window, as in apx_plan_desc (0, 0 = [1, B/2])                 */
+    int32_t peak_mode;       /* APX_PEAK_MAX or APX_PEAK_LOCAL_MAX                                                   */
+    int32_t normalise;       /* 1 = amplitudes are written as A / N_c (normalised intensity: ~1.0 for perfect
+                                crystals, L424; 0 for an empty ROI); 0 = raw |X_k|                                    */
+} apx_sig_spec;
+
 /* Plan (step a0): derived constants R2 = fl32(R*R), s = fl32((B/2-pad)/R) = 1/dR, scaled directions
  * n' = fl32(n*s), twiddle tables; owns all internal device buffers.  *out is NULL on failure. */
 int apx_plan_create(const apx_plan_desc *desc, apx_plan **out);
+/* A plan that computes n_specs (1..APX_MAX_SIGNATURES) signatures per material point from ONE ingest and ONE launch:
+ * ions are ingested once (union of the masks), specs with the same type mask share one gather, one binning pass and one
+ * transform per direction, every spec takes its peak from its own window.  desc->type_mask / k_lo / k_hi are ignored.
+ * Outputs of apx_query / apx_run / apx_run_host then hold one plane per spec, in spec order:
+ *   sig float32[n_specs][M][D][2], counts uint32[n_specs][M].
+ * Each plane equals what a single-signature plan with that mask and window produces. */
+int apx_plan_create_multi(const apx_plan_desc *desc, const apx_sig_spec *specs, int32_t n_specs, apx_plan **out);
+int apx_plan_num_signatures(const apx_plan *plan);
 int apx_plan_destroy(apx_plan *plan);
 
 /* The exact fp32 constants the kernels use (HOST out pointers, any may be NULL):

@@ -1,4 +1,5 @@
 """Build paper_2009_00735_b200/libaptsig.so in-tree with nvcc for sm_100a (cross-compiles without a GPU)."""
+from __future__ import annotations
 import glob
 import os
 import subprocess
@@ -15,11 +16,16 @@ def sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cpp")))
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, out: str | None = None) -> str:
+    if out is not None:                                            # a development variant beside the product library
+        extra = os.environ.get("APX_NVCC_FLAGS", "").split()
+        subprocess.check_call([NVCC, *FLAGS, *extra, *sources(), "-o", out])
+        return out
     deps = sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(HERE, "..", "include", "*.h"))
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
-    cmd = [NVCC, *FLAGS, *(["-Xptxas", "-v"] if verbose else []), *sources(), "-o", LIB]
+    extra = os.environ.get("APX_NVCC_FLAGS", "").split()          # development switches, e.g. -DAPX_TRACE
+    cmd = [NVCC, *FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), *sources(), "-o", LIB]
     subprocess.check_call(cmd)
     return LIB
 

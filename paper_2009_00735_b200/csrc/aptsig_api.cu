@@ -10,7 +10,6 @@
 
 using namespace apx;
 
-struct apx_plan : public apx::Plan {};
 
 #define CU(p, call)                                   \
     do {                                              \
@@ -65,7 +64,7 @@ extern "C" int apx_plan_destroy(apx_plan *p)
 {
     if (!p) return APX_OK;
     DeviceGuard guard(p->device);
-    void *bufs[] = {p->dbg_centre, p->dbg_sig, p->d_dirs_scaled, p->d_twiddle, p->d_mma_table, p->d_mma_zero, p->d_mma_phase, p->d_dirs_sorted, p->d_dir_perm, p->d_dir_perm_mirror, p->d_type_mask, p->d_grid, p->d_cell_start,
+    void *bufs[] = {p->dbg_centre, p->dbg_sig, p->d_refine_off, p->d_kaxis, p->d_dirs_scaled, p->d_twiddle, p->d_mma_table, p->d_mma_zero, p->d_mma_phase, p->d_dirs_sorted, p->d_dir_perm, p->d_dir_perm_mirror, p->d_type_mask, p->d_grid, p->d_cell_start,
                     p->d_cell_cursor, p->d_scan_tiles, p->d_cell_of_ion, p->d_sorted, p->d_deferred, p->h2d_xyz, p->h2d_types, p->h2d_centres,
                     p->d2h_sig, p->d2h_counts};
     for (void *b : bufs)
@@ -80,20 +79,42 @@ extern "C" int apx_plan_destroy(apx_plan *p)
     return APX_OK;
 }
 
-extern "C" int apx_plan_create(const apx_plan_desc *desc, apx_plan **out)
+static int create_plan(const apx_plan_desc *desc, const apx_sig_spec *specs_in, int n_specs, apx_plan **out)
 {
     if (!out) return APX_EINVAL;
     *out = nullptr;
-    if (!desc || !desc->dirs) return APX_EINVAL;
+    if (!desc || !desc->dirs || !specs_in || n_specs < 1 || n_specs > APX_MAX_SIGNATURES) return APX_EINVAL;
     const int B = desc->B;
     if (!(desc->R > 0.0f) || !std::isfinite(desc->R)) return APX_EINVAL;
     if (B < 256 || B > 4096 || (B & (B - 1))) return APX_EINVAL;
     if (desc->pad != 0 && desc->pad != 1) return APX_EINVAL;
     if (desc->D < 1) return APX_EINVAL;
-    int k_lo = desc->k_lo, k_hi = desc->k_hi;
-    if (k_lo == 0 && k_hi == 0) { k_lo = 1; k_hi = B / 2; }
-    if (k_lo < 0 || k_hi > B / 2 || k_lo > k_hi) return APX_EINVAL;
     if ((desc->flags & APX_FLAG_FORCE_FFT) && (desc->flags & APX_FLAG_FORCE_MMA)) return APX_EINVAL;
+    // specs -> classes (distinct type masks), union window, union type mask
+    SpecSet ss;
+    std::memset(&ss, 0, sizeof(ss));
+    ss.n_specs = n_specs;
+    int k_lo = B, k_hi = -1;
+    bool any_local = false;
+    uint32_t union_mask[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (int i = 0; i < n_specs; ++i) {
+        int lo = specs_in[i].k_lo, hi = specs_in[i].k_hi;
+        if (lo == 0 && hi == 0) { lo = 1; hi = B / 2; }
+        if (lo < 0 || hi > B / 2 || lo > hi) return APX_EINVAL;
+        if (specs_in[i].peak_mode != APX_PEAK_MAX && specs_in[i].peak_mode != APX_PEAK_LOCAL_MAX) return APX_EINVAL;
+        ss.k_lo[i] = lo; ss.k_hi[i] = hi; ss.mode[i] = specs_in[i].peak_mode; ss.norm[i] = specs_in[i].normalise ? 1 : 0;
+        any_local = any_local || specs_in[i].peak_mode == APX_PEAK_LOCAL_MAX;
+        k_lo = lo < k_lo ? lo : k_lo; k_hi = hi > k_hi ? hi : k_hi;
+        uint32_t m[8];
+        std::memcpy(m, specs_in[i].type_mask, 32);
+        int cls = -1;
+        for (int c = 0; c < ss.n_classes; ++c)
+            if (!std::memcmp(ss.cls_mask[c], m, 32)) cls = c;
+        if (cls < 0) { cls = ss.n_classes++; std::memcpy(ss.cls_mask[cls], m, 32); }
+        ss.cls_of[i] = cls;
+        for (int wd = 0; wd < 8; ++wd) union_mask[wd] |= m[wd];
+    }
+    if (any_local && (desc->flags & APX_FLAG_FORCE_MMA)) return APX_EINVAL;       // local-maximum mode: general kernel only
 
     apx_plan *p = new (std::nothrow) apx_plan();
     if (!p) return APX_ENOMEM;
@@ -101,6 +122,7 @@ extern "C" int apx_plan_create(const apx_plan_desc *desc, apx_plan **out)
     p->desc = *desc;
     p->desc.dirs = nullptr;
     p->B = B; p->D = desc->D; p->pad = desc->pad; p->k_lo = k_lo; p->k_hi = k_hi; p->W = k_hi - k_lo + 1;
+    p->specs = ss;
     p->R = desc->R; p->device = desc->device;
     volatile float r2 = desc->R * desc->R;                                     // one fp32 multiply
     p->R2 = r2;
@@ -122,7 +144,7 @@ extern "C" int apx_plan_create(const apx_plan_desc *desc, apx_plan **out)
         tw[r] = make_float2((float)std::cos(th), (float)-std::sin(th));
     }
     uint32_t mask[8];
-    std::memcpy(mask, desc->type_mask, 32);
+    std::memcpy(mask, union_mask, 32);                                         // ingest keeps every ion some spec accepts
 
 #define CUF(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { p->last_cuda = (int)e__; \
         return fail(e__ == cudaErrorMemoryAllocation ? APX_ENOMEM : APX_ECUDA); } } while (0)
@@ -157,7 +179,7 @@ extern "C" int apx_plan_create(const apx_plan_desc *desc, apx_plan **out)
         p->need_clamp = unit ? 0 : 1;
     }
     p->path = 0;
-    if (!(desc->flags & APX_FLAG_FORCE_FFT) && mma_path_supported(p)) {
+    if (!(desc->flags & APX_FLAG_FORCE_FFT) && !any_local && mma_path_supported(p)) {
         CUF(mma_path_prepare(p));
         p->path = 1;
     } else if (desc->flags & APX_FLAG_FORCE_MMA) {
@@ -167,6 +189,26 @@ extern "C" int apx_plan_create(const apx_plan_desc *desc, apx_plan **out)
     *out = p;
     return APX_OK;
 }
+
+extern "C" int apx_plan_create(const apx_plan_desc *desc, apx_plan **out)
+{
+    if (!out) return APX_EINVAL;
+    *out = nullptr;
+    if (!desc) return APX_EINVAL;
+    apx_sig_spec one;
+    std::memcpy(one.type_mask, desc->type_mask, 32);
+    one.k_lo = desc->k_lo; one.k_hi = desc->k_hi;
+    one.peak_mode = (desc->flags & APX_FLAG_LOCAL_MAX) ? APX_PEAK_LOCAL_MAX : APX_PEAK_MAX;
+    one.normalise = (desc->flags & APX_FLAG_NORMALISE) ? 1 : 0;
+    return create_plan(desc, &one, 1, out);
+}
+
+extern "C" int apx_plan_create_multi(const apx_plan_desc *desc, const apx_sig_spec *specs, int32_t n_specs, apx_plan **out)
+{
+    return create_plan(desc, specs, n_specs, out);
+}
+
+extern "C" int apx_plan_num_signatures(const apx_plan *p) { return p ? p->specs.n_specs : APX_EINVAL; }
 
 extern "C" int apx_plan_constants(const apx_plan *p, float *R2, float *s, float *freq_per_bin)
 {
@@ -234,7 +276,8 @@ extern "C" int apx_run_host(apx_plan *p, const float *xyz, const uint8_t *types,
     if (N >= (1LL << 31)) return APX_ERANGE;
     ON_DEVICE(p);
     cudaStream_t st = p->own_stream;
-    const int64_t row_bytes = (int64_t)p->D * 8;
+    const int S = p->specs.n_specs;
+    const int64_t row_bytes = (int64_t)p->D * 8 * S;              // all signature planes of one material point
     // material points per slab: bounded by the staging size, and at most a quarter of the job so that copies overlap
     int64_t slab = kSlabBytes / row_bytes;
     if (slab < 1) slab = 1;
@@ -246,7 +289,7 @@ extern "C" int apx_run_host(apx_plan *p, const float *xyz, const uint8_t *types,
     if (types && (rc = grow(p, &p->h2d_types, &p->cap_types, N + 16))) return rc;
     if ((rc = grow(p, &p->h2d_centres, &p->cap_centres, M * 12 + 16))) return rc;
     if ((rc = grow(p, &p->d2h_sig, &p->cap_sig, (nslab > 1 ? 2 : 1) * slab * row_bytes + 16))) return rc;
-    if (counts && (rc = grow(p, &p->d2h_counts, &p->cap_counts, M * 4 + 16))) return rc;
+    if (counts && (rc = grow(p, &p->d2h_counts, &p->cap_counts, (nslab > 1 ? 2 : 1) * slab * 4 * S + 16))) return rc;
     if ((rc = ensure_capacity(p, N))) return rc;
     if (p->path == 1) CU(p, mma_reserve_for(p, slab));
     // from here on work is in flight on the two internal streams: never return before both have drained, the copies
@@ -265,15 +308,20 @@ extern "C" int apx_run_host(apx_plan *p, const float *xyz, const uint8_t *types,
     if (rc) return drain(rc);
     for (int64_t m0 = 0, i = 0; m0 < M; m0 += slab, ++i) {
         const int64_t mc = (M - m0 < slab) ? M - m0 : slab;
-        float *dsig = (float *)p->d2h_sig + (i & 1) * slab * (int64_t)p->D * 2;
-        uint32_t *dcnt = counts ? (uint32_t *)p->d2h_counts + m0 : nullptr;
+        // a slab's staging holds its planes back to back: [S][mc][D][2] and [S][mc]
+        float *dsig = (float *)p->d2h_sig + (i & 1) * slab * (int64_t)p->D * 2 * S;
+        uint32_t *dcnt = counts ? (uint32_t *)p->d2h_counts + (i & 1) * slab * S : nullptr;
         if (i >= 2) CUD(cudaStreamWaitEvent(st, p->copy_done[i & 1], 0));       // the buffer's previous slab has left
         rc = apx_query(p, (const float *)p->h2d_centres + 3 * m0, mc, dsig, dcnt, st);
         if (rc) return drain(rc);
         CUD(cudaEventRecord(p->slab_done[i & 1], st));
         CUD(cudaStreamWaitEvent(p->copy_stream, p->slab_done[i & 1], 0));
-        CUD(cudaMemcpyAsync(sig + m0 * (int64_t)p->D * 2, dsig, (size_t)(mc * row_bytes), cudaMemcpyDeviceToHost, p->copy_stream));
-        if (counts) CUD(cudaMemcpyAsync(counts + m0, dcnt, (size_t)mc * 4, cudaMemcpyDeviceToHost, p->copy_stream));
+        for (int sp = 0; sp < S; ++sp) {                              // plane sp of the slab -> plane sp of the caller's array
+            CUD(cudaMemcpyAsync(sig + ((int64_t)sp * M + m0) * p->D * 2, dsig + (int64_t)sp * mc * p->D * 2,
+                                (size_t)(mc * (int64_t)p->D * 8), cudaMemcpyDeviceToHost, p->copy_stream));
+            if (counts) CUD(cudaMemcpyAsync(counts + (int64_t)sp * M + m0, dcnt + (int64_t)sp * mc, (size_t)mc * 4,
+                                            cudaMemcpyDeviceToHost, p->copy_stream));
+        }
         CUD(cudaEventRecord(p->copy_done[i & 1], p->copy_stream));
     }
 #undef CUD
@@ -293,8 +341,8 @@ extern "C" int apx_debug_histograms(apx_plan *p, const float *centre3, int32_t d
     ON_DEVICE(p);
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
-    int64_t cap = p->dbg_sig ? (int64_t)p->D * 8 : 0;
-    if ((rc = grow(p, (void **)&p->dbg_sig, &cap, (int64_t)p->D * 8))) return rc;
+    int64_t cap = p->dbg_sig ? (int64_t)p->D * 8 * p->specs.n_specs : 0;
+    if ((rc = grow(p, (void **)&p->dbg_sig, &cap, (int64_t)p->D * 8 * p->specs.n_specs))) return rc;
     CU(p, cudaMemcpyAsync(p->dbg_centre, centre3, 12, cudaMemcpyHostToDevice, st));
     CU(p, cudaMemsetAsync(out, 0, (size_t)nd * p->B * sizeof(uint32_t), st));
     p->dbg_hist_out = out; p->dbg_d0 = d0; p->dbg_nd = nd;
@@ -302,6 +350,16 @@ extern "C" int apx_debug_histograms(apx_plan *p, const float *centre3, int32_t d
     p->dbg_hist_out = nullptr; p->dbg_d0 = 0; p->dbg_nd = 0;
     return rc;
 }
+
+#ifdef APX_TRACE
+// development builds only (-DAPX_TRACE, not declared in the public headers): timeline buffer for k_signature_mma
+extern "C" int apx_debug_trace(apx_plan *p, long long *device_buf, int block, int cap)
+{
+    if (!p) return APX_EINVAL;
+    p->dbg_trace = device_buf; p->dbg_trace_block = block; p->dbg_trace_cap = cap;
+    return APX_OK;
+}
+#endif
 
 extern "C" const char *apx_strerror(int s)
 {

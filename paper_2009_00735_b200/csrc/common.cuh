@@ -20,9 +20,30 @@ struct GridParams {
 
 constexpr int kMaxCells = 1 << 21;
 
+// Signatures of one plan ("multiple signatures (for different atom types) are computed per
+// ROI", L126-130, L208 "several lattice plane families {002}, {220}, {111}", L416-418): up to kMaxSpecs (type mask, spectral
+// window, peak mode, normalisation) tuples served by ONE ingest and one launch.  Specs with the same type mask form a class:
+// a class is gathered and binned once, its histograms transformed once over the union window [plan k_lo, plan k_hi], and
+// every spec of the class picks its peak from its own sub-window.
+constexpr int kMaxSpecs = APX_MAX_SIGNATURES;
+constexpr uint32_t kUntyped = 0xFFFFu;      // type stored for ions ingested without a type array: accepted by every class
+struct SpecSet {
+    int n_specs, n_classes;
+    int cls_of[kMaxSpecs];                  // class of every spec
+    int k_lo[kMaxSpecs], k_hi[kMaxSpecs];   // inclusive sub-window, inside the plan's union window
+    int mode[kMaxSpecs];                    // APX_PEAK_MAX / APX_PEAK_LOCAL_MAX
+    int norm[kMaxSpecs];                    // 1 = write A / N_c
+    uint32_t cls_mask[kMaxSpecs][8];        // accepted ion types of every class
+};
+__device__ __forceinline__ bool type_in_class(const SpecSet &ss, int cls, uint32_t t)
+{
+    return t == kUntyped || ((ss.cls_mask[cls][(t >> 5) & 7] >> (t & 31)) & 1u);
+}
+
 struct Plan {
     apx_plan_desc desc;            // copy (dirs pointer nulled)
-    int B, D, pad, k_lo, k_hi, W;
+    int B, D, pad, k_lo, k_hi, W;  // k_lo..k_hi = union window of all specs, W = its width
+    SpecSet specs;
     float R, R2, s;
     int device;
     int path;                      // 0 = FFT kernel, 1 = MMA kernel
@@ -40,20 +61,26 @@ struct Plan {
     int *d_dir_perm_mirror;        // [Dp] half-grid mode: index of the direction opposite to the slot's
     int Dp;                        // D rounded up to a multiple of 32
     int mma_paired;                // 1 = half-grid mode: the grid is antipodally symmetric, one direction per pair is binned
+    int tune_binclear, tune_unit_split;   // k_signature_mma scheduling knobs (see mma_path_prepare)
     int need_clamp;                // 1 = the bin clamp of Eq. 1 can trigger and must stay in the kernels' inner loops
     uint32_t *d_deferred;          // [0] count, [1..] material points the MMA kernel left to the FFT kernel
     int64_t cap_deferred;
     uint32_t *dbg_hist_out;        // non-null only inside apx_debug_histograms: the kernels also export their histograms
     int dbg_d0, dbg_nd;
+    long long *dbg_trace;          // APX_TRACE builds only: pipeline timeline buffer of k_signature_mma (else unused)
+    int dbg_trace_block, dbg_trace_cap;
     float *dbg_centre;             // [3] device copy of the debug centre
     float *dbg_sig;                // [D][2] scratch signature output of the debug run
+    float *d_refine_off;           // [16] sub-cell centre offsets of apx_refine_centres
+    float *d_kaxis;                // [cap_kaxis] k values of one axis of apx_fsp's reciprocal-space grid
+    int cap_kaxis;
     uint32_t *d_type_mask;         // [8] words
     GridParams *d_grid;
     uint32_t *d_cell_start;        // [kMaxCells + 1]
     uint32_t *d_cell_cursor;       // [kMaxCells]
     uint32_t *d_scan_tiles;        // [kMaxCells / 8192] tile totals of the cell scan
     uint32_t *d_cell_of_ion;       // [capacity]
-    float4 *d_sorted;              // [capacity]  (x, y, z, original index bits)
+    float4 *d_sorted;              // [capacity]  (x, y, z, ion type bits)
     int64_t capacity;              // ions the sorted buffers can hold
     // host staging for apx_run_host
     cudaStream_t own_stream, copy_stream;
@@ -112,7 +139,7 @@ cudaError_t launch_ingest(Plan *p, const float *xyz, const uint8_t *types, int64
 cudaError_t launch_signature_fft(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts,
                                  cudaStream_t st);
 // FFT kernel over a device-side list of material points (list[0] = count, list[1..] = ids)
-cudaError_t launch_signature_fft_list(Plan *p, const float *centres, const uint32_t *list, float *sig,
+cudaError_t launch_signature_fft_list(Plan *p, const float *centres, const uint32_t *list, int64_t M, float *sig,
                                       uint32_t *counts, cudaStream_t st);
 cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float *sig, uint32_t *counts,
                                  cudaStream_t st);
@@ -122,3 +149,5 @@ cudaError_t mma_reserve_deferred(Plan *p, int64_t need);   // deferred list of a
 cudaError_t mma_reserve_for(Plan *p, int64_t M);           // ... sized for any apx_query of up to M material points
 
 }  // namespace apx
+
+struct apx_plan : public apx::Plan {};

@@ -210,7 +210,8 @@ __global__ void __launch_bounds__(1024) k_scan_add(uint32_t *cell, uint32_t *cur
     if (threadIdx.x == 0 && (tile + 1) * kScanTile >= n) cell[n] = off + tile_sum[tile];   // the last tile: grand total
 }
 
-__global__ void __launch_bounds__(256) k_scatter(const float *__restrict__ xyz, int64_t N,
+// record = (x, y, z, ion type): the type lets one sorted copy serve several type masks (classes of a multi-signature plan)
+__global__ void __launch_bounds__(256) k_scatter(const float *__restrict__ xyz, const uint8_t *__restrict__ types, int64_t N,
                                                  const uint32_t *__restrict__ cell_of_ion, uint32_t *cursor,
                                                  float4 *__restrict__ sorted)
 {
@@ -218,7 +219,7 @@ __global__ void __launch_bounds__(256) k_scatter(const float *__restrict__ xyz, 
         uint32_t c = cell_of_ion[i];
         if (c == 0xFFFFFFFFu) continue;
         uint32_t pos = atomicAdd(&cursor[c], 1u);
-        sorted[pos] = make_float4(xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2], __uint_as_float((uint32_t)i));
+        sorted[pos] = make_float4(xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2], __uint_as_float(types ? (uint32_t)types[i] : kUntyped));
     }
 }
 
@@ -233,7 +234,7 @@ cudaError_t launch_ingest(Plan *p, const float *xyz, const uint8_t *types, int64
         k_count<<<blocks, 256, 0, st>>>(xyz, types, N, p->d_type_mask, p->d_grid, p->d_cell_start, p->d_cell_of_ion);
     k_scan_local<<<kMaxCells / kScanTile, 1024, 0, st>>>(p->d_cell_start, p->d_scan_tiles, p->d_grid);
     k_scan_add<<<kMaxCells / kScanTile, 1024, 0, st>>>(p->d_cell_start, p->d_cell_cursor, p->d_scan_tiles, p->d_grid);
-    if (N > 0) k_scatter<<<blocks, 256, 0, st>>>(xyz, N, p->d_cell_of_ion, p->d_cell_cursor, p->d_sorted);
+    if (N > 0) k_scatter<<<blocks, 256, 0, st>>>(xyz, types, N, p->d_cell_of_ion, p->d_cell_cursor, p->d_sorted);
     return cudaGetLastError();
 }
 

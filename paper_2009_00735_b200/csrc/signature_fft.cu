@@ -36,6 +36,8 @@ struct FftParams {
     int hist_d0, hist_nd;      // [hist_d0, hist_d0 + hist_nd), copied from the shared counters the FFT is about to read
     int D, k_lo, k_hi, cap, nchunks, ngroups, clamp;
     float R, R2;
+    SpecSet ss;                // signatures of the plan: classes (type masks) and per-spec windows / modes
+    int64_t M;                 // material points of the call: plane stride of sig (M * D) and counts (M)
 };
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
@@ -130,7 +132,7 @@ __device__ __forceinline__ int fft_pos(int k)
 // Gather (step a2): every warp walks x-rows of cells (contiguous in the sorted array), keeps ions with
 // r^2 <= R2 and appends d = p - c as a packed 12-byte record.  *s_n may exceed cap (then the streaming path is used).
 __device__ __forceinline__ void gather_roi(const FftParams &p, const GridParams &g, const RoiCells &rc,
-                                           float cx, float cy, float cz, float *ions, int *s_n)
+                                           float cx, float cy, float cz, float *ions, int *s_n, int cls)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int ny_r = rc.iy1 - rc.iy0 + 1, nz_r = rc.iz1 - rc.iz0 + 1;
@@ -144,7 +146,7 @@ __device__ __forceinline__ void gather_roi(const FftParams &p, const GridParams 
             if (i < end) {
                 float4 q = p.sorted[i];
                 dx = __fsub_rn(q.x, cx); dy = __fsub_rn(q.y, cy); dz = __fsub_rn(q.z, cz);
-                in = inside(dx, dy, dz, p.R2);
+                in = inside(dx, dy, dz, p.R2) && (p.ss.n_classes == 1 || type_in_class(p.ss, cls, __float_as_uint(q.w)));
             }
             unsigned msk = __ballot_sync(0xffffffffu, in);
             if (msk) {
@@ -158,7 +160,7 @@ __device__ __forceinline__ void gather_roi(const FftParams &p, const GridParams 
 }
 
 template <int B>
-__global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const FftParams p)
+__global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const __grid_constant__ FftParams p)
 {
     constexpr int G = (B <= 1024) ? 32 : 32768 / B;            // directions per group
     constexpr int N = B / 2, T = kFftThreads / G, LPD = 32 / G; // threads per direction, ions per warp instruction
@@ -188,13 +190,16 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const FftParam
         const float cx = p.centres[3 * m], cy = p.centres[3 * m + 1], cz = p.centres[3 * m + 2];
         const RoiCells rc = roi_cells(g, cx, cy, cz, p.R);
 
+      for (int cls = 0; cls < p.ss.n_classes; ++cls) {     // specs with the same type mask share gather, binning and FFT
         __syncthreads();                 // previous item done with the shared buffers; s_tw loaded
         if (tid == 0) s_n = 0;
         __syncthreads();
-        if (g.n_accepted) gather_roi(p, g, rc, cx, cy, cz, ions, &s_n);
+        if (g.n_accepted) gather_roi(p, g, rc, cx, cy, cz, ions, &s_n, cls);
         __syncthreads();
         const int n = s_n;
-        if (chunk == 0 && tid == 0 && p.counts) p.counts[m] = (uint32_t)n;
+        if (chunk == 0 && tid == 0 && p.counts)
+            for (int sp = 0; sp < p.ss.n_specs; ++sp)
+                if (p.ss.cls_of[sp] == cls) p.counts[(size_t)sp * p.M + m] = (uint32_t)n;
         const bool stream = n > p.cap;
 
         for (int gi = g_begin; gi < g_end; ++gi) {
@@ -237,13 +242,14 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const FftParam
                         for (uint32_t i = beg + lane / G; i < end; i += LPD) {
                             const float4 q = p.sorted[i];
                             const float dx = __fsub_rn(q.x, cx), dy = __fsub_rn(q.y, cy), dz = __fsub_rn(q.z, cz);
-                            if (inside(dx, dy, dz, p.R2)) atomicAdd(cnt + bin_of(npx, npy, npz, dx, dy, dz, half_b, magic) * G, 1u);
+                            if (inside(dx, dy, dz, p.R2) && (p.ss.n_classes == 1 || type_in_class(p.ss, cls, __float_as_uint(q.w))))
+                                atomicAdd(cnt + bin_of(npx, npy, npz, dx, dy, dz, half_b, magic) * G, 1u);
                         }
                     }
                 }
             }
             __syncthreads();
-            if (p.hist_out) {                                    // test hook: the counters are complete, the FFT has not started
+            if (p.hist_out && cls == 0) {                        // test hook (first class): counters complete, FFT not started
                 const uint32_t *ub = reinterpret_cast<const uint32_t *>(buf);
                 for (int i = tid; i < B * G; i += kFftThreads) {
                     const int b = i / G, dg = gi * G + i % G;
@@ -265,10 +271,10 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const FftParam
                 fft_pass<B, G, (kLast > 1 ? kLast : 2), false>(buf, s_tw, d, t, kLast);
                 __syncthreads();
             }
-            // ---- split step on the window + arg-max (steps a5 tail, a6) ------------------------------------
-            float best = -1.0f;
-            int kbest = p.k_lo;
-            for (int k = p.k_lo + t; k <= p.k_hi; k += T) {
+            // ---- split step on the window + arg-max (steps a5 tail, a6), once per spec of this class ---------------
+            // 4 |X_k|^2 of spectral bin k (0 <= k <= B/2 + 1; A_{B/2+1} = A_{B/2-1} by conjugate symmetry)
+            auto power_at = [&](int k) -> float {
+                if (k > N) k = B - k;
                 const int ea = fft_pos<B>(k & (N - 1)), eb = fft_pos<B>((N - k) & (N - 1));
                 const float2 za = make_float2(buf[(2 * ea) * G + d], buf[(2 * ea + 1) * G + d]);
                 const float2 zb = make_float2(buf[(2 * eb) * G + d], buf[(2 * eb + 1) * G + d]);
@@ -278,25 +284,41 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const FftParam
                 // -i * w * (orr + i oi) = (w.y*orr + w.x*oi) + i (w.y*oi - w.x*orr)
                 const float xr = er + (w.y * orr + w.x * oi);
                 const float xi = ei + (w.y * oi - w.x * orr);
-                const float pw = xr * xr + xi * xi;                       // 4 |X_k|^2
-                if (pw > best) { best = pw; kbest = k; }                  // ascending k per thread: lowest k kept on ties
-            }
-            cand[t * G + d] = make_float2(best, __int_as_float(kbest));
-            __syncthreads();
-            if (tid < G) {
-                float bb = -1.0f;
-                int kb = p.k_lo;
-                for (int s = 0; s < T; ++s) {
-                    const float2 c = cand[s * G + tid];
-                    const int ck = __float_as_int(c.y);
-                    if (c.x > bb || (c.x == bb && ck < kb)) { bb = c.x; kb = ck; }
+                return xr * xr + xi * xi;
+            };
+            for (int sp = 0; sp < p.ss.n_specs; ++sp) {
+                if (p.ss.cls_of[sp] != cls) continue;
+                const int s_lo = p.ss.k_lo[sp], s_hi = p.ss.k_hi[sp];
+                const bool local = p.ss.mode[sp] == APX_PEAK_LOCAL_MAX;
+                float best = -1.0f;
+                int kbest = s_lo;
+                for (int k = s_lo + t; k <= s_hi; k += T) {
+                    const float pw = power_at(k);
+                    // local-maximum mode (reading #20): only bins with A_k > A_{k-1} and A_k >= A_{k+1} compete
+                    if (local && !(pw > power_at(k == 0 ? 1 : k - 1) && pw >= power_at(k + 1))) continue;
+                    if (pw > best) { best = pw; kbest = k; }              // ascending k per thread: lowest k kept on ties
                 }
-                const int dg = gi * G + tid;
-                if (dg < p.D) p.sig[(size_t)m * p.D + dg] = make_float2(0.5f * sqrtf(fmaxf(bb, 0.0f)), (float)kb);
+                cand[t * G + d] = make_float2(best, __int_as_float(kbest));
+                __syncthreads();
+                if (tid < G) {
+                    float bb = -1.0f;
+                    int kb = s_lo;
+                    for (int s = 0; s < T; ++s) {
+                        const float2 c = cand[s * G + tid];
+                        const int ck = __float_as_int(c.y);
+                        if (c.x > bb || (c.x == bb && ck < kb)) { bb = c.x; kb = ck; }
+                    }
+                    const int dg = gi * G + tid;
+                    float amp = 0.5f * sqrtf(fmaxf(bb, 0.0f));
+                    if (p.ss.norm[sp]) amp = n ? __fdiv_rn(amp, (float)n) : 0.0f;
+                    if (dg < p.D) p.sig[(size_t)sp * p.M * p.D + (size_t)m * p.D + dg] = make_float2(amp, (float)kb);
+                }
+                __syncthreads();                                          // cand is reused by the next spec
             }
             // the next group's clear of buf is ordered after this group's reads by the barrier above; cand is
             // rewritten only after three more barriers
         }
+      }
     }
 }
 
@@ -312,6 +334,7 @@ static int fft_cap_for(int B)
     return (int)(((budget - fft_smem_for(B, 0)) / 12) & ~(size_t)63);
 }
 
+// M = material points of the call (plane stride of the outputs); list != nullptr: only the listed ones are processed
 static cudaError_t launch_fft_common(Plan *p, const float *centres, int64_t M, const uint32_t *list, float *sig,
                                      uint32_t *counts, cudaStream_t st)
 {
@@ -320,6 +343,7 @@ static cudaError_t launch_fft_common(Plan *p, const float *centres, int64_t M, c
     q.sorted = p->d_sorted; q.cell_start = p->d_cell_start; q.grid = p->d_grid; q.centres = centres;
     q.dirs_scaled = p->d_dirs_scaled; q.tw = p->d_twiddle; q.sig = reinterpret_cast<float2 *>(sig); q.counts = counts;
     q.hist_out = p->dbg_hist_out; q.hist_d0 = p->dbg_d0; q.hist_nd = p->dbg_nd;
+    q.ss = p->specs; q.M = M;
     q.list = list; q.D = p->D; q.k_lo = p->k_lo; q.k_hi = p->k_hi; q.cap = fft_cap_for(B);
     q.ngroups = (p->D + G - 1) / G;
     // enough CTAs to fill the machine a few times over, but at least a handful of groups per CTA (one gather each)
@@ -358,10 +382,10 @@ cudaError_t launch_signature_fft(Plan *p, const float *centres, int64_t M, float
     return launch_fft_common(p, centres, M, nullptr, sig, counts, st);
 }
 
-cudaError_t launch_signature_fft_list(Plan *p, const float *centres, const uint32_t *list, float *sig,
+cudaError_t launch_signature_fft_list(Plan *p, const float *centres, const uint32_t *list, int64_t M, float *sig,
                                       uint32_t *counts, cudaStream_t st)
 {
-    return launch_fft_common(p, centres, 0, list, sig, counts, st);
+    return launch_fft_common(p, centres, M, list, sig, counts, st);
 }
 
 }  // namespace apx

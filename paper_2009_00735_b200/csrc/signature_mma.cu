@@ -32,6 +32,7 @@
 // serves both; see the comment above struct Detect.
 #include <algorithm>
 #include <array>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <cmath>
@@ -70,6 +71,22 @@ constexpr int kStsClearBelow = 700;      // ROIs with fewer ions clear with plai
 constexpr int kEpiRound = 4;             // window bins per epilogue round (one tcgen05.ld x16)
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+// Development aid (build with -DAPX_TRACE): lane 0 of selected warps of ONE CTA appends (event, group, SM clock) records to a
+// global buffer, which shows the timeline of the warp-specialised pipeline.  Compiled out otherwise.
+#ifdef APX_TRACE
+#define APX_TRACE_EVENT(p, ev, grp)                                                                   \
+    do {                                                                                              \
+        if ((p).trace && blockIdx.x == (unsigned)(p).trace_block && (threadIdx.x & 31) == 0) {        \
+            const unsigned long long i__ = atomicAdd((unsigned long long *)(p).trace, 1ull);          \
+            if (i__ < (unsigned long long)(p).trace_cap) {                                            \
+                (p).trace[1 + 2 * i__] = ((long long)(ev) << 48) | ((long long)(threadIdx.x >> 5) << 32) | (long long)(grp); \
+                (p).trace[2 + 2 * i__] = clock64();                                                   \
+            }                                                                                         \
+        }                                                                                             \
+    } while (0)
+#else
+#define APX_TRACE_EVENT(p, ev, grp) do { } while (0)
+#endif
 __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t cnt)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(cnt));
@@ -152,8 +169,15 @@ struct MmaParams {
     uint32_t *deferred;        // [0] = count, [1..] = material point ids left to the FFT kernel
     uint32_t *hist_out;        // test hook (apx_debug_histograms, M = 1): uint32[hist_nd][B] histograms of the directions
     int hist_d0, hist_nd;      // [hist_d0, hist_d0 + hist_nd), decoded from the shared-memory buffers the tensor core reads
+#ifdef APX_TRACE
+    long long *trace;          // [0] = record count, then (tag, clock) pairs
+    int trace_block, trace_cap;
+#endif
     int D, B, nl, k_lo, W, N, cap, cap_big, nchunks, ngroups, clamp, M;
     int half;                  // 1 = half-grid mode: one direction per antipodal pair is binned (perm_mirror != nullptr)
+    SpecSet ss;                // signatures of the plan: classes (type masks), per-spec sub-windows of [k_lo, k_lo + W)
+    int binclear_below;        // double-buffered ROIs with fewer ions: the binning warps clear the buffers themselves
+    int unit_split;            // 1 = ions are dealt to the binning warps in whole blocks of 4 * NS (no ragged tails)
     uint32_t tmem_cols;
     float R, R2;
 };
@@ -187,7 +211,7 @@ __host__ __device__ inline MmaSmem mma_smem_layout(int B, int N, int W, int cap)
 // Gather (step a2) into quad-blocked records: four ions = 48 B = [dx0..dx3][dy0..dy3][dz0..dz3], i.e. three LDS.128
 // whose register pairs are the operands of the packed fp32x2 arithmetic of the binning warps.
 __device__ __forceinline__ void gather_roi3(const MmaParams &p, const GridParams &g, const RoiCells &rc,
-                                            float cx, float cy, float cz, float *ions, int *s_n)
+                                            float cx, float cy, float cz, float *ions, int *s_n, int cls)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int ny_r = rc.iy1 - rc.iy0 + 1, nz_r = rc.iz1 - rc.iz0 + 1;
@@ -201,7 +225,7 @@ __device__ __forceinline__ void gather_roi3(const MmaParams &p, const GridParams
             if (i < end) {
                 float4 q = p.sorted[i];
                 dx = __fsub_rn(q.x, cx); dy = __fsub_rn(q.y, cy); dz = __fsub_rn(q.z, cz);
-                in = inside(dx, dy, dz, p.R2);
+                in = inside(dx, dy, dz, p.R2) && (p.ss.n_classes == 1 || type_in_class(p.ss, cls, __float_as_uint(q.w)));
             }
             unsigned msk = __ballot_sync(0xffffffffu, in);
             if (msk) {
@@ -366,6 +390,7 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
 // Output: mode 0 (ordinary group gi) writes the slot's own direction and, in half-grid mode, the opposite direction
 // unless the pair was flagged (bit of `mask`); mode 1 (fix-up group) writes only the opposite direction of the listed pair.
 struct EpiOut {
+    int cls, n;                          // class of signatures served by this histogram, its ROI ion count (normalisation)
     int mode, gi, g0, f, nfix;           // g0 = first group of the sub-range, f = fix-up group, nfix = listed pairs
     uint32_t *flag;                      // mode 0, half-grid: flag word of this group (read, then reset)
     const uint16_t *fix;
@@ -378,8 +403,12 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
     const uint32_t mask = (kHalf && mode == 0) ? *eo.flag : 0u;         // complete: every binning warp has arrived
     const uint32_t acc0 = acc + ((uint32_t)(q * 32) << 16);
     float2 *exch = exch_all + set * (kEpiRound * 4 * 32), *cand = cand_all + set * (4 * 32);
-    float best = -1.0f;
-    int kbest = p.k_lo;
+    // one running maximum per spec of the class (a spec's window is a sub-range of the transformed union window)
+    float best[kMaxSpecs];
+    int kbest[kMaxSpecs];
+#pragma unroll
+    for (int sp = 0; sp < kMaxSpecs; ++sp) { best[sp] = -1.0f; kbest[sp] = sp < p.ss.n_specs ? p.ss.k_lo[sp] : 0; }
+    const bool one_spec = p.ss.n_specs == 1;
 #pragma unroll 1
     for (int r0 = 0; r0 < p.W; r0 += kEpiRound) {
         uint32_t v[16];
@@ -412,39 +441,63 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
                 xr += e.x; xi += e.y;
             }
             const float pw = xr * xr + xi * xi;
-            if (pw > best) { best = pw; kbest = p.k_lo + w; }            // ascending w: lowest k kept on ties
+            const int k = p.k_lo + w;
+            if (one_spec) {
+                if (pw > best[0]) { best[0] = pw; kbest[0] = k; }        // ascending w: lowest k kept on ties
+            } else {
+#pragma unroll
+                for (int sp = 0; sp < kMaxSpecs; ++sp)
+                    if (sp < p.ss.n_specs && p.ss.cls_of[sp] == eo.cls && k >= p.ss.k_lo[sp] && k <= p.ss.k_hi[sp] && pw > best[sp]) {
+                        best[sp] = pw; kbest[sp] = k;
+                    }
+            }
         }
         if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
     }
-    cand[q * 32 + lane] = make_float2(best, __int_as_float(kbest));
-    if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
-    if (q == 0 && lane < Lay<NB>::G) {                   // (NB = 8: lanes 16..31 carry copies of lanes 0..15)
-        constexpr int G = Lay<NB>::G;
-        if (kHalf && lane == 0 && mode == 0) *eo.flag = 0u;             // every thread of the set has read it (barriers above)
-        float bb = -1.0f;
-        int kb = p.k_lo;
+    if (kHalf && mode == 0 && q == 0 && lane == 0) *eo.flag = 0u;     // every thread of the set has read it (barriers above)
+#pragma unroll 1
+    for (int sp = 0; sp < p.ss.n_specs; ++sp) {
+        if (p.ss.cls_of[sp] != eo.cls) continue;
+        float bsel = best[0];
+        int ksel = kbest[0];
 #pragma unroll
-        for (int s = 0; s < 4; ++s) {
-            const float2 c2 = cand[s * 32 + lane];
-            const int ck = __float_as_int(c2.y);
-            if (c2.x > bb || (c2.x == bb && ck < kb)) { bb = c2.x; kb = ck; }
+        for (int j = 1; j < kMaxSpecs; ++j)
+            if (j == sp) { bsel = best[j]; ksel = kbest[j]; }
+        cand[q * 32 + lane] = make_float2(bsel, __int_as_float(ksel));
+        if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
+        if (q == 0 && lane < Lay<NB>::G) {                   // (NB = 8: lanes 16..31 carry copies of lanes 0..15)
+            constexpr int G = Lay<NB>::G;
+            float bb = -1.0f;
+            int kb = p.ss.k_lo[sp];
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                const float2 c2 = cand[s * 32 + lane];
+                const int ck = __float_as_int(c2.y);
+                if (c2.x > bb || (c2.x == bb && ck < kb)) { bb = c2.x; kb = ck; }
+            }
+            // M row (within a part) = chunk * 8 + word * 2 + half  ->  slot = half * G/2 + chunk * 4 + word
+            const int slot = (lane & 1) * (G / 2) + ((lane >> 3) << 2) + ((lane & 7) >> 1);
+            float amp = 16777216.0f * sqrtf(fmaxf(bb, 0.0f));
+            if (p.ss.norm[sp]) amp = eo.n ? __fdiv_rn(amp, (float)eo.n) : 0.0f;   // normalised intensity A / N_c (L424)
+            const float2 res = make_float2(amp, (float)kb);
+            float2 *out = p.sig + (size_t)sp * (size_t)p.M * p.D + (size_t)m * p.D;
+            if (mode == 0) {
+                const int d = p.perm[eo.gi * G + slot];
+                if (d >= 0) out[d] = res;
+                if (kHalf && !((mask >> slot) & 1u)) {               // the mirrored histogram has the same amplitude spectrum
+                    const int d2 = p.perm_mirror[eo.gi * G + slot];
+                    if (d2 >= 0) out[d2] = res;
+                }
+            } else {
+                const int e = eo.f * G + slot;
+                if (e < eo.nfix) {
+                    const int d2 = p.perm_mirror[eo.g0 * G + (int)eo.fix[e]];
+                    if (d2 >= 0) out[d2] = res;
+                }
+            }
         }
-        // M row (within a part) = chunk * 8 + word * 2 + half  ->  slot = half * G/2 + chunk * 4 + word
-        const int slot = (lane & 1) * (G / 2) + ((lane >> 3) << 2) + ((lane & 7) >> 1);
-        const float2 res = make_float2(16777216.0f * sqrtf(fmaxf(bb, 0.0f)), (float)kb);
-        if (mode == 0) {
-            const int d = p.perm[eo.gi * G + slot];
-            if (d >= 0) p.sig[(size_t)m * p.D + d] = res;
-            if (kHalf && !((mask >> slot) & 1u)) {               // the mirrored histogram has the same amplitude spectrum
-                const int d2 = p.perm_mirror[eo.gi * G + slot];
-                if (d2 >= 0) p.sig[(size_t)m * p.D + d2] = res;
-            }
-        } else {
-            const int e = eo.f * G + slot;
-            if (e < eo.nfix) {
-                const int d2 = p.perm_mirror[eo.g0 * G + (int)eo.fix[e]];
-                if (d2 >= 0) p.sig[(size_t)m * p.D + d2] = res;
-            }
+        if (!one_spec) {                                     // cand is reused by the next spec of the class
+            if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
         }
     }
     // the set's cand is rewritten only after the barriers of the rounds of its next epilogue
@@ -505,7 +558,7 @@ struct PipeShared {
 template <int KS, int NB, bool kBig, bool kHalf>
 __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &L, unsigned char *smem, uint32_t tmem, int n_ions,
                                              const Seq &sq, int64_t m, const float *ions, const float2 *phase,
-                                             float2 *exch, float2 *cand, const PipeShared &ps)
+                                             float2 *exch, float2 *cand, const PipeShared &ps, int cls)
 {
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);      // provably warp-uniform: ion addresses live in uniform registers
@@ -522,6 +575,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
     const int nitems = sq.ngrp * npass;
     const int mode = kHalf ? sq.mode : 0;
     const int it_base = sq.grp_base * npass;
+    const bool binclr = !kBig && n < p.binclear_below;
     if (warp < kBinWarps) {
         BinConst c;
         c.half_b = (float)(p.B / 2); c.magic_a = magic_for(p.B); c.magic_b = 12582912.0f + 4.0f;
@@ -545,6 +599,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                 const float *db = p.dirs_sorted + (eb < sq.nfix ? (size_t)(sq.g0 * G + (int)ps.fix[eb]) * 3 : 0);
                 n.ax = -da[0]; n.ay = -da[1]; n.az = -da[2]; n.bx = -db[0]; n.by = -db[1]; n.bz = -db[2];
             }
+            APX_TRACE_EVENT(p, 0, sq.grp_base + gl);                                 // binning warp ready for the item
             if (kBig) {
                 // single-buffered: the shared-memory pipe is idle while the tensor core transforms the buffer, so the 16
                 // binning warps clear it themselves as soon as it has been read (a few STS.128 per thread)
@@ -554,12 +609,30 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                     for (int i = tid; i < (int)(L.hist_bytes / 16); i += kBinWarps * 32) hb[i] = make_uint4(0, 0, 0, 0);
                     asm volatile("bar.sync 5, %0;" ::"n"(kBinWarps * 32) : "memory");
                 }
+            } else if (binclr) {
+                // few ions: a group is binned long before the tensor core needs the other buffer back, so the chain
+                // transform -> clear warp -> free only adds latency; the 16 binning warps clear the buffer themselves
+                // (10 STS.128 per thread) as soon as its MMAs have completed
+                if (use >= 1) {
+                    mbar_wait(&ps.done[buf], (uint32_t)((use - 1) & 1));
+                    uint4 *hb = reinterpret_cast<uint4 *>(smem + (buf ? L.hist1 : L.hist0));
+                    for (int i = tid; i < (int)(L.hist_bytes / 16); i += kBinWarps * 32) hb[i] = make_uint4(0, 0, 0, 0);
+                    asm volatile("bar.sync 5, %0;" ::"n"(kBinWarps * 32) : "memory");
+                }
             } else if (use >= 1) {
                 mbar_wait_lean(&ps.free_[buf], (uint32_t)((use - 1) & 1));             // cleared after its previous use
             }
+            APX_TRACE_EVENT(p, 1, sq.grp_base + gl);                                 // bin start (buffer free)
             const int a0 = pass * 2048, a1 = min(n_ions, a0 + 2048);
-            const int nq = (a1 - a0 + 3) >> 2;                                       // quads of this pass, split evenly
-            const int i0 = a0 + 4 * ((warp * nq) / kBinWarps), i1 = min(a1, a0 + 4 * (((warp + 1) * nq) / kBinWarps));
+            int i0, i1;
+            if (p.unit_split) {                                                      // whole blocks of 4 * NS ions per warp
+                constexpr int U = 4 * Lay<NB>::NS;
+                const int nu = (a1 - a0 + U - 1) / U;
+                i0 = a0 + U * ((warp * nu) / kBinWarps); i1 = min(a1, a0 + U * (((warp + 1) * nu) / kBinWarps));
+            } else {
+                const int nq = (a1 - a0 + 3) >> 2;                                   // quads of this pass, split evenly
+                i0 = a0 + 4 * ((warp * nq) / kBinWarps); i1 = min(a1, a0 + 4 * (((warp + 1) * nq) / kBinWarps));
+            }
             const uint32_t k0 = k0base + (uint32_t)buf * (L.hist1 - L.hist0);
             Detect dta, dtb;
             if (detect) {
@@ -575,6 +648,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
             __syncwarp();
+            APX_TRACE_EVENT(p, 2, sq.grp_base + gl);                                 // bin end
             if (lane == 0) mbar_arrive(&ps.full[buf]);
             if (++pass == npass) { pass = 0; ++gl; }
         }
@@ -591,9 +665,11 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
             const int gq = sq.grp_base + gl;
             mbar_wait<100>(&ps.full[buf], (uint32_t)(use & 1));
+            APX_TRACE_EVENT(p, 3, gq);                                                // MMA warp: buffer full
             if (pass == 0 && gq >= 2) mbar_wait(&ps.tfree[gq & 1], (uint32_t)(((gq >> 1) - 1) & 1));
+            APX_TRACE_EVENT(p, 4, gq);                                                // accumulator free, MMAs issued next
             asm volatile("tcgen05.fence::after_thread_sync;");
-            if (p.hist_out)                                      // test hook: the buffer is complete (all binning warps arrived)
+            if (p.hist_out && cls == 0)                          // test hook (first class): the buffer is complete
                 export_hist<NB, kHalf>(p, smem + (buf ? L.hist1 : L.hist0), mode, sq.g0 + gl, sq.g0, gl, sq.nfix, ps.fix,
                                        (kHalf && mode == 0) ? ps.flag[gq & 3] : 0u, pass, lane);
             const uint32_t acc = tmem + (uint32_t)((gq & 1) * p.N);
@@ -618,9 +694,10 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
     } else if (warp == kClrWarp) {
         // ---- clear warp: once the tensor core has read a buffer, clear it with bulk copies of zeros (TMA engine, no
         //      LSU work); free(buf) completes when all bytes have landed
-        for (int it = 0; it < (kBig ? 0 : nitems); ++it) {           // (single-buffered: the binning warps clear)
+        for (int it = 0; it < ((kBig || binclr) ? 0 : nitems); ++it) {   // (otherwise the binning warps clear)
             const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
             mbar_wait<100>(&ps.done[buf], (uint32_t)(use & 1));
+            APX_TRACE_EVENT(p, 5, it_base + it);                                      // clear warp: MMAs of the buffer done
             if (n < kStsClearBelow) {
                 // few ions: the LSU pipe has room, clear with plain stores and spare the L2 the zero traffic
                 uint4 *hp = reinterpret_cast<uint4 *>(smem + (buf ? L.hist1 : L.hist0));
@@ -644,20 +721,23 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         for (int gl = (set ^ sq.grp_base) & 1; gl < sq.ngrp; gl += 2) {
             const int gq = sq.grp_base + gl;
             mbar_wait_lean<200>(&ps.epi[set], (uint32_t)((gq >> 1) & 1));
+            APX_TRACE_EVENT(p, 7, gq);                                                // epilogue start
             asm volatile("tcgen05.fence::after_thread_sync;");
             EpiOut eo;
+            eo.cls = cls; eo.n = n;
             eo.mode = mode; eo.gi = sq.g0 + gl; eo.g0 = sq.g0; eo.f = gl; eo.nfix = sq.nfix;
             eo.flag = kHalf ? &ps.flag[gq & 3] : nullptr; eo.fix = ps.fix;
             epilogue_group<kHalf, NB>(p, tmem + (uint32_t)(set * p.N), eo, m, phase, exch, cand, set, q, lane);
             asm volatile("tcgen05.fence::before_thread_sync;");
             __syncwarp();
+            APX_TRACE_EVENT(p, 8, gq);                                                // epilogue end
             if (lane == 0) mbar_arrive(&ps.tfree[set]);
         }
     }
 }
 
 template <int KS, int NB, bool kHalf>   // KS = K/16 k-steps per group, NB = bin parts (layout), kHalf = half-grid mode
-__global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParams p)
+__global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_constant__ MmaParams p)
 {
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned, still shared-space
@@ -692,9 +772,13 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
     float2 *phase = reinterpret_cast<float2 *>(smem + L.phase);
     constexpr int K = KS * 16;
 
-    // ---- setup: barriers, TMEM, zero histograms, twiddle table, gather ------------------------------
-    if (tid == 0) {
+    // ---- setup: barriers, TMEM, twiddle table ----------------------------------------------------------
+    auto init_barriers = [&](bool again) {
         for (int i = 0; i < 2; ++i) {
+            if (again) {                                   // a new class of signatures restarts the pipeline's phase counts
+                uint64_t *bars[5] = {&s_full[i], &s_done[i], &s_free[i], &s_epi[i], &s_tfree[i]};
+                for (uint64_t *b : bars) asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(b)) : "memory");
+            }
             mbar_init(&s_full[i], kBinWarps);
             mbar_init(&s_done[i], 1);
             mbar_init(&s_free[i], 1);
@@ -704,73 +788,87 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const MmaParam
         asm volatile("fence.mbarrier_init.release.cluster;");
         s_n = 0; s_nfix = 0;
         for (int i = 0; i < 4; ++i) s_flag[i] = 0u;
-    }
+    };
+    if (tid == 0) init_barriers(false);
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "r"(p.tmem_cols));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     {
-        uint4 *h0 = reinterpret_cast<uint4 *>(smem + L.hist0), *h1 = reinterpret_cast<uint4 *>(smem + L.hist1);
-        for (int i = tid; i < (int)(L.hist_bytes / 16); i += kMmaThreads) {
-            h0[i] = make_uint4(0, 0, 0, 0);
-            if (NB == 4) h1[i] = make_uint4(0, 0, 0, 0);
-        }
         uint4 *t = reinterpret_cast<uint4 *>(smem + L.table);
         for (int i = tid; i < K * p.N / 8; i += kMmaThreads) t[i] = p.table[i];
         for (int i = tid; i < NB * p.W; i += kMmaThreads) phase[i] = p.phase[i];
     }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    asm volatile("tcgen05.fence::before_thread_sync;");
-    __syncthreads();
-    asm volatile("tcgen05.fence::after_thread_sync;");
-    const uint32_t tmem = s_tmem;
-    if (g.n_accepted) gather_roi3(p, g, rc, cx, cy, cz, ions, &s_n);
-    __syncthreads();
-    const int n = s_n;
-    if (chunk == 0 && tid == 0 && p.counts) p.counts[m] = (uint32_t)n;
-
     PipeShared ps;
     ps.full = s_full; ps.done = s_done; ps.free_ = s_free; ps.epi = s_epi; ps.tfree = s_tfree;
     ps.flag = s_flag; ps.nfix = &s_nfix; ps.fix = s_fix;
-    int grp_total = 0;                                     // groups run by this CTA (ordinary + fix-up)
-    if (n > p.cap_big) {
-        // too many ions even for ion buffer + second histogram buffer: leave this material point to the FFT kernel
-        if (chunk == 0 && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
-    } else {
-        auto run = [&](const Seq &sq) {
-            if (NB == 8 || n > p.cap) run_pipeline<KS, NB, true, kHalf>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps);
-            else run_pipeline<KS, NB, false, kHalf>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps);
-        };
-        // half-grid mode: sub-ranges of kSubGroups groups, each followed by the fix-up groups of its flagged pairs
-        const int sub = kHalf ? kSubGroups : (g_end - g_begin);
-        bool overflow = false;
-        for (int sg = g_begin; sg < g_end; sg += sub) {
-            Seq sq;
-            sq.mode = 0; sq.g0 = sg; sq.ngrp = min(sub, g_end - sg); sq.grp_base = grp_total; sq.nfix = 0;
-            run(sq);
-            grp_total += sq.ngrp;
-            if (kHalf) {
-                __syncthreads();                           // every epilogue of the sub-range is done, the list is complete
-                const int nf = s_nfix;
-                __syncthreads();
-                if (tid == 0) s_nfix = 0;
-                if (nf > kFixCap) overflow = true;         // pathological input: the FFT kernel redoes this material point
-                sq.mode = 1; sq.nfix = min(nf, kFixCap); sq.ngrp = (sq.nfix + Lay<NB>::G - 1) / Lay<NB>::G; sq.grp_base = grp_total;
-                if (sq.ngrp) run(sq);
-                grp_total += sq.ngrp;
-                __syncthreads();                           // the list is consumed before the next sub-range appends
+    uint32_t tmem = 0;
+    // ---- one pass per class of signatures (specs with the same type mask): gather, then the group pipeline ---------
+    for (int cls = 0; cls < p.ss.n_classes; ++cls) {
+        if (cls > 0) {
+            __syncthreads();                               // the previous class has drained (epilogues done, clears landed)
+            if (tid == 0) init_barriers(true);
+        }
+        {
+            uint4 *h0 = reinterpret_cast<uint4 *>(smem + L.hist0), *h1 = reinterpret_cast<uint4 *>(smem + L.hist1);
+            for (int i = tid; i < (int)(L.hist_bytes / 16); i += kMmaThreads) {
+                h0[i] = make_uint4(0, 0, 0, 0);
+                if (NB == 4) h1[i] = make_uint4(0, 0, 0, 0);
             }
         }
-        if (overflow && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
-        // the bulk copies that clear the buffers after their last use must land before the CTA gives up its shared memory
-        if (warp == kClrWarp && grp_total > 0) {
-            const int npass = n > 2048 ? (n + 2047) / 2048 : 1, items = grp_total * npass;
-            if (NB == 8 || n > p.cap) {
-                // single-buffered: cleared with plain stores by the binning warps, nothing in flight
-            } else {
-                const int u0 = (items + 1) >> 1, u1 = items >> 1;
-                if (u0) mbar_wait(&s_free[0], (uint32_t)((u0 - 1) & 1));
-                if (u1) mbar_wait(&s_free[1], (uint32_t)((u1 - 1) & 1));
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("tcgen05.fence::before_thread_sync;");
+        __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;");
+        tmem = s_tmem;
+        if (g.n_accepted) gather_roi3(p, g, rc, cx, cy, cz, ions, &s_n, cls);
+        __syncthreads();
+        const int n = s_n;
+        if (chunk == 0 && tid == 0 && p.counts)
+            for (int sp = 0; sp < p.ss.n_specs; ++sp)
+                if (p.ss.cls_of[sp] == cls) p.counts[(size_t)sp * p.M + m] = (uint32_t)n;
+
+        int grp_total = 0;                                     // groups run by this CTA for this class (ordinary + fix-up)
+        if (n > p.cap_big) {
+            // too many ions even for ion buffer + second histogram buffer: leave this material point to the FFT kernel
+            if (chunk == 0 && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
+        } else {
+            auto run = [&](const Seq &sq) {
+                if (NB == 8 || n > p.cap) run_pipeline<KS, NB, true, kHalf>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
+                else run_pipeline<KS, NB, false, kHalf>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
+            };
+            // half-grid mode: sub-ranges of kSubGroups groups, each followed by the fix-up groups of its flagged pairs
+            const int sub = kHalf ? kSubGroups : (g_end - g_begin);
+            bool overflow = false;
+            for (int sg = g_begin; sg < g_end; sg += sub) {
+                Seq sq;
+                sq.mode = 0; sq.g0 = sg; sq.ngrp = min(sub, g_end - sg); sq.grp_base = grp_total; sq.nfix = 0;
+                run(sq);
+                grp_total += sq.ngrp;
+                if (kHalf) {
+                    __syncthreads();                           // every epilogue of the sub-range is done, the list is complete
+                    const int nf = s_nfix;
+                    __syncthreads();
+                    if (tid == 0) s_nfix = 0;
+                    if (nf > kFixCap) overflow = true;         // pathological input: the FFT kernel redoes this material point
+                    sq.mode = 1; sq.nfix = min(nf, kFixCap); sq.ngrp = (sq.nfix + Lay<NB>::G - 1) / Lay<NB>::G; sq.grp_base = grp_total;
+                    if (sq.ngrp) run(sq);
+                    grp_total += sq.ngrp;
+                    __syncthreads();                           // the list is consumed before the next sub-range appends
+                }
+            }
+            if (overflow && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
+            // the bulk copies that clear the buffers after their last use must land before the CTA gives up its shared memory
+            // (or re-initialises the barriers for the next class)
+            if (warp == kClrWarp && grp_total > 0) {
+                const int npass = n > 2048 ? (n + 2047) / 2048 : 1, items = grp_total * npass;
+                if (NB == 8 || n > p.cap || n < p.binclear_below) {
+                    // cleared with plain stores by the binning warps, nothing in flight
+                } else {
+                    const int u0 = (items + 1) >> 1, u1 = items >> 1;
+                    if (u0) mbar_wait(&s_free[0], (uint32_t)((u0 - 1) & 1));
+                    if (u1) mbar_wait(&s_free[1], (uint32_t)((u1 - 1) & 1));
+                }
             }
         }
     }
@@ -970,6 +1068,10 @@ cudaError_t mma_path_prepare(Plan *p)
             for (int a = 0; a < 3; ++a) sorted[3 * i + a] = nps[3 * (size_t)src + a];
         }
     }
+    // tuning knobs (development): defaults chosen from measurements, overridable from the environment
+    p->tune_binclear = 0; p->tune_unit_split = 0;
+    if (const char *ev = std::getenv("APX_TUNE_BINCLEAR")) p->tune_binclear = std::atoi(ev);
+    if (const char *ev = std::getenv("APX_TUNE_UNITS")) p->tune_unit_split = std::atoi(ev);
     const int Dp = (int)perm.size();
     p->mma_paired = sym ? 1 : 0;
     p->Dp = Dp;
@@ -1015,9 +1117,10 @@ cudaError_t mma_reserve_for(Plan *p, int64_t M)
 {
     if (M <= 0) return cudaSuccess;
     // M * (nchunks(M) + 1) + 1 is not monotone in M below sm_count * 8 (where nchunks drops to 1): take the maximum
-    int64_t need = M * (mma_nchunks_for(p, M) + 1) + 1;
+    const int64_t nc = p->specs.n_classes;
+    int64_t need = nc * M * (mma_nchunks_for(p, M) + 1) + 1;
     for (int64_t m = 1; m <= std::min<int64_t>(M, (int64_t)p->sm_count * 8); ++m)
-        need = std::max(need, m * (mma_nchunks_for(p, m) + 1) + 1);
+        need = std::max(need, nc * m * (mma_nchunks_for(p, m) + 1) + 1);
     return mma_reserve_deferred(p, need);
 }
 
@@ -1028,7 +1131,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     const int slots_per_group = 128 / mma_nb_for(p->B);
     // deferred list: ROIs too large (<= M) + fix-list overflows (<= 1 per CTA).  Grown here only when apx_plan_reserve
     // has not sized it already (cudaFree / cudaMalloc synchronise the device: reserve first to keep apx_query asynchronous)
-    cudaError_t e = mma_reserve_deferred(p, M * (nchunks + 1) + 1);
+    cudaError_t e = mma_reserve_deferred(p, p->specs.n_classes * M * (nchunks + 1) + 1);
     if (e != cudaSuccess) return e;
     e = cudaMemsetAsync(p->d_deferred, 0, 4, st);
     if (e != cudaSuccess) return e;
@@ -1039,6 +1142,10 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.table = reinterpret_cast<const uint4 *>(p->d_mma_table); q.phase = p->d_mma_phase; q.zeros = p->d_mma_zero;
     q.sig = reinterpret_cast<float2 *>(sig); q.counts = counts; q.deferred = p->d_deferred;
     q.hist_out = p->dbg_hist_out; q.hist_d0 = p->dbg_d0; q.hist_nd = p->dbg_nd;
+#ifdef APX_TRACE
+    q.trace = p->dbg_trace; q.trace_block = p->dbg_trace_block; q.trace_cap = p->dbg_trace_cap;
+#endif
+    q.ss = p->specs;
     q.D = p->D; q.B = p->B; q.k_lo = p->k_lo; q.W = p->W; q.N = mma_n_for(p->W);
     q.nl = 0;
     while ((8 << q.nl) < p->B) ++q.nl;
@@ -1050,6 +1157,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.M = (int)M;
     q.clamp = p->need_clamp;
     q.half = p->mma_paired;
+    q.binclear_below = p->tune_binclear; q.unit_split = p->tune_unit_split;
     uint32_t cols = 32;
     while (cols < (uint32_t)(2 * q.N)) cols *= 2;
     q.tmem_cols = cols;
@@ -1077,7 +1185,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     if (e != cudaSuccess) return e;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    return launch_signature_fft_list(p, centres, p->d_deferred, sig, counts, st);
+    return launch_signature_fft_list(p, centres, p->d_deferred, M, sig, counts, st);
 }
 
 }  // namespace apx

@@ -21,7 +21,7 @@ def lib():
 
 
 def test_every_declared_symbol_is_exported(lib):
-    for header, exports in (("aptsig.h", apx.EXPORTS), ("aptsig_peaks.h", apx.PEAK_EXPORTS)):
+    for header, exports in (("aptsig.h", apx.EXPORTS), ("aptsig_peaks.h", apx.PEAK_EXPORTS), ("aptsig_ext.h", apx.EXT_EXPORTS)):
         hdr = open(os.path.join(ROOT, "include", header)).read()
         hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
         declared = set(re.findall(r"\b(apx_[a-z_0-9]+)\s*\(", hdr))
@@ -99,3 +99,14 @@ def test_binding_argument_checks_host_side():
         with pytest.raises(apx.ApxError) as ei:
             bad()
         assert ei.value.status == apx.APX_EINVAL
+
+
+def test_so3_grid_matches_oracle_grid():
+    """The library's orientation set (host) against the oracle's own construction of reading #23."""
+    from oracle import next_oracle as X
+    for spacing in (10.0, 5.0):
+        a, b = apx.apx_so3_grid_cubic(spacing), X.so3_grid_cubic(spacing)
+        assert a.shape == b.shape
+        np.testing.assert_allclose(a, b, rtol=0, atol=1e-7)
+    with pytest.raises(apx.ApxError):
+        apx.apx_so3_grid_cubic(0.0)

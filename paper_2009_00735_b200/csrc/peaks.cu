@@ -86,22 +86,24 @@ __global__ void __launch_bounds__(kThreads, 1) k_peak(int iters, float seed, flo
         }
     } else {
         // shared-memory loads; results are folded into acc so that every load is live
-        const uint32_t wbase = base + (uint32_t)warp * 12u * 128u;
+        // (loads may reach into the rows of the following warps: wrap the warp's base so that everything stays inside sm[])
+        const uint32_t wbase = base + (uint32_t)(warp % 26) * 12u * 128u;
         for (int it = 0; it < iters; ++it) {
 #pragma unroll
             for (int u = 0; u < kUnroll; ++u) {
-                const uint32_t row = (uint32_t)(u % 6) * 128u;
+                // sixteen DIFFERENT addresses per loop body: identical asm statements would be merged by the compiler
                 if (TEST == APX_PEAK_LDS32_BROADCAST || TEST == APX_PEAK_LDS32_CONFLICT_FREE) {
-                    const uint32_t off = TEST == APX_PEAK_LDS32_BROADCAST ? row : row + (uint32_t)lane * 4u;
+                    const uint32_t off = TEST == APX_PEAK_LDS32_BROADCAST ? (uint32_t)u * 4u : (uint32_t)(u % 12) * 128u + (uint32_t)lane * 4u + (uint32_t)(u / 12) * 1536u;
                     float v;
                     asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(wbase + off) : "memory");
                     acc += v;
                 } else {
                     uint32_t off;
+                    const uint32_t row = (uint32_t)u * 64u;                                              // 16 rows of 64 B
                     if (TEST == APX_PEAK_LDS128_BROADCAST_1) off = row;                                   // one address per warp
                     else if (TEST == APX_PEAK_LDS128_BROADCAST_2) off = row + (uint32_t)(lane >> 4) * 16u;     // two (half-warps)
                     else if (TEST == APX_PEAK_LDS128_BROADCAST_4) off = row + (uint32_t)(lane >> 3) * 16u;     // four (quarter-warps)
-                    else off = (uint32_t)(u % 3) * 512u + (uint32_t)lane * 16u;                          // 512 B per instruction
+                    else off = (uint32_t)(u % 3) * 512u + (uint32_t)lane * 16u + (uint32_t)(u / 3) * 1536u;    // 512 B per instruction
                     float x, y, z, w;
                     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(wbase + off) : "memory");
                     acc += x + y + z + w;

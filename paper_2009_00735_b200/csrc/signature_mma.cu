@@ -74,14 +74,14 @@ __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)_
 // Development aid (build with -DAPX_TRACE): lane 0 of selected warps of ONE CTA appends (event, group, SM clock) records to a
 // global buffer, which shows the timeline of the warp-specialised pipeline.  Compiled out otherwise.
 #ifdef APX_TRACE
+// per-warp regions of trace_cap records each, index kept in a register (trace_n of run_pipeline): two plain stores per
+// event, no atomics, nothing to wait for -- the timeline is not disturbed
 #define APX_TRACE_EVENT(p, ev, grp)                                                                   \
     do {                                                                                              \
-        if ((p).trace && blockIdx.x == (unsigned)(p).trace_block && (threadIdx.x & 31) == 0) {        \
-            const unsigned long long i__ = atomicAdd((unsigned long long *)(p).trace, 1ull);          \
-            if (i__ < (unsigned long long)(p).trace_cap) {                                            \
-                (p).trace[1 + 2 * i__] = ((long long)(ev) << 48) | ((long long)(threadIdx.x >> 5) << 32) | (long long)(grp); \
-                (p).trace[2 + 2 * i__] = clock64();                                                   \
-            }                                                                                         \
+        if ((p).trace && blockIdx.x == (unsigned)(p).trace_block && (threadIdx.x & 31) == 0 && trace_n < (p).trace_cap) { \
+            long long *r__ = (p).trace + 2 * ((long long)(threadIdx.x >> 5) * (p).trace_cap + trace_n++);       \
+            r__[0] = ((long long)(ev) << 48) | ((long long)(threadIdx.x >> 5) << 32) | (long long)(grp) | (1ll << 62); \
+            r__[1] = clock64();                                                                       \
         }                                                                                             \
     } while (0)
 #else
@@ -177,6 +177,8 @@ struct MmaParams {
     int half;                  // 1 = half-grid mode: one direction per antipodal pair is binned (perm_mirror != nullptr)
     SpecSet ss;                // signatures of the plan: classes (type masks), per-spec sub-windows of [k_lo, k_lo + W)
     int binclear_below;        // double-buffered ROIs with fewer ions: the binning warps clear the buffers themselves
+    int prefetch;              // 1 = binning warps load the next group's directions while they bin the current one
+    int quiet;                 // 1 = quiet signalling: hardware barriers / a single polling warp instead of many mbarrier waiters
     int unit_split;            // 1 = ions are dealt to the binning warps in whole blocks of 4 * NS (no ragged tails)
     uint32_t tmem_cols;
     float R, R2;
@@ -298,11 +300,13 @@ __device__ __noinline__ void flag_pair(uint32_t *flag, int *nfix, uint16_t *fix,
     }
 }
 // two ions (dx0,dx1), (dy0,dy1), (dz0,dz1) for this lane's direction
-// returns (only with kDetect) the number of the two projections that are NOT exact integers
+// kDetect: nonint2 (packed fp32 pair) accumulates, per component, the number of projections that are NOT exact integers:
+// RU(x + magic) - RD(x + magic) is exactly 1.0f for a non-integer x and 0.0f for an integer (adjacent floats with ulp 1), so
+// the test costs three packed FP instructions per two ions and no integer work.
 template <bool kDetect, int BLK>
-__device__ __forceinline__ uint32_t bin_pair(float dx0, float dx1, float dy0, float dy1, float dz0, float dz1, uint64_t nx2,
+__device__ __forceinline__ void bin_pair(float dx0, float dx1, float dy0, float dy1, float dz0, float dz1, uint64_t nx2,
                                          uint64_t ny2, uint64_t nz2, uint64_t ma2, uint64_t sc2, uint64_t mb2, uint32_t kz,
-                                         uint32_t k0, uint32_t inc, const Detect &dt)
+                                         uint32_t k0, uint32_t inc, uint64_t &nonint2)
 {
     uint64_t t, ua, va;
     asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(t) : "l"(nx2), "l"(pack2(dx0, dx1)));
@@ -313,12 +317,18 @@ __device__ __forceinline__ uint32_t bin_pair(float dx0, float dx1, float dy0, fl
     const uint32_t ua0 = (uint32_t)ua, ua1 = (uint32_t)(ua >> 32), va0 = (uint32_t)va, va1 = (uint32_t)(va >> 32);
     red_shared_add(ua0 * (uint32_t)BLK + (va0 * kz + k0), inc);
     red_shared_add(ua1 * (uint32_t)BLK + (va1 * kz + k0), inc);
-    if (kDetect) {                                       // RU(x + magic) - RD(x + magic) = 1, or 0 for an integer x
-        uint64_t up;
+    if (kDetect) {
+        uint64_t up, d;
         asm("add.rp.f32x2 %0, %1, %2;" : "=l"(up) : "l"(t), "l"(ma2));
-        return ((uint32_t)up - ua0) + ((uint32_t)(up >> 32) - ua1);
+        asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(up), "l"(ua));              // exact: (0 or 1, 0 or 1)
+        asm("add.rn.f32x2 %0, %1, %2;" : "=l"(nonint2) : "l"(nonint2), "l"(d));
     }
-    return 0u;
+}
+__device__ __forceinline__ float sum2(uint64_t v)
+{
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+    return lo + hi;
 }
 
 // One direction pair of a lane: set A (low u16, increment 1) and set B (high u16, increment 65536) of the same word.
@@ -343,31 +353,31 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
             float4 q[6];
 #pragma unroll
             for (int u = 0; u < 6; ++u) q[u] = lds128(src + (uint32_t)u * 16u);
-            uint32_t na = 0u, nb = 0u;
+            uint64_t na = 0ull, nb = 0ull;                    // packed (0.0f, 0.0f)
 #pragma unroll
             for (int hh = 0; hh < 2; ++hh) {
                 const float4 X = q[3 * hh], Y = q[3 * hh + 1], Z = q[3 * hh + 2];
-                na += bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
-                na += bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
-                nb += bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
-                nb += bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
+                bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, na);
+                bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, na);
+                bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, nb);
+                bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, nb);
             }
             if (kDetect) {
-                if (__builtin_expect(na != 8u, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
-                if (__builtin_expect(nb != 8u, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
+                if (__builtin_expect(sum2(na) != 8.0f, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
+                if (__builtin_expect(sum2(nb) != 8.0f, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
             }
         }
         if (ib + 4 * NS <= i1) {                             // one quad per stream
             const uint32_t a = ions_s + (uint32_t)ib * 12u + (uint32_t)h * 48u;
             const float4 X = lds128(a), Y = lds128(a + 16u), Z = lds128(a + 32u);
-            uint32_t na = 0u, nb = 0u;
-            na += bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
-            na += bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, da);
-            nb += bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
-            nb += bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, db);
+            uint64_t na = 0ull, nb = 0ull;
+            bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, na);
+            bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, na);
+            bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, nb);
+            bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, nb);
             if (kDetect) {
-                if (__builtin_expect(na != 4u, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
-                if (__builtin_expect(nb != 4u, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
+                if (__builtin_expect(sum2(na) != 4.0f, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
+                if (__builtin_expect(sum2(nb) != 4.0f, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
             }
             ib += 4 * NS;
         }
@@ -576,6 +586,9 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
     const int mode = kHalf ? sq.mode : 0;
     const int it_base = sq.grp_base * npass;
     const bool binclr = !kBig && n < p.binclear_below;
+#ifdef APX_TRACE
+    int trace_n = sq.grp_base == 0 && sq.mode == 0 && cls == 0 ? 0 : (1 << 30);      // the CTA's first sequence only
+#endif
     if (warp < kBinWarps) {
         BinConst c;
         c.half_b = (float)(p.B / 2); c.magic_a = magic_for(p.B); c.magic_b = 12582912.0f + 4.0f;
@@ -587,42 +600,60 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                                 - 0x4B400000u * (uint32_t)Lay<NB>::BLK - 0x4B400000u * c.kz;
         const uint32_t ions_s = smem_u32(ions);
         const bool detect = kHalf && mode == 0;
-        for (int it = 0, gl = 0, pass = 0; it < nitems; ++it) {
-            const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
+        auto load_dirs = [&](int g_idx) {
             LaneDirs n;
             if (mode == 0) {
-                const float *da = p.dirs_sorted + (size_t)((sq.g0 + gl) * G + l) * 3;
+                const float *da = p.dirs_sorted + (size_t)((sq.g0 + g_idx) * G + l) * 3;
                 n.ax = da[0]; n.ay = da[1]; n.az = da[2]; n.bx = da[3 * LW]; n.by = da[3 * LW + 1]; n.bz = da[3 * LW + 2];
             } else {                                                     // the opposite of a flagged pair's direction
-                const int ea = gl * G + l, eb = ea + LW;
+                const int ea = g_idx * G + l, eb = ea + LW;
                 const float *da = p.dirs_sorted + (ea < sq.nfix ? (size_t)(sq.g0 * G + (int)ps.fix[ea]) * 3 : 0);
                 const float *db = p.dirs_sorted + (eb < sq.nfix ? (size_t)(sq.g0 * G + (int)ps.fix[eb]) * 3 : 0);
                 n.ax = -da[0]; n.ay = -da[1]; n.az = -da[2]; n.bx = -db[0]; n.by = -db[1]; n.bz = -db[2];
             }
+            return n;
+        };
+        LaneDirs n_next;
+        n_next.ax = n_next.ay = n_next.az = n_next.bx = n_next.by = n_next.bz = 0.f;
+        for (int it = 0, gl = 0, pass = 0; it < nitems; ++it) {
+            const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
+            // this item's directions; those of the NEXT group are requested before the binning of this one starts (below), so
+            // that their L2 latency (~700 clk) is not part of every group's serial path
+            LaneDirs n;
+            if (p.prefetch && it > 0) n = n_next;
+            else n = load_dirs(gl);
             APX_TRACE_EVENT(p, 0, sq.grp_base + gl);                                 // binning warp ready for the item
-            if (kBig) {
-                // single-buffered: the shared-memory pipe is idle while the tensor core transforms the buffer, so the 16
-                // binning warps clear it themselves as soon as it has been read (a few STS.128 per thread)
-                if (use >= 1) {
-                    mbar_wait(&ps.done[0], (uint32_t)((use - 1) & 1));
-                    uint4 *hb = reinterpret_cast<uint4 *>(smem + L.hist0);
-                    for (int i = tid; i < (int)(L.hist_bytes / 16); i += kBinWarps * 32) hb[i] = make_uint4(0, 0, 0, 0);
+            // Before the item: the buffer must be clear again after its previous use.
+            //   double-buffered, many ions : the clear warp's bulk copies of zeros complete on free[buf]
+            //   double-buffered, few ions  : (binclr) a group is binned long before the tensor core needs the other buffer
+            //                                back, so the chain transform -> clear warp -> free only adds latency: the 16
+            //                                binning warps clear the buffer themselves once its MMAs have completed (done[buf])
+            //   single-buffered (kBig)     : the shared-memory pipe is idle while the tensor core transforms the buffer, the
+            //                                binning warps clear it as soon as it has been read (done[0])
+            // Quiet signalling: only warp 0 polls the mbarrier, the other 15 block on a hardware barrier -- every waiter on an
+            // mbarrier is woken by every update of it (each bulk-copy chunk, each arrival) and burns issue slots re-checking.
+            if (use >= 1) {
+                const bool self_clear = kBig || binclr;
+                uint64_t *wbar = self_clear ? &ps.done[buf] : &ps.free_[buf];
+                if (p.quiet) {
+                    if (warp == 0) mbar_wait(wbar, (uint32_t)((use - 1) & 1));
                     asm volatile("bar.sync 5, %0;" ::"n"(kBinWarps * 32) : "memory");
+                } else if (self_clear) {
+                    mbar_wait(wbar, (uint32_t)((use - 1) & 1));
+                } else {
+                    mbar_wait_lean(wbar, (uint32_t)((use - 1) & 1));
                 }
-            } else if (binclr) {
-                // few ions: a group is binned long before the tensor core needs the other buffer back, so the chain
-                // transform -> clear warp -> free only adds latency; the 16 binning warps clear the buffer themselves
-                // (10 STS.128 per thread) as soon as its MMAs have completed
-                if (use >= 1) {
-                    mbar_wait(&ps.done[buf], (uint32_t)((use - 1) & 1));
+                if (self_clear) {
                     uint4 *hb = reinterpret_cast<uint4 *>(smem + (buf ? L.hist1 : L.hist0));
                     for (int i = tid; i < (int)(L.hist_bytes / 16); i += kBinWarps * 32) hb[i] = make_uint4(0, 0, 0, 0);
                     asm volatile("bar.sync 5, %0;" ::"n"(kBinWarps * 32) : "memory");
                 }
-            } else if (use >= 1) {
-                mbar_wait_lean(&ps.free_[buf], (uint32_t)((use - 1) & 1));             // cleared after its previous use
             }
             APX_TRACE_EVENT(p, 1, sq.grp_base + gl);                                 // bin start (buffer free)
+            if (p.prefetch && it + 1 < nitems) {
+                const int gl_next = (pass + 1 == npass) ? gl + 1 : gl;
+                n_next = gl_next == gl ? n : load_dirs(gl_next);
+            }
             const int a0 = pass * 2048, a1 = min(n_ions, a0 + 2048);
             int i0, i1;
             if (p.unit_split) {                                                      // whole blocks of 4 * NS ions per warp
@@ -649,7 +680,14 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
             __syncwarp();
             APX_TRACE_EVENT(p, 2, sq.grp_base + gl);                                 // bin end
-            if (lane == 0) mbar_arrive(&ps.full[buf]);
+            // buffer full -> MMA warp: a hardware barrier (16 binning warps arrive, the MMA warp syncs) or, in the old
+            // scheme, 16 arrivals on an mbarrier the MMA warp polls
+            if (p.quiet) {
+                if (buf) asm volatile("bar.arrive 7, %0;" ::"n"(kBinWarps * 32 + 32) : "memory");
+                else asm volatile("bar.arrive 6, %0;" ::"n"(kBinWarps * 32 + 32) : "memory");
+            } else if (lane == 0) {
+                mbar_arrive(&ps.full[buf]);
+            }
             if (++pass == npass) { pass = 0; ++gl; }
         }
     } else if (warp == kMmaWarp) {
@@ -664,7 +702,12 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         for (int it = 0, gl = 0, pass = 0; it < nitems; ++it) {
             const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
             const int gq = sq.grp_base + gl;
-            mbar_wait<100>(&ps.full[buf], (uint32_t)(use & 1));
+            if (p.quiet) {
+                if (buf) asm volatile("bar.sync 7, %0;" ::"n"(kBinWarps * 32 + 32) : "memory");
+                else asm volatile("bar.sync 6, %0;" ::"n"(kBinWarps * 32 + 32) : "memory");
+            } else {
+                mbar_wait<100>(&ps.full[buf], (uint32_t)(use & 1));
+            }
             APX_TRACE_EVENT(p, 3, gq);                                                // MMA warp: buffer full
             if (pass == 0 && gq >= 2) mbar_wait(&ps.tfree[gq & 1], (uint32_t)(((gq >> 1) - 1) & 1));
             APX_TRACE_EVENT(p, 4, gq);                                                // accumulator free, MMAs issued next
@@ -720,7 +763,12 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         const int q = warp & 3, set = (warp - kSvcWarp0) >> 2;
         for (int gl = (set ^ sq.grp_base) & 1; gl < sq.ngrp; gl += 2) {
             const int gq = sq.grp_base + gl;
-            mbar_wait_lean<200>(&ps.epi[set], (uint32_t)((gq >> 1) & 1));
+            if (p.quiet) {                                                           // one warp polls, three block in hardware
+                if (q == 0) mbar_wait<200>(&ps.epi[set], (uint32_t)((gq >> 1) & 1));
+                if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
+            } else {
+                mbar_wait_lean<200>(&ps.epi[set], (uint32_t)((gq >> 1) & 1));
+            }
             APX_TRACE_EVENT(p, 7, gq);                                                // epilogue start
             asm volatile("tcgen05.fence::after_thread_sync;");
             EpiOut eo;
@@ -731,7 +779,12 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             asm volatile("tcgen05.fence::before_thread_sync;");
             __syncwarp();
             APX_TRACE_EVENT(p, 8, gq);                                                // epilogue end
-            if (lane == 0) mbar_arrive(&ps.tfree[set]);
+            if (p.quiet) {                                                           // all four warps have read the accumulator
+                if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
+                if (q == 0 && lane == 0) mbar_arrive(&ps.tfree[set]);
+            } else if (lane == 0) {
+                mbar_arrive(&ps.tfree[set]);
+            }
         }
     }
 }
@@ -783,7 +836,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
             mbar_init(&s_done[i], 1);
             mbar_init(&s_free[i], 1);
             mbar_init(&s_epi[i], 1);
-            mbar_init(&s_tfree[i], 4);
+            mbar_init(&s_tfree[i], p.quiet ? 1 : 4);
         }
         asm volatile("fence.mbarrier_init.release.cluster;");
         s_n = 0; s_nfix = 0;
@@ -1069,7 +1122,9 @@ cudaError_t mma_path_prepare(Plan *p)
         }
     }
     // tuning knobs (development): defaults chosen from measurements, overridable from the environment
-    p->tune_binclear = 0; p->tune_unit_split = 0;
+    p->tune_binclear = 0; p->tune_unit_split = 0; p->tune_quiet = 0; p->tune_prefetch = 0;
+    if (const char *ev = std::getenv("APX_TUNE_PREFETCH")) p->tune_prefetch = std::atoi(ev);
+    if (const char *ev = std::getenv("APX_TUNE_QUIET")) p->tune_quiet = std::atoi(ev);
     if (const char *ev = std::getenv("APX_TUNE_BINCLEAR")) p->tune_binclear = std::atoi(ev);
     if (const char *ev = std::getenv("APX_TUNE_UNITS")) p->tune_unit_split = std::atoi(ev);
     const int Dp = (int)perm.size();
@@ -1157,7 +1212,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.M = (int)M;
     q.clamp = p->need_clamp;
     q.half = p->mma_paired;
-    q.binclear_below = p->tune_binclear; q.unit_split = p->tune_unit_split;
+    q.binclear_below = p->tune_binclear; q.unit_split = p->tune_unit_split; q.quiet = p->tune_quiet; q.prefetch = p->tune_prefetch;
     uint32_t cols = 32;
     while (cols < (uint32_t)(2 * q.N)) cols *= 2;
     q.tmem_cols = cols;

@@ -31,7 +31,11 @@ enum {
     APX_PEAK_LDS128_CONFLICT_FREE = 11,/* ... 32 consecutive 16-byte words = 512 B per instruction            */
     APX_PEAK_RED_INC_CONFLICT_FREE = 12,/* red.shared.add.u32 of the literal 1 (ATOMS.POPC.INC), 32 banks; tests 2-5 add a
                                           register value (ATOMS.ADD)                                             */
-    APX_PEAK_COUNT = 13
+    APX_PEAK_RED_SCATTERED_CONFLICT_FREE = 13, /* 32 different banks, every lane in a different 128-byte row: the access
+                                          pattern of project-and-bin (a lane's row is its bin), the roofline denominator   */
+    APX_PEAK_RED_SCATTERED_HALVES = 14,/* the kernel's bank map: lanes 0-15 on banks {0-3,8-11,16-19,24-27}, lanes 16-31 on
+                                          the other sixteen, rows scattered                                           */
+    APX_PEAK_COUNT = 15
 };
 
 typedef struct {

@@ -20,7 +20,7 @@ constexpr int kSmemWords = 12288;          // 48 KB of shared memory: 384 rows o
 __device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 template <int TEST>
-__global__ void __launch_bounds__(kThreads, 1) k_peak(int iters, float seed, float *sink, long long *cycles)
+__global__ void __launch_bounds__(kThreads, 1) k_peak(int iters, float seed, int zero, float *sink, long long *cycles)
 {
     __shared__ __align__(16) uint32_t sm[kSmemWords];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -63,7 +63,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_peak(int iters, float seed, flo
             asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a[u]));
             acc += lo + hi;
         }
-    } else if ((TEST >= APX_PEAK_RED_CONFLICT_FREE && TEST <= APX_PEAK_RED_RANDOM_BANK) || TEST == APX_PEAK_RED_INC_CONFLICT_FREE) {
+    } else if ((TEST >= APX_PEAK_RED_CONFLICT_FREE && TEST <= APX_PEAK_RED_RANDOM_BANK) || TEST == APX_PEAK_RED_INC_CONFLICT_FREE ||
+               TEST == APX_PEAK_RED_SCATTERED_CONFLICT_FREE || TEST == APX_PEAK_RED_SCATTERED_HALVES) {
         // shared-memory reduction atomics without return value (the binning instruction); every warp works on its own
         // 12 rows of 32 words so that warps never share an address
         // increment from a kernel argument -> ATOMS.ADD (the high-u16 counters' 65536); the literal 1 of the INC test
@@ -79,6 +80,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_peak(int iters, float seed, flo
                 if (TEST == APX_PEAK_RED_CONFLICT_FREE || TEST == APX_PEAK_RED_INC_CONFLICT_FREE) off = row * 128u + (uint32_t)lane * 4u;   // 32 banks
                 else if (TEST == APX_PEAK_RED_2WAY) off = (2u * row + (uint32_t)(lane >> 4)) * 128u + (uint32_t)(lane & 15) * 4u;
                 else if (TEST == APX_PEAK_RED_SAME_ADDRESS) off = row * 128u;
+                // 32 different banks, but every lane in a different 128-byte row (the binning pattern: a lane's row is its bin)
+                else if (TEST == APX_PEAK_RED_SCATTERED_CONFLICT_FREE) off = (((uint32_t)lane * 5u + (uint32_t)u) % 12u) * 128u + (uint32_t)lane * 4u;
+                // the kernel's layout: lanes 0-15 on the 16 banks {0-3, 8-11, 16-19, 24-27}, lanes 16-31 on the other 16, rows scattered
+                else if (TEST == APX_PEAK_RED_SCATTERED_HALVES)
+                    off = (((uint32_t)lane * 5u + (uint32_t)u) % 12u) * 128u + ((uint32_t)(lane & 3) + 8u * (uint32_t)((lane >> 2) & 3) + 4u * (uint32_t)(lane >> 4)) * 4u;
                 else { lcg = lcg * 1664525u + 1013904223u; off = ((lcg >> 10) % (12u * 32u)) * 4u; }            // random word
                 if (TEST == APX_PEAK_RED_INC_CONFLICT_FREE) asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(wbase + off) : "memory");
                 else asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(wbase + off), "r"(inc) : "memory");
@@ -87,8 +93,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_peak(int iters, float seed, flo
     } else {
         // shared-memory loads; results are folded into acc so that every load is live
         // (loads may reach into the rows of the following warps: wrap the warp's base so that everything stays inside sm[])
-        const uint32_t wbase = base + (uint32_t)(warp % 26) * 12u * 128u;
+        // `zero` is a kernel argument that is 0 at run time: making the address formally depend on the iteration keeps the
+        // compiler from hoisting the (loop-invariant) loads out of the timed loop
+        const uint32_t wbase0 = base + (uint32_t)(warp % 26) * 12u * 128u;
         for (int it = 0; it < iters; ++it) {
+            const uint32_t wbase = wbase0 + (uint32_t)(it * zero);
 #pragma unroll
             for (int u = 0; u < kUnroll; ++u) {
                 // sixteen DIFFERENT addresses per loop body: identical asm statements would be merged by the compiler
@@ -125,9 +134,9 @@ cudaError_t run_test(int blocks, int iters, float *sink, long long *cycles, floa
     if (e != cudaSuccess) return e;
     e = cudaEventCreate(&b);
     if (e != cudaSuccess) return e;
-    k_peak<TEST><<<blocks, kThreads>>>(iters / 8 + 1, 1.0f, sink, cycles);      // warm-up
+    k_peak<TEST><<<blocks, kThreads>>>(iters / 8 + 1, 1.0f, 0, sink, cycles);      // warm-up
     cudaEventRecord(a);
-    k_peak<TEST><<<blocks, kThreads>>>(iters, 1.0f, sink, cycles);
+    k_peak<TEST><<<blocks, kThreads>>>(iters, 1.0f, 0, sink, cycles);
     cudaEventRecord(b);
     e = cudaEventSynchronize(b);
     if (e == cudaSuccess) e = cudaGetLastError();
@@ -155,6 +164,8 @@ extern "C" const char *apx_peak_name(int test)
         case APX_PEAK_LDS128_BROADCAST_4: return "lds128_broadcast_4_addresses";
         case APX_PEAK_LDS128_CONFLICT_FREE: return "lds128_conflict_free";
         case APX_PEAK_RED_INC_CONFLICT_FREE: return "red_shared_inc_conflict_free";
+        case APX_PEAK_RED_SCATTERED_CONFLICT_FREE: return "red_shared_scattered_rows_conflict_free";
+        case APX_PEAK_RED_SCATTERED_HALVES: return "red_shared_scattered_rows_half_warp_banks";
         default: return nullptr;
     }
 }
@@ -178,7 +189,8 @@ extern "C" int apx_peak_measure(int device, int test, int iters, apx_peak_result
             CASE(APX_PEAK_FFMA) CASE(APX_PEAK_FFMA2) CASE(APX_PEAK_RED_CONFLICT_FREE) CASE(APX_PEAK_RED_2WAY)
             CASE(APX_PEAK_RED_SAME_ADDRESS) CASE(APX_PEAK_RED_RANDOM_BANK) CASE(APX_PEAK_LDS32_BROADCAST)
             CASE(APX_PEAK_LDS32_CONFLICT_FREE) CASE(APX_PEAK_LDS128_BROADCAST_1) CASE(APX_PEAK_LDS128_BROADCAST_2)
-            CASE(APX_PEAK_LDS128_BROADCAST_4) CASE(APX_PEAK_LDS128_CONFLICT_FREE) CASE(APX_PEAK_RED_INC_CONFLICT_FREE)
+            CASE(APX_PEAK_LDS128_BROADCAST_4) CASE(APX_PEAK_LDS128_CONFLICT_FREE) CASE(APX_PEAK_RED_INC_CONFLICT_FREE) CASE(APX_PEAK_RED_SCATTERED_CONFLICT_FREE)
+            CASE(APX_PEAK_RED_SCATTERED_HALVES)
 #undef CASE
         }
     }

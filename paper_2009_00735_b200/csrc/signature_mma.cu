@@ -176,9 +176,9 @@ struct MmaParams {
     int D, B, nl, k_lo, W, N, cap, cap_big, nchunks, ngroups, clamp, M;
     int half;                  // 1 = half-grid mode: one direction per antipodal pair is binned (perm_mirror != nullptr)
     SpecSet ss;                // signatures of the plan: classes (type masks), per-spec sub-windows of [k_lo, k_lo + W)
-    int binclear_below;        // double-buffered ROIs with fewer ions: the binning warps clear the buffers themselves
-    int prefetch;              // 1 = binning warps load the next group's directions while they bin the current one
-    int quiet;                 // 1 = quiet signalling: hardware barriers / a single polling warp instead of many mbarrier waiters
+    int nacc, nacc_log2;       // TMEM accumulators (2 or 4): group gq uses accumulator gq & (nacc - 1), so the MMAs of a group
+                               // wait for the epilogue of group gq - nacc only
+    int lanemap;               // 1 (NB = 4): all lanes of a warp bin the same ions, half-warps = sets A / B (bin_ions_one)
     int unit_split;            // 1 = ions are dealt to the binning warps in whole blocks of 4 * NS (no ragged tails)
     uint32_t tmem_cols;
     float R, R2;
@@ -283,6 +283,10 @@ __device__ __forceinline__ void bin_one(float dx, float dy, float dz, float npx,
 // histogram of v and has the same amplitude spectrum.  x is an integer exactly when rounding x + magic down and up gives
 // the same number; a pair for which that happens for any ion (~1e-5 of all (ion, direction) pairs) is flagged, its -v
 // member gets no output from this group and is binned on its own in a fix-up group.
+// flag words in flight: the binning warps run at most nacc + 1 groups ahead of the epilogue that reads and resets a group's
+// word (bin(g + nacc + 2) needs the buffer back from the MMAs of g + nacc, which wait for the epilogue of g): 8 slots for up to
+// four accumulators
+constexpr int kFlagSlots = 8;
 constexpr int kFixCap = 512;             // flagged pairs per sub-range of kSubGroups groups
 constexpr int kSubGroups = 128;
 struct Detect {
@@ -390,6 +394,55 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(a + 32u));
         bin_one<kClamp, kDetect, BLK>(dx, dy, dz, n.ax, n.ay, n.az, c, k0, 1u, da.flag, da.nfix, da.fix, da.bit, da.id);
         bin_one<kClamp, kDetect, BLK>(dx, dy, dz, n.bx, n.by, n.bz, c, k0, 65536u, db.flag, db.nfix, db.fix, db.bit, db.id);
+    }
+}
+
+// The same step with the other lane map (NB = 4 only): all 32 lanes of a warp work on the SAME ions; lane l < 16 bins them
+// for direction l of set A (low u16, +1), lane l >= 16 for direction l - 16 of set B (high u16, +65536).  Set B is the patch
+// antipodal to set A, so for one ion hi3(B) = 7 - hi3(A): the two half-warps of one shared atomic always fall on the two
+// different bank halves -- conflict-free by construction instead of by the luck of two unrelated ions (measured 1.9
+// wavefronts per ATOMS before).  One ion load now serves 32 instead of 64 pairs; at 2.3 clk per broadcast LDS.128 against
+// 1.9 -> ~1.1 clk per ATOMS this lowers the shared-memory time per pair from 0.144 to ~0.09 clk.
+template <bool kClamp, bool kDetect, int BLK>
+__device__ __forceinline__ void bin_ions_one(uint32_t ions_s, int i0, int i1, float nx, float ny, float nz, const BinConst &c,
+                                             uint32_t k0, uint32_t inc, const Detect &dt)
+{
+    int ib = i0;
+    if (!kClamp) {
+        const uint64_t nx2 = pack2(nx, nx), ny2 = pack2(ny, ny), nz2 = pack2(nz, nz);
+        const uint64_t ma2 = pack2(c.magic_a, c.magic_a), sc2 = pack2(c.scl, c.scl), mb2 = pack2(c.magic_b, c.magic_b);
+        uint32_t src = ions_s + (uint32_t)ib * 12u;
+#pragma unroll 2
+        for (; ib + 8 <= i1; ib += 8, src += 96u) {          // 8 ions = 6 LDS.128 (one address per warp), 4 packed chains
+            float4 q[6];
+#pragma unroll
+            for (int u = 0; u < 6; ++u) q[u] = lds128(src + (uint32_t)u * 16u);
+            uint64_t nn = 0ull;
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {
+                const float4 X = q[3 * hh], Y = q[3 * hh + 1], Z = q[3 * hh + 2];
+                bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc, nn);
+                bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc, nn);
+            }
+            if (kDetect && __builtin_expect(sum2(nn) != 8.0f, 0)) flag_pair(dt.flag, dt.nfix, dt.fix, dt.bit, dt.id);
+        }
+        if (ib + 4 <= i1) {                                  // one quad
+            const uint32_t a = ions_s + (uint32_t)ib * 12u;
+            const float4 X = lds128(a), Y = lds128(a + 16u), Z = lds128(a + 32u);
+            uint64_t nn = 0ull;
+            bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc, nn);
+            bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc, nn);
+            if (kDetect && __builtin_expect(sum2(nn) != 4.0f, 0)) flag_pair(dt.flag, dt.nfix, dt.fix, dt.bit, dt.id);
+            ib += 4;
+        }
+    }
+    for (int i = ib; i < i1; ++i) {                          // ragged tail (and every ion when the clamp is needed)
+        const uint32_t a = ions_s + (uint32_t)(i >> 2) * 48u + (uint32_t)(i & 3) * 4u;
+        float dx, dy, dz;
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dx) : "r"(a));
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dy) : "r"(a + 16u));
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(a + 32u));
+        bin_one<kClamp, kDetect, BLK>(dx, dy, dz, nx, ny, nz, c, k0, inc, dt.flag, dt.nfix, dt.fix, dt.bit, dt.id);
     }
 }
 
@@ -577,7 +630,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
     //   binning warps 0..15 : wait free(buf) -> project-and-bin the item -> arrive full(buf)
     //   MMA warp 16         : wait full(buf) [, tfree(acc)] -> K/16 tcgen05.mma -> commit to done(buf) [, epi(acc)]
     //   clear warp 17       : wait done(buf) -> clear the buffer -> free(buf)
-    //   service warps 18..25: set s = gq & 1: wait epi(acc) -> epilogue from TMEM -> arrive tfree(acc)
+    //   service warps 18..25: set s = gq & 1: wait epi(acc) -> epilogue from TMEM -> arrive tfree(acc), acc = gq & (nacc - 1)
     // A ROI with more than `cap` ions has spilled into the second histogram buffer: it runs with buffer 0 only
     // (bin -> transform -> clear serial per item); `use` counts the uses of a buffer.
     const int n = n_ions;
@@ -585,7 +638,6 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
     const int nitems = sq.ngrp * npass;
     const int mode = kHalf ? sq.mode : 0;
     const int it_base = sq.grp_base * npass;
-    const bool binclr = !kBig && n < p.binclear_below;
 #ifdef APX_TRACE
     int trace_n = sq.grp_base == 0 && sq.mode == 0 && cls == 0 ? 0 : (1 << 30);      // the CTA's first sequence only
 #endif
@@ -600,64 +652,37 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                                 - 0x4B400000u * (uint32_t)Lay<NB>::BLK - 0x4B400000u * c.kz;
         const uint32_t ions_s = smem_u32(ions);
         const bool detect = kHalf && mode == 0;
-        auto load_dirs = [&](int g_idx) {
+        for (int it = 0, gl = 0, pass = 0; it < nitems; ++it) {
+            const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
             LaneDirs n;
             if (mode == 0) {
-                const float *da = p.dirs_sorted + (size_t)((sq.g0 + g_idx) * G + l) * 3;
+                const float *da = p.dirs_sorted + (size_t)((sq.g0 + gl) * G + l) * 3;
                 n.ax = da[0]; n.ay = da[1]; n.az = da[2]; n.bx = da[3 * LW]; n.by = da[3 * LW + 1]; n.bz = da[3 * LW + 2];
             } else {                                                     // the opposite of a flagged pair's direction
-                const int ea = g_idx * G + l, eb = ea + LW;
+                const int ea = gl * G + l, eb = ea + LW;
                 const float *da = p.dirs_sorted + (ea < sq.nfix ? (size_t)(sq.g0 * G + (int)ps.fix[ea]) * 3 : 0);
                 const float *db = p.dirs_sorted + (eb < sq.nfix ? (size_t)(sq.g0 * G + (int)ps.fix[eb]) * 3 : 0);
                 n.ax = -da[0]; n.ay = -da[1]; n.az = -da[2]; n.bx = -db[0]; n.by = -db[1]; n.bz = -db[2];
             }
-            return n;
-        };
-        LaneDirs n_next;
-        n_next.ax = n_next.ay = n_next.az = n_next.bx = n_next.by = n_next.bz = 0.f;
-        for (int it = 0, gl = 0, pass = 0; it < nitems; ++it) {
-            const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
-            // this item's directions; those of the NEXT group are requested before the binning of this one starts (below), so
-            // that their L2 latency (~700 clk) is not part of every group's serial path
-            LaneDirs n;
-            if (p.prefetch && it > 0) n = n_next;
-            else n = load_dirs(gl);
             APX_TRACE_EVENT(p, 0, sq.grp_base + gl);                                 // binning warp ready for the item
-            // Before the item: the buffer must be clear again after its previous use.
-            //   double-buffered, many ions : the clear warp's bulk copies of zeros complete on free[buf]
-            //   double-buffered, few ions  : (binclr) a group is binned long before the tensor core needs the other buffer
-            //                                back, so the chain transform -> clear warp -> free only adds latency: the 16
-            //                                binning warps clear the buffer themselves once its MMAs have completed (done[buf])
-            //   single-buffered (kBig)     : the shared-memory pipe is idle while the tensor core transforms the buffer, the
-            //                                binning warps clear it as soon as it has been read (done[0])
-            // Quiet signalling: only warp 0 polls the mbarrier, the other 15 block on a hardware barrier -- every waiter on an
-            // mbarrier is woken by every update of it (each bulk-copy chunk, each arrival) and burns issue slots re-checking.
-            if (use >= 1) {
-                const bool self_clear = kBig || binclr;
-                uint64_t *wbar = self_clear ? &ps.done[buf] : &ps.free_[buf];
-                if (p.quiet) {
-                    if (warp == 0) mbar_wait(wbar, (uint32_t)((use - 1) & 1));
-                    asm volatile("bar.sync 5, %0;" ::"n"(kBinWarps * 32) : "memory");
-                } else if (self_clear) {
-                    mbar_wait(wbar, (uint32_t)((use - 1) & 1));
-                } else {
-                    mbar_wait_lean(wbar, (uint32_t)((use - 1) & 1));
-                }
-                if (self_clear) {
-                    uint4 *hb = reinterpret_cast<uint4 *>(smem + (buf ? L.hist1 : L.hist0));
+            if (kBig) {
+                // single-buffered: the shared-memory pipe is idle while the tensor core transforms the buffer, so the 16
+                // binning warps clear it themselves as soon as it has been read (a few STS.128 per thread)
+                if (use >= 1) {
+                    mbar_wait(&ps.done[0], (uint32_t)((use - 1) & 1));
+                    uint4 *hb = reinterpret_cast<uint4 *>(smem + L.hist0);
                     for (int i = tid; i < (int)(L.hist_bytes / 16); i += kBinWarps * 32) hb[i] = make_uint4(0, 0, 0, 0);
                     asm volatile("bar.sync 5, %0;" ::"n"(kBinWarps * 32) : "memory");
                 }
+            } else if (use >= 1) {
+                mbar_wait_lean(&ps.free_[buf], (uint32_t)((use - 1) & 1));             // cleared after its previous use
             }
             APX_TRACE_EVENT(p, 1, sq.grp_base + gl);                                 // bin start (buffer free)
-            if (p.prefetch && it + 1 < nitems) {
-                const int gl_next = (pass + 1 == npass) ? gl + 1 : gl;
-                n_next = gl_next == gl ? n : load_dirs(gl_next);
-            }
             const int a0 = pass * 2048, a1 = min(n_ions, a0 + 2048);
+            const bool one_ion = NB == 4 && p.lanemap;                              // all lanes on the same ions (bin_ions_one)
             int i0, i1;
-            if (p.unit_split) {                                                      // whole blocks of 4 * NS ions per warp
-                constexpr int U = 4 * Lay<NB>::NS;
+            if (p.unit_split) {                                                      // whole blocks of ions per warp: no ragged tails
+                const int U = one_ion ? 4 : 4 * Lay<NB>::NS;
                 const int nu = (a1 - a0 + U - 1) / U;
                 i0 = a0 + U * ((warp * nu) / kBinWarps); i1 = min(a1, a0 + U * (((warp + 1) * nu) / kBinWarps));
             } else {
@@ -667,10 +692,20 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             const uint32_t k0 = k0base + (uint32_t)buf * (L.hist1 - L.hist0);
             Detect dta, dtb;
             if (detect) {
-                dta.flag = dtb.flag = &ps.flag[(sq.grp_base + gl) & 3];
+                dta.flag = dtb.flag = &ps.flag[(sq.grp_base + gl) & (kFlagSlots - 1)];
                 dta.nfix = dtb.nfix = ps.nfix; dta.fix = dtb.fix = ps.fix;
                 dta.bit = 1u << l; dtb.bit = 1u << (LW + l);
                 dta.id = (uint32_t)(gl * G + l); dtb.id = dta.id + (uint32_t)LW;
+            }
+            if (one_ion) {
+                const bool hiB = lane >= LW;                                         // upper half-warp: set B, high u16
+                const float nx = hiB ? n.bx : n.ax, ny = hiB ? n.by : n.ay, nz = hiB ? n.bz : n.az;
+                const uint32_t inc = hiB ? 65536u : 1u;
+                const Detect &dt = hiB ? dtb : dta;
+                if (detect) bin_ions_one<false, true, Lay<NB>::BLK>(ions_s, i0, i1, nx, ny, nz, c, k0, inc, dt);
+                else if (p.clamp) bin_ions_one<true, false, Lay<NB>::BLK>(ions_s, i0, i1, nx, ny, nz, c, k0, inc, dt);
+                else bin_ions_one<false, false, Lay<NB>::BLK>(ions_s, i0, i1, nx, ny, nz, c, k0, inc, dt);
+            } else if (detect) {
                 bin_ions<false, true, NB>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
             } else if (p.clamp) {
                 bin_ions<true, false, NB>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
@@ -680,14 +715,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
             __syncwarp();
             APX_TRACE_EVENT(p, 2, sq.grp_base + gl);                                 // bin end
-            // buffer full -> MMA warp: a hardware barrier (16 binning warps arrive, the MMA warp syncs) or, in the old
-            // scheme, 16 arrivals on an mbarrier the MMA warp polls
-            if (p.quiet) {
-                if (buf) asm volatile("bar.arrive 7, %0;" ::"n"(kBinWarps * 32 + 32) : "memory");
-                else asm volatile("bar.arrive 6, %0;" ::"n"(kBinWarps * 32 + 32) : "memory");
-            } else if (lane == 0) {
-                mbar_arrive(&ps.full[buf]);
-            }
+            if (lane == 0) mbar_arrive(&ps.full[buf]);
             if (++pass == npass) { pass = 0; ++gl; }
         }
     } else if (warp == kMmaWarp) {
@@ -702,20 +730,15 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         for (int it = 0, gl = 0, pass = 0; it < nitems; ++it) {
             const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
             const int gq = sq.grp_base + gl;
-            if (p.quiet) {
-                if (buf) asm volatile("bar.sync 7, %0;" ::"n"(kBinWarps * 32 + 32) : "memory");
-                else asm volatile("bar.sync 6, %0;" ::"n"(kBinWarps * 32 + 32) : "memory");
-            } else {
-                mbar_wait<100>(&ps.full[buf], (uint32_t)(use & 1));
-            }
+            mbar_wait<100>(&ps.full[buf], (uint32_t)(use & 1));
             APX_TRACE_EVENT(p, 3, gq);                                                // MMA warp: buffer full
-            if (pass == 0 && gq >= 2) mbar_wait(&ps.tfree[gq & 1], (uint32_t)(((gq >> 1) - 1) & 1));
+            if (pass == 0 && gq >= p.nacc) mbar_wait(&ps.tfree[gq & (p.nacc - 1)], (uint32_t)(((gq >> p.nacc_log2) - 1) & 1));
             APX_TRACE_EVENT(p, 4, gq);                                                // accumulator free, MMAs issued next
             asm volatile("tcgen05.fence::after_thread_sync;");
             if (p.hist_out && cls == 0)                          // test hook (first class): the buffer is complete
                 export_hist<NB, kHalf>(p, smem + (buf ? L.hist1 : L.hist0), mode, sq.g0 + gl, sq.g0, gl, sq.nfix, ps.fix,
-                                       (kHalf && mode == 0) ? ps.flag[gq & 3] : 0u, pass, lane);
-            const uint32_t acc = tmem + (uint32_t)((gq & 1) * p.N);
+                                       (kHalf && mode == 0) ? ps.flag[gq & (kFlagSlots - 1)] : 0u, pass, lane);
+            const uint32_t acc = tmem + (uint32_t)((gq & (p.nacc - 1)) * p.N);
             if (lane == 0) {
                 const uint32_t a_lo = a_lo0 + (uint32_t)buf * ((L.hist1 - L.hist0) >> 4);
 #pragma unroll
@@ -729,7 +752,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                              ::"r"(smem_u32(&ps.done[buf])) : "memory");
                 if (pass == npass - 1)                                           // the group's accumulator is complete
                     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
-                                 ::"r"(smem_u32(&ps.epi[gq & 1])) : "memory");
+                                 ::"r"(smem_u32(&ps.epi[gq & (p.nacc - 1)])) : "memory");
             }
             __syncwarp();
             if (++pass == npass) { pass = 0; ++gl; }
@@ -737,7 +760,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
     } else if (warp == kClrWarp) {
         // ---- clear warp: once the tensor core has read a buffer, clear it with bulk copies of zeros (TMA engine, no
         //      LSU work); free(buf) completes when all bytes have landed
-        for (int it = 0; it < ((kBig || binclr) ? 0 : nitems); ++it) {   // (otherwise the binning warps clear)
+        for (int it = 0; it < (kBig ? 0 : nitems); ++it) {           // (single-buffered: the binning warps clear)
             const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
             mbar_wait<100>(&ps.done[buf], (uint32_t)(use & 1));
             APX_TRACE_EVENT(p, 5, it_base + it);                                      // clear warp: MMAs of the buffer done
@@ -763,28 +786,18 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         const int q = warp & 3, set = (warp - kSvcWarp0) >> 2;
         for (int gl = (set ^ sq.grp_base) & 1; gl < sq.ngrp; gl += 2) {
             const int gq = sq.grp_base + gl;
-            if (p.quiet) {                                                           // one warp polls, three block in hardware
-                if (q == 0) mbar_wait<200>(&ps.epi[set], (uint32_t)((gq >> 1) & 1));
-                if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
-            } else {
-                mbar_wait_lean<200>(&ps.epi[set], (uint32_t)((gq >> 1) & 1));
-            }
+            mbar_wait_lean<200>(&ps.epi[gq & (p.nacc - 1)], (uint32_t)((gq >> p.nacc_log2) & 1));
             APX_TRACE_EVENT(p, 7, gq);                                                // epilogue start
             asm volatile("tcgen05.fence::after_thread_sync;");
             EpiOut eo;
             eo.cls = cls; eo.n = n;
             eo.mode = mode; eo.gi = sq.g0 + gl; eo.g0 = sq.g0; eo.f = gl; eo.nfix = sq.nfix;
-            eo.flag = kHalf ? &ps.flag[gq & 3] : nullptr; eo.fix = ps.fix;
-            epilogue_group<kHalf, NB>(p, tmem + (uint32_t)(set * p.N), eo, m, phase, exch, cand, set, q, lane);
+            eo.flag = kHalf ? &ps.flag[gq & (kFlagSlots - 1)] : nullptr; eo.fix = ps.fix;
+            epilogue_group<kHalf, NB>(p, tmem + (uint32_t)((gq & (p.nacc - 1)) * p.N), eo, m, phase, exch, cand, set, q, lane);
             asm volatile("tcgen05.fence::before_thread_sync;");
             __syncwarp();
             APX_TRACE_EVENT(p, 8, gq);                                                // epilogue end
-            if (p.quiet) {                                                           // all four warps have read the accumulator
-                if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
-                if (q == 0 && lane == 0) mbar_arrive(&ps.tfree[set]);
-            } else if (lane == 0) {
-                mbar_arrive(&ps.tfree[set]);
-            }
+            if (lane == 0) mbar_arrive(&ps.tfree[gq & (p.nacc - 1)]);
         }
     }
 }
@@ -796,10 +809,10 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned, still shared-space
     const MmaSmem L = mma_smem_layout(p.B, p.N, p.W, p.cap);
     // per histogram buffer: full (binned), done (transformed), free (cleared); per accumulator: tfree (read out)
-    __shared__ uint64_t s_full[2], s_done[2], s_free[2], s_epi[2], s_tfree[2];
+    __shared__ uint64_t s_full[2], s_done[2], s_free[2], s_epi[4], s_tfree[4];      // per histogram buffer / per accumulator
     __shared__ uint32_t s_tmem;
     __shared__ int s_n, s_nfix;
-    __shared__ uint32_t s_flag[4];
+    __shared__ uint32_t s_flag[kFlagSlots];
     __shared__ uint16_t s_fix[kFixCap];
 
     const int tid = threadIdx.x, warp = tid >> 5;
@@ -829,18 +842,24 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
     auto init_barriers = [&](bool again) {
         for (int i = 0; i < 2; ++i) {
             if (again) {                                   // a new class of signatures restarts the pipeline's phase counts
-                uint64_t *bars[5] = {&s_full[i], &s_done[i], &s_free[i], &s_epi[i], &s_tfree[i]};
+                uint64_t *bars[3] = {&s_full[i], &s_done[i], &s_free[i]};
                 for (uint64_t *b : bars) asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(b)) : "memory");
             }
             mbar_init(&s_full[i], kBinWarps);
             mbar_init(&s_done[i], 1);
             mbar_init(&s_free[i], 1);
+        }
+        for (int i = 0; i < 4; ++i) {
+            if (again) {
+                asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&s_epi[i])) : "memory");
+                asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&s_tfree[i])) : "memory");
+            }
             mbar_init(&s_epi[i], 1);
-            mbar_init(&s_tfree[i], p.quiet ? 1 : 4);
+            mbar_init(&s_tfree[i], 4);
         }
         asm volatile("fence.mbarrier_init.release.cluster;");
         s_n = 0; s_nfix = 0;
-        for (int i = 0; i < 4; ++i) s_flag[i] = 0u;
+        for (int i = 0; i < kFlagSlots; ++i) s_flag[i] = 0u;
     };
     if (tid == 0) init_barriers(false);
     if (warp == 0) {
@@ -915,8 +934,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
             // (or re-initialises the barriers for the next class)
             if (warp == kClrWarp && grp_total > 0) {
                 const int npass = n > 2048 ? (n + 2047) / 2048 : 1, items = grp_total * npass;
-                if (NB == 8 || n > p.cap || n < p.binclear_below) {
-                    // cleared with plain stores by the binning warps, nothing in flight
+                if (NB == 8 || n > p.cap) {
+                    // single-buffered: cleared with plain stores by the binning warps, nothing in flight
                 } else {
                     const int u0 = (items + 1) >> 1, u1 = items >> 1;
                     if (u0) mbar_wait(&s_free[0], (uint32_t)((u0 - 1) & 1));
@@ -1121,12 +1140,11 @@ cudaError_t mma_path_prepare(Plan *p)
             for (int a = 0; a < 3; ++a) sorted[3 * i + a] = nps[3 * (size_t)src + a];
         }
     }
-    // tuning knobs (development): defaults chosen from measurements, overridable from the environment
-    p->tune_binclear = 0; p->tune_unit_split = 0; p->tune_quiet = 0; p->tune_prefetch = 0;
-    if (const char *ev = std::getenv("APX_TUNE_PREFETCH")) p->tune_prefetch = std::atoi(ev);
-    if (const char *ev = std::getenv("APX_TUNE_QUIET")) p->tune_quiet = std::atoi(ev);
-    if (const char *ev = std::getenv("APX_TUNE_BINCLEAR")) p->tune_binclear = std::atoi(ev);
+    // scheduling knobs: defaults chosen from measurements, overridable from the environment for A/B runs
+    p->tune_unit_split = 1; p->tune_nacc = 4; p->tune_lanemap = 1;
     if (const char *ev = std::getenv("APX_TUNE_UNITS")) p->tune_unit_split = std::atoi(ev);
+    if (const char *ev = std::getenv("APX_TUNE_NACC")) p->tune_nacc = std::atoi(ev);
+    if (const char *ev = std::getenv("APX_TUNE_LANEMAP")) p->tune_lanemap = std::atoi(ev);
     const int Dp = (int)perm.size();
     p->mma_paired = sym ? 1 : 0;
     p->Dp = Dp;
@@ -1212,9 +1230,11 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.M = (int)M;
     q.clamp = p->need_clamp;
     q.half = p->mma_paired;
-    q.binclear_below = p->tune_binclear; q.unit_split = p->tune_unit_split; q.quiet = p->tune_quiet; q.prefetch = p->tune_prefetch;
+    q.unit_split = p->tune_unit_split; q.lanemap = p->tune_lanemap;
+    q.nacc = (p->tune_nacc == 4 && 4 * q.N <= 512) ? 4 : 2;
+    q.nacc_log2 = q.nacc == 4 ? 2 : 1;
     uint32_t cols = 32;
-    while (cols < (uint32_t)(2 * q.N)) cols *= 2;
+    while (cols < (uint32_t)(q.nacc * q.N)) cols *= 2;
     q.tmem_cols = cols;
     q.R = p->R; q.R2 = p->R2;
     const MmaSmem L = mma_smem_layout(p->B, q.N, p->W, q.cap);

@@ -352,6 +352,14 @@ extern "C" int apx_debug_histograms(apx_plan *p, const float *centre3, int32_t d
 }
 
 #ifdef APX_TRACE
+// development builds only: the tensor-core path's slot order (original direction index per slot, -1 = padding)
+extern "C" int apx_debug_slot_order(apx_plan *p, int *perm, int *mirror)
+{
+    if (!p || p->path != 1) return APX_EINVAL;
+    if (perm) cudaMemcpy(perm, p->d_dir_perm, (size_t)p->Dp * 4, cudaMemcpyDeviceToHost);
+    if (mirror && p->d_dir_perm_mirror) cudaMemcpy(mirror, p->d_dir_perm_mirror, (size_t)p->Dp * 4, cudaMemcpyDeviceToHost);
+    return p->Dp;
+}
 // development builds only (-DAPX_TRACE, not declared in the public headers): timeline buffer for k_signature_mma
 extern "C" int apx_debug_trace(apx_plan *p, long long *device_buf, int block, int cap)
 {

@@ -178,7 +178,6 @@ struct MmaParams {
     SpecSet ss;                // signatures of the plan: classes (type masks), per-spec sub-windows of [k_lo, k_lo + W)
     int nacc, nacc_log2;       // TMEM accumulators (2 or 4): group gq uses accumulator gq & (nacc - 1), so the MMAs of a group
                                // wait for the epilogue of group gq - nacc only
-    int lanemap;               // 1 (NB = 4): all lanes of a warp bin the same ions, half-warps = sets A / B (bin_ions_one)
     int unit_split;            // 1 = ions are dealt to the binning warps in whole blocks of 4 * NS (no ragged tails)
     uint32_t tmem_cols;
     float R, R2;
@@ -397,55 +396,6 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
     }
 }
 
-// The same step with the other lane map (NB = 4 only): all 32 lanes of a warp work on the SAME ions; lane l < 16 bins them
-// for direction l of set A (low u16, +1), lane l >= 16 for direction l - 16 of set B (high u16, +65536).  Set B is the patch
-// antipodal to set A, so for one ion hi3(B) = 7 - hi3(A): the two half-warps of one shared atomic always fall on the two
-// different bank halves -- conflict-free by construction instead of by the luck of two unrelated ions (measured 1.9
-// wavefronts per ATOMS before).  One ion load now serves 32 instead of 64 pairs; at 2.3 clk per broadcast LDS.128 against
-// 1.9 -> ~1.1 clk per ATOMS this lowers the shared-memory time per pair from 0.144 to ~0.09 clk.
-template <bool kClamp, bool kDetect, int BLK>
-__device__ __forceinline__ void bin_ions_one(uint32_t ions_s, int i0, int i1, float nx, float ny, float nz, const BinConst &c,
-                                             uint32_t k0, uint32_t inc, const Detect &dt)
-{
-    int ib = i0;
-    if (!kClamp) {
-        const uint64_t nx2 = pack2(nx, nx), ny2 = pack2(ny, ny), nz2 = pack2(nz, nz);
-        const uint64_t ma2 = pack2(c.magic_a, c.magic_a), sc2 = pack2(c.scl, c.scl), mb2 = pack2(c.magic_b, c.magic_b);
-        uint32_t src = ions_s + (uint32_t)ib * 12u;
-#pragma unroll 2
-        for (; ib + 8 <= i1; ib += 8, src += 96u) {          // 8 ions = 6 LDS.128 (one address per warp), 4 packed chains
-            float4 q[6];
-#pragma unroll
-            for (int u = 0; u < 6; ++u) q[u] = lds128(src + (uint32_t)u * 16u);
-            uint64_t nn = 0ull;
-#pragma unroll
-            for (int hh = 0; hh < 2; ++hh) {
-                const float4 X = q[3 * hh], Y = q[3 * hh + 1], Z = q[3 * hh + 2];
-                bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc, nn);
-                bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc, nn);
-            }
-            if (kDetect && __builtin_expect(sum2(nn) != 8.0f, 0)) flag_pair(dt.flag, dt.nfix, dt.fix, dt.bit, dt.id);
-        }
-        if (ib + 4 <= i1) {                                  // one quad
-            const uint32_t a = ions_s + (uint32_t)ib * 12u;
-            const float4 X = lds128(a), Y = lds128(a + 16u), Z = lds128(a + 32u);
-            uint64_t nn = 0ull;
-            bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc, nn);
-            bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, nx2, ny2, nz2, ma2, sc2, mb2, c.kz, k0, inc, nn);
-            if (kDetect && __builtin_expect(sum2(nn) != 4.0f, 0)) flag_pair(dt.flag, dt.nfix, dt.fix, dt.bit, dt.id);
-            ib += 4;
-        }
-    }
-    for (int i = ib; i < i1; ++i) {                          // ragged tail (and every ion when the clamp is needed)
-        const uint32_t a = ions_s + (uint32_t)(i >> 2) * 48u + (uint32_t)(i & 3) * 4u;
-        float dx, dy, dz;
-        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dx) : "r"(a));
-        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dy) : "r"(a + 16u));
-        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(a + 32u));
-        bin_one<kClamp, kDetect, BLK>(dx, dy, dz, nx, ny, nz, c, k0, inc, dt.flag, dt.nfix, dt.fix, dt.bit, dt.id);
-    }
-}
-
 // Epilogue of one direction group (a5 tail, a6, a7) by one set of four service warps.  Service warp q reads TMEM
 // lane quarter q = M rows 32q..32q+31 = part blk = q of all 32 direction slots (slot from the lane).  Window bins
 // are handled in rounds of 4: each thread scales its 4 partial sums by the phase w^{blk k}, keeps the one whose
@@ -610,7 +560,7 @@ struct Seq {
     int mode, g0, ngrp, grp_base, nfix;
 };
 struct PipeShared {
-    uint64_t *full, *done, *free_, *epi, *tfree;
+    uint64_t *full, *done, *doneq, *free_, *epi, *tfree;    // doneq[buf * 3 + q]: first three quarters of a buffer's MMAs complete
     uint32_t *flag;
     int *nfix;
     uint16_t *fix;
@@ -654,6 +604,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         const bool detect = kHalf && mode == 0;
         for (int it = 0, gl = 0, pass = 0; it < nitems; ++it) {
             const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
+            APX_TRACE_EVENT(p, 10, sq.grp_base + gl);                                // loop top
             LaneDirs n;
             if (mode == 0) {
                 const float *da = p.dirs_sorted + (size_t)((sq.g0 + gl) * G + l) * 3;
@@ -679,10 +630,9 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             }
             APX_TRACE_EVENT(p, 1, sq.grp_base + gl);                                 // bin start (buffer free)
             const int a0 = pass * 2048, a1 = min(n_ions, a0 + 2048);
-            const bool one_ion = NB == 4 && p.lanemap;                              // all lanes on the same ions (bin_ions_one)
             int i0, i1;
-            if (p.unit_split) {                                                      // whole blocks of ions per warp: no ragged tails
-                const int U = one_ion ? 4 : 4 * Lay<NB>::NS;
+            if (p.unit_split) {                                                      // whole blocks of 4 * NS ions per warp: no ragged tails
+                constexpr int U = 4 * Lay<NB>::NS;
                 const int nu = (a1 - a0 + U - 1) / U;
                 i0 = a0 + U * ((warp * nu) / kBinWarps); i1 = min(a1, a0 + U * (((warp + 1) * nu) / kBinWarps));
             } else {
@@ -696,16 +646,6 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                 dta.nfix = dtb.nfix = ps.nfix; dta.fix = dtb.fix = ps.fix;
                 dta.bit = 1u << l; dtb.bit = 1u << (LW + l);
                 dta.id = (uint32_t)(gl * G + l); dtb.id = dta.id + (uint32_t)LW;
-            }
-            if (one_ion) {
-                const bool hiB = lane >= LW;                                         // upper half-warp: set B, high u16
-                const float nx = hiB ? n.bx : n.ax, ny = hiB ? n.by : n.ay, nz = hiB ? n.bz : n.az;
-                const uint32_t inc = hiB ? 65536u : 1u;
-                const Detect &dt = hiB ? dtb : dta;
-                if (detect) bin_ions_one<false, true, Lay<NB>::BLK>(ions_s, i0, i1, nx, ny, nz, c, k0, inc, dt);
-                else if (p.clamp) bin_ions_one<true, false, Lay<NB>::BLK>(ions_s, i0, i1, nx, ny, nz, c, k0, inc, dt);
-                else bin_ions_one<false, false, Lay<NB>::BLK>(ions_s, i0, i1, nx, ny, nz, c, k0, inc, dt);
-            } else if (detect) {
                 bin_ions<false, true, NB>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
             } else if (p.clamp) {
                 bin_ions<true, false, NB>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
@@ -716,6 +656,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             __syncwarp();
             APX_TRACE_EVENT(p, 2, sq.grp_base + gl);                                 // bin end
             if (lane == 0) mbar_arrive(&ps.full[buf]);
+            APX_TRACE_EVENT(p, 9, sq.grp_base + gl);                                 // arrived
             if (++pass == npass) { pass = 0; ++gl; }
         }
     } else if (warp == kMmaWarp) {
@@ -747,6 +688,11 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                     const uint64_t bd = ((uint64_t)b_hi << 32) | (b_lo0 + (uint32_t)(ks >> 2) * kblk_step + (uint32_t)(ks & 3) * 2u);
                     if (ks == 0) mma_f16_ss(acc, ad, bd, idesc, pass > 0 ? 1u : 0u);
                     else mma_f16_acc(acc, ad, bd, idesc);
+                    // k-steps 4q..4q+3 read the q-th quarter of the buffer (contiguous bytes): a commit per quarter lets the
+                    // clear warp zero it while the remaining MMAs still run
+                    if (!kBig && KS >= 4 && (ks + 1) % (KS / 4) == 0 && ks + 1 < KS)
+                        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
+                                     ::"r"(smem_u32(&ps.doneq[buf * 3 + (ks + 1) / (KS / 4) - 1])) : "memory");
                 }
                 asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
                              ::"r"(smem_u32(&ps.done[buf])) : "memory");
@@ -762,22 +708,26 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
         //      LSU work); free(buf) completes when all bytes have landed
         for (int it = 0; it < (kBig ? 0 : nitems); ++it) {           // (single-buffered: the binning warps clear)
             const int itg = it_base + it, buf = kBig ? 0 : (itg & 1), use = kBig ? itg : (itg >> 1);
-            mbar_wait<100>(&ps.done[buf], (uint32_t)(use & 1));
-            APX_TRACE_EVENT(p, 5, it_base + it);                                      // clear warp: MMAs of the buffer done
-            if (n < kStsClearBelow) {
-                // few ions: the LSU pipe has room, clear with plain stores and spare the L2 the zero traffic
-                uint4 *hp = reinterpret_cast<uint4 *>(smem + (buf ? L.hist1 : L.hist0));
-                for (int i = lane; i < (int)(L.hist_bytes / 16); i += 32) hp[i] = make_uint4(0, 0, 0, 0);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&ps.free_[buf]);
-            } else if (lane == 0) {
-                const uint32_t dst = smem_u32(smem + (buf ? L.hist1 : L.hist0)), bar = smem_u32(&ps.free_[buf]);
-                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(L.hist_bytes) : "memory");
-                const uint32_t piece = L.hist_bytes / 4;
-#pragma unroll
-                for (int c4 = 0; c4 < 4; ++c4)
+            const uint32_t piece = L.hist_bytes / 4;
+            if (n >= kStsClearBelow && lane == 0)
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&ps.free_[buf])), "r"(L.hist_bytes) : "memory");
+#pragma unroll 1
+            for (int c4 = 0; c4 < 4; ++c4) {                     // quarter by quarter, as the tensor core releases them
+                mbar_wait<100>(c4 < 3 ? &ps.doneq[buf * 3 + c4] : &ps.done[buf], (uint32_t)(use & 1));
+                if (c4 == 3) APX_TRACE_EVENT(p, 5, it_base + it);                     // clear warp: all MMAs of the buffer done
+                if (n < kStsClearBelow) {
+                    // few ions: the LSU pipe has room, clear with plain stores and spare the L2 the zero traffic
+                    uint4 *hp = reinterpret_cast<uint4 *>(smem + (buf ? L.hist1 : L.hist0) + c4 * piece);
+                    for (int i = lane; i < (int)(piece / 16); i += 32) hp[i] = make_uint4(0, 0, 0, 0);
+                } else if (lane == 0) {
+                    const uint32_t dst = smem_u32(smem + (buf ? L.hist1 : L.hist0)), bar = smem_u32(&ps.free_[buf]);
                     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                                  ::"r"(dst + c4 * piece), "l"((const char *)p.zeros + c4 * piece), "r"(piece), "r"(bar) : "memory");
+                }
+            }
+            if (n < kStsClearBelow) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&ps.free_[buf]);
             }
             __syncwarp();
         }
@@ -809,7 +759,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned, still shared-space
     const MmaSmem L = mma_smem_layout(p.B, p.N, p.W, p.cap);
     // per histogram buffer: full (binned), done (transformed), free (cleared); per accumulator: tfree (read out)
-    __shared__ uint64_t s_full[2], s_done[2], s_free[2], s_epi[4], s_tfree[4];      // per histogram buffer / per accumulator
+    __shared__ uint64_t s_full[2], s_done[2], s_doneq[6], s_free[2], s_epi[4], s_tfree[4];      // per histogram buffer / per accumulator
     __shared__ uint32_t s_tmem;
     __shared__ int s_n, s_nfix;
     __shared__ uint32_t s_flag[kFlagSlots];
@@ -849,6 +799,10 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
             mbar_init(&s_done[i], 1);
             mbar_init(&s_free[i], 1);
         }
+        for (int i = 0; i < 6; ++i) {
+            if (again) asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&s_doneq[i])) : "memory");
+            mbar_init(&s_doneq[i], 1);
+        }
         for (int i = 0; i < 4; ++i) {
             if (again) {
                 asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&s_epi[i])) : "memory");
@@ -872,7 +826,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
         for (int i = tid; i < NB * p.W; i += kMmaThreads) phase[i] = p.phase[i];
     }
     PipeShared ps;
-    ps.full = s_full; ps.done = s_done; ps.free_ = s_free; ps.epi = s_epi; ps.tfree = s_tfree;
+    ps.full = s_full; ps.done = s_done; ps.doneq = s_doneq; ps.free_ = s_free; ps.epi = s_epi; ps.tfree = s_tfree;
     ps.flag = s_flag; ps.nfix = &s_nfix; ps.fix = s_fix;
     uint32_t tmem = 0;
     // ---- one pass per class of signatures (specs with the same type mask): gather, then the group pipeline ---------
@@ -1141,10 +1095,9 @@ cudaError_t mma_path_prepare(Plan *p)
         }
     }
     // scheduling knobs: defaults chosen from measurements, overridable from the environment for A/B runs
-    p->tune_unit_split = 1; p->tune_nacc = 4; p->tune_lanemap = 1;
+    p->tune_unit_split = 1; p->tune_nacc = 4;
     if (const char *ev = std::getenv("APX_TUNE_UNITS")) p->tune_unit_split = std::atoi(ev);
     if (const char *ev = std::getenv("APX_TUNE_NACC")) p->tune_nacc = std::atoi(ev);
-    if (const char *ev = std::getenv("APX_TUNE_LANEMAP")) p->tune_lanemap = std::atoi(ev);
     const int Dp = (int)perm.size();
     p->mma_paired = sym ? 1 : 0;
     p->Dp = Dp;
@@ -1230,7 +1183,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.M = (int)M;
     q.clamp = p->need_clamp;
     q.half = p->mma_paired;
-    q.unit_split = p->tune_unit_split; q.lanemap = p->tune_lanemap;
+    q.unit_split = p->tune_unit_split;
     q.nacc = (p->tune_nacc == 4 && 4 * q.N <= 512) ? 4 : 2;
     q.nacc_log2 = q.nacc == 4 ? 2 : 1;
     uint32_t cols = 32;

@@ -38,6 +38,7 @@
 #include <cmath>
 #include <cuda_fp16.h>
 #include <numeric>
+#include <type_traits>
 #include <vector>
 #include "common.cuh"
 
@@ -110,17 +111,22 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         }
     } while (!done);
 }
-// The same wait without the trap guard, for the two waits that poll most (binning warps on `free`, service warps on
-// `epi`): three instructions fewer per attempt.  A lost arrival would still be caught by the guarded waits of the MMA and
-// clear warps that feed these barriers.
+// The same wait as one tight PTX loop (no flag materialised in a register, no selp), for the two waits that poll most
+// (binning warps on `free`, service warps on `epi`).  It carries the same guard: after 2^22 unsuccessful attempts (seconds)
+// the warp traps instead of hanging the device on a lost arrival.
 template <unsigned kSleepNs = 64>
 __device__ __forceinline__ void mbar_wait_lean(uint64_t *bar, uint32_t parity)
 {
-    asm volatile("{\n .reg .pred p;\n"
+    asm volatile("{\n .reg .pred p;\n .reg .u32 n;\n mov.u32 n, 0;\n"
                  "WAIT_LOOP:\n"
                  " mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
                  " @p bra WAIT_DONE;\n"
                  " nanosleep.u32 %3;\n"
+#ifndef APX_LEAN_NOGUARD
+                 " add.u32 n, n, 1;\n"
+                 " setp.gt.u32 p, n, 4194304;\n"
+                 " @p trap;\n"
+#endif
                  " bra WAIT_LOOP;\n"
                  "WAIT_DONE:\n}"
                  ::"r"(smem_u32(bar)), "r"(parity), "r"(1000000u), "n"(kSleepNs) : "memory");
@@ -175,6 +181,7 @@ struct MmaParams {
 #endif
     int D, B, nl, k_lo, W, N, cap, cap_big, nchunks, ngroups, clamp, M;
     int half;                  // 1 = half-grid mode: one direction per antipodal pair is binned (perm_mirror != nullptr)
+    int norm0;                 // single-signature plans: 1 = write A / N_c
     SpecSet ss;                // signatures of the plan: classes (type masks), per-spec sub-windows of [k_lo, k_lo + W)
     int nacc, nacc_log2;       // TMEM accumulators (2 or 4): group gq uses accumulator gq & (nacc - 1), so the MMAs of a group
                                // wait for the epilogue of group gq - nacc only
@@ -211,6 +218,7 @@ __host__ __device__ inline MmaSmem mma_smem_layout(int B, int N, int W, int cap)
 
 // Gather (step a2) into quad-blocked records: four ions = 48 B = [dx0..dx3][dy0..dy3][dz0..dz3], i.e. three LDS.128
 // whose register pairs are the operands of the packed fp32x2 arithmetic of the binning warps.
+template <bool kMulti>
 __device__ __forceinline__ void gather_roi3(const MmaParams &p, const GridParams &g, const RoiCells &rc,
                                             float cx, float cy, float cz, float *ions, int *s_n, int cls)
 {
@@ -226,7 +234,7 @@ __device__ __forceinline__ void gather_roi3(const MmaParams &p, const GridParams
             if (i < end) {
                 float4 q = p.sorted[i];
                 dx = __fsub_rn(q.x, cx); dy = __fsub_rn(q.y, cy); dz = __fsub_rn(q.z, cz);
-                in = inside(dx, dy, dz, p.R2) && (p.ss.n_classes == 1 || type_in_class(p.ss, cls, __float_as_uint(q.w)));
+                in = inside(dx, dy, dz, p.R2) && (!kMulti || p.ss.n_classes == 1 || type_in_class(p.ss, cls, __float_as_uint(q.w)));
             }
             unsigned msk = __ballot_sync(0xffffffffu, in);
             if (msk) {
@@ -321,14 +329,23 @@ __device__ __forceinline__ void bin_pair(float dx0, float dx1, float dy0, float 
     red_shared_add(ua0 * (uint32_t)BLK + (va0 * kz + k0), inc);
     red_shared_add(ua1 * (uint32_t)BLK + (va1 * kz + k0), inc);
     if (kDetect) {
-        uint64_t up, d;
+        uint64_t up;
         asm("add.rp.f32x2 %0, %1, %2;" : "=l"(up) : "l"(t), "l"(ma2));
+#ifndef APX_DETECT_FP
+        // integer variant: RU - RD of the bit patterns, accumulated in the low word of nonint2
+        nonint2 += (uint64_t)(((uint32_t)up - ua0) + ((uint32_t)(up >> 32) - ua1));
+#else
+        uint64_t d;
         asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(up), "l"(ua));              // exact: (0 or 1, 0 or 1)
         asm("add.rn.f32x2 %0, %1, %2;" : "=l"(nonint2) : "l"(nonint2), "l"(d));
+#endif
     }
 }
 __device__ __forceinline__ float sum2(uint64_t v)
 {
+#ifndef APX_DETECT_FP
+    return (float)(uint32_t)v;
+#endif
     float lo, hi;
     asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
     return lo + hi;
@@ -408,7 +425,7 @@ struct EpiOut {
     uint32_t *flag;                      // mode 0, half-grid: flag word of this group (read, then reset)
     const uint16_t *fix;
 };
-template <bool kHalf, int NB>
+template <bool kHalf, int NB, bool kMulti>
 __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc, const EpiOut &eo, int64_t m, const float2 *phase,
                                                float2 *exch_all, float2 *cand_all, int set, int q, int lane)
 {
@@ -417,11 +434,14 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
     const uint32_t acc0 = acc + ((uint32_t)(q * 32) << 16);
     float2 *exch = exch_all + set * (kEpiRound * 4 * 32), *cand = cand_all + set * (4 * 32);
     // one running maximum per spec of the class (a spec's window is a sub-range of the transformed union window)
-    float best[kMaxSpecs];
-    int kbest[kMaxSpecs];
+    // (kMulti = false: the plan has ONE signature -- the common case keeps the single-maximum code of a one-signature kernel)
+    constexpr int NSP = kMulti ? kMaxSpecs : 1;
+    const int n_specs = kMulti ? p.ss.n_specs : 1;      // the single-signature kernel never touches p.ss (window = union window)
+    float best[NSP];
+    int kbest[NSP];
 #pragma unroll
-    for (int sp = 0; sp < kMaxSpecs; ++sp) { best[sp] = -1.0f; kbest[sp] = sp < p.ss.n_specs ? p.ss.k_lo[sp] : 0; }
-    const bool one_spec = p.ss.n_specs == 1;
+    for (int sp = 0; sp < NSP; ++sp) { best[sp] = -1.0f; kbest[sp] = !kMulti ? p.k_lo : (sp < n_specs ? p.ss.k_lo[sp] : 0); }
+    const bool one_spec = !kMulti || n_specs == 1;
 #pragma unroll 1
     for (int r0 = 0; r0 < p.W; r0 += kEpiRound) {
         uint32_t v[16];
@@ -459,8 +479,8 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
                 if (pw > best[0]) { best[0] = pw; kbest[0] = k; }        // ascending w: lowest k kept on ties
             } else {
 #pragma unroll
-                for (int sp = 0; sp < kMaxSpecs; ++sp)
-                    if (sp < p.ss.n_specs && p.ss.cls_of[sp] == eo.cls && k >= p.ss.k_lo[sp] && k <= p.ss.k_hi[sp] && pw > best[sp]) {
+                for (int sp = 0; sp < NSP; ++sp)
+                    if (kMulti && sp < n_specs && p.ss.cls_of[sp] == eo.cls && k >= p.ss.k_lo[sp] && k <= p.ss.k_hi[sp] && pw > best[sp]) {
                         best[sp] = pw; kbest[sp] = k;
                     }
             }
@@ -469,19 +489,19 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
     }
     if (kHalf && mode == 0 && q == 0 && lane == 0) *eo.flag = 0u;     // every thread of the set has read it (barriers above)
 #pragma unroll 1
-    for (int sp = 0; sp < p.ss.n_specs; ++sp) {
-        if (p.ss.cls_of[sp] != eo.cls) continue;
+    for (int sp = 0; sp < n_specs; ++sp) {
+        if (kMulti && p.ss.cls_of[sp] != eo.cls) continue;
         float bsel = best[0];
         int ksel = kbest[0];
 #pragma unroll
-        for (int j = 1; j < kMaxSpecs; ++j)
+        for (int j = 1; j < NSP; ++j)
             if (j == sp) { bsel = best[j]; ksel = kbest[j]; }
         cand[q * 32 + lane] = make_float2(bsel, __int_as_float(ksel));
         if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
         if (q == 0 && lane < Lay<NB>::G) {                   // (NB = 8: lanes 16..31 carry copies of lanes 0..15)
             constexpr int G = Lay<NB>::G;
             float bb = -1.0f;
-            int kb = p.ss.k_lo[sp];
+            int kb = kMulti ? p.ss.k_lo[sp] : p.k_lo;
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
                 const float2 c2 = cand[s * 32 + lane];
@@ -491,9 +511,9 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
             // M row (within a part) = chunk * 8 + word * 2 + half  ->  slot = half * G/2 + chunk * 4 + word
             const int slot = (lane & 1) * (G / 2) + ((lane >> 3) << 2) + ((lane & 7) >> 1);
             float amp = 16777216.0f * sqrtf(fmaxf(bb, 0.0f));
-            if (p.ss.norm[sp]) amp = eo.n ? __fdiv_rn(amp, (float)eo.n) : 0.0f;   // normalised intensity A / N_c (L424)
+            if (kMulti ? p.ss.norm[sp] : p.norm0) amp = eo.n ? __fdiv_rn(amp, (float)eo.n) : 0.0f;   // normalised intensity A / N_c (L424)
             const float2 res = make_float2(amp, (float)kb);
-            float2 *out = p.sig + (size_t)sp * (size_t)p.M * p.D + (size_t)m * p.D;
+            float2 *out = p.sig + (kMulti ? (size_t)sp * (size_t)p.M * p.D : (size_t)0) + (size_t)m * p.D;
             if (mode == 0) {
                 const int d = p.perm[eo.gi * G + slot];
                 if (d >= 0) out[d] = res;
@@ -521,8 +541,13 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
 // halves: (bin b, slot) lives in half (slot / LW) of word (slot % LW) at byte (w/4)*SBO + (w%4)*4 + 16*hi3 + BLK*low.
 // Pass 0 of a group stores, later passes of a ROI with more than 2048 ions add.  Half-grid mode: the mirrored direction
 // gets the histogram reversed (b -> B-1-b) unless the pair is flagged; flagged pairs are stored by their fix-up group.
+struct ExportArgs {                      // by value: taking the address of the kernel's parameter block would force a local copy
+    uint32_t *hist_out;
+    const int *perm, *perm_mirror;
+    int hist_d0, hist_nd, B, nl;
+};
 template <int NB, bool kHalf>
-__device__ __noinline__ void export_hist(const MmaParams &p, const unsigned char *hist, int mode, int gi, int g0, int f, int nfix,
+__device__ __noinline__ void export_hist(const ExportArgs p, const unsigned char *hist, int mode, int gi, int g0, int f, int nfix,
                                          const uint16_t *fix, uint32_t mask, int pass, int lane)
 {
     constexpr int G = Lay<NB>::G, LW = Lay<NB>::LW, SBO = Lay<NB>::SBO, BLK = Lay<NB>::BLK;
@@ -568,7 +593,7 @@ struct PipeShared {
 
 // The warp-specialised pipeline of one (material point, chunk).  kBig: the ROI's ions have spilled into the second
 // histogram buffer, so only buffer 0 is used and bin -> transform -> clear are serial per item.
-template <int KS, int NB, bool kBig, bool kHalf>
+template <int KS, int NB, bool kBig, bool kHalf, bool kMulti>
 __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &L, unsigned char *smem, uint32_t tmem, int n_ions,
                                              const Seq &sq, int64_t m, const float *ions, const float2 *phase,
                                              float2 *exch, float2 *cand, const PipeShared &ps, int cls)
@@ -677,7 +702,8 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             APX_TRACE_EVENT(p, 4, gq);                                                // accumulator free, MMAs issued next
             asm volatile("tcgen05.fence::after_thread_sync;");
             if (p.hist_out && cls == 0)                          // test hook (first class): the buffer is complete
-                export_hist<NB, kHalf>(p, smem + (buf ? L.hist1 : L.hist0), mode, sq.g0 + gl, sq.g0, gl, sq.nfix, ps.fix,
+                export_hist<NB, kHalf>(ExportArgs{p.hist_out, p.perm, p.perm_mirror, p.hist_d0, p.hist_nd, p.B, p.nl},
+                                       smem + (buf ? L.hist1 : L.hist0), mode, sq.g0 + gl, sq.g0, gl, sq.nfix, ps.fix,
                                        (kHalf && mode == 0) ? ps.flag[gq & (kFlagSlots - 1)] : 0u, pass, lane);
             const uint32_t acc = tmem + (uint32_t)((gq & (p.nacc - 1)) * p.N);
             if (lane == 0) {
@@ -743,7 +769,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             eo.cls = cls; eo.n = n;
             eo.mode = mode; eo.gi = sq.g0 + gl; eo.g0 = sq.g0; eo.f = gl; eo.nfix = sq.nfix;
             eo.flag = kHalf ? &ps.flag[gq & (kFlagSlots - 1)] : nullptr; eo.fix = ps.fix;
-            epilogue_group<kHalf, NB>(p, tmem + (uint32_t)((gq & (p.nacc - 1)) * p.N), eo, m, phase, exch, cand, set, q, lane);
+            epilogue_group<kHalf, NB, kMulti>(p, tmem + (uint32_t)((gq & (p.nacc - 1)) * p.N), eo, m, phase, exch, cand, set, q, lane);
             asm volatile("tcgen05.fence::before_thread_sync;");
             __syncwarp();
             APX_TRACE_EVENT(p, 8, gq);                                                // epilogue end
@@ -752,7 +778,19 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
     }
 }
 
-template <int KS, int NB, bool kHalf>   // KS = K/16 k-steps per group, NB = bin parts (layout), kHalf = half-grid mode
+// one sequence, in the double-buffered pipeline or -- the ROI's ions have spilled into the second buffer, or B = 2048 -- the
+// single-buffered one
+template <int KS, int NB, bool kHalf, bool kMulti>
+__device__ __forceinline__ void run_seq(const MmaParams &p, const MmaSmem &L, unsigned char *smem, uint32_t tmem, int n, const Seq &sq,
+                                        int64_t m, const float *ions, const float2 *phase, float2 *exch, float2 *cand,
+                                        const PipeShared &ps, int cls)
+{
+    if (NB == 8 || n > p.cap) run_pipeline<KS, NB, true, kHalf, kMulti>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
+    else run_pipeline<KS, NB, false, kHalf, kMulti>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
+}
+
+// KS = K/16 k-steps per group, NB = bin parts (layout), kHalf = half-grid mode, kMulti = several signatures per plan
+template <int KS, int NB, bool kHalf, bool kMulti>
 __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_constant__ MmaParams p)
 {
     extern __shared__ unsigned char smem_raw[];
@@ -830,7 +868,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
     ps.flag = s_flag; ps.nfix = &s_nfix; ps.fix = s_fix;
     uint32_t tmem = 0;
     // ---- one pass per class of signatures (specs with the same type mask): gather, then the group pipeline ---------
-    for (int cls = 0; cls < p.ss.n_classes; ++cls) {
+    const int n_classes = kMulti ? p.ss.n_classes : 1;
+    for (int cls = 0; cls < n_classes; ++cls) {
         if (cls > 0) {
             __syncthreads();                               // the previous class has drained (epilogues done, clears landed)
             if (tid == 0) init_barriers(true);
@@ -847,29 +886,28 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
         __syncthreads();
         asm volatile("tcgen05.fence::after_thread_sync;");
         tmem = s_tmem;
-        if (g.n_accepted) gather_roi3(p, g, rc, cx, cy, cz, ions, &s_n, cls);
+        if (g.n_accepted) gather_roi3<kMulti>(p, g, rc, cx, cy, cz, ions, &s_n, cls);
         __syncthreads();
         const int n = s_n;
-        if (chunk == 0 && tid == 0 && p.counts)
-            for (int sp = 0; sp < p.ss.n_specs; ++sp)
-                if (p.ss.cls_of[sp] == cls) p.counts[(size_t)sp * p.M + m] = (uint32_t)n;
+        if (chunk == 0 && tid == 0 && p.counts) {
+            if (!kMulti) p.counts[m] = (uint32_t)n;
+            else
+                for (int sp = 0; sp < p.ss.n_specs; ++sp)
+                    if (p.ss.cls_of[sp] == cls) p.counts[(size_t)sp * p.M + m] = (uint32_t)n;
+        }
 
         int grp_total = 0;                                     // groups run by this CTA for this class (ordinary + fix-up)
         if (n > p.cap_big) {
             // too many ions even for ion buffer + second histogram buffer: leave this material point to the FFT kernel
             if (chunk == 0 && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
         } else {
-            auto run = [&](const Seq &sq) {
-                if (NB == 8 || n > p.cap) run_pipeline<KS, NB, true, kHalf>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
-                else run_pipeline<KS, NB, false, kHalf>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
-            };
             // half-grid mode: sub-ranges of kSubGroups groups, each followed by the fix-up groups of its flagged pairs
             const int sub = kHalf ? kSubGroups : (g_end - g_begin);
             bool overflow = false;
             for (int sg = g_begin; sg < g_end; sg += sub) {
                 Seq sq;
                 sq.mode = 0; sq.g0 = sg; sq.ngrp = min(sub, g_end - sg); sq.grp_base = grp_total; sq.nfix = 0;
-                run(sq);
+                run_seq<KS, NB, kHalf, kMulti>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
                 grp_total += sq.ngrp;
                 if (kHalf) {
                     __syncthreads();                           // every epilogue of the sub-range is done, the list is complete
@@ -878,7 +916,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
                     if (tid == 0) s_nfix = 0;
                     if (nf > kFixCap) overflow = true;         // pathological input: the FFT kernel redoes this material point
                     sq.mode = 1; sq.nfix = min(nf, kFixCap); sq.ngrp = (sq.nfix + Lay<NB>::G - 1) / Lay<NB>::G; sq.grp_base = grp_total;
-                    if (sq.ngrp) run(sq);
+                    if (sq.ngrp) run_seq<KS, NB, kHalf, kMulti>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
                     grp_total += sq.ngrp;
                     __syncthreads();                           // the list is consumed before the next sub-range appends
                 }
@@ -1171,7 +1209,7 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
 #ifdef APX_TRACE
     q.trace = p->dbg_trace; q.trace_block = p->dbg_trace_block; q.trace_cap = p->dbg_trace_cap;
 #endif
-    q.ss = p->specs;
+    q.ss = p->specs; q.norm0 = p->specs.norm[0];
     q.D = p->D; q.B = p->B; q.k_lo = p->k_lo; q.W = p->W; q.N = mma_n_for(p->W);
     q.nl = 0;
     while ((8 << q.nl) < p->B) ++q.nl;
@@ -1199,17 +1237,16 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
         kern<<<(unsigned)blocks, kMmaThreads, L.total, st>>>(q);
         return cudaSuccess;
     };
-    if (p->mma_paired) {
-        if (p->B == 2048) e = launch(k_signature_mma<16, 8, true>);
-        else if (p->B == 1024) e = launch(k_signature_mma<16, 4, true>);
-        else if (p->B == 512) e = launch(k_signature_mma<8, 4, true>);
-        else e = launch(k_signature_mma<4, 4, true>);
-    } else {
-        if (p->B == 2048) e = launch(k_signature_mma<16, 8, false>);
-        else if (p->B == 1024) e = launch(k_signature_mma<16, 4, false>);
-        else if (p->B == 512) e = launch(k_signature_mma<8, 4, false>);
-        else e = launch(k_signature_mma<4, 4, false>);
-    }
+    const bool multi = p->specs.n_specs > 1;
+    auto pick = [&](auto half_tag, auto multi_tag) -> cudaError_t {
+        constexpr bool H = decltype(half_tag)::value, Mu = decltype(multi_tag)::value;
+        if (p->B == 2048) return launch(k_signature_mma<16, 8, H, Mu>);
+        if (p->B == 1024) return launch(k_signature_mma<16, 4, H, Mu>);
+        if (p->B == 512) return launch(k_signature_mma<8, 4, H, Mu>);
+        return launch(k_signature_mma<4, 4, H, Mu>);
+    };
+    if (p->mma_paired) e = multi ? pick(std::true_type{}, std::true_type{}) : pick(std::true_type{}, std::false_type{});
+    else e = multi ? pick(std::false_type{}, std::true_type{}) : pick(std::false_type{}, std::false_type{});
     if (e != cudaSuccess) return e;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;

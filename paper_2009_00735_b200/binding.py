@@ -21,7 +21,7 @@ EXPORTS = ["apx_plan_create", "apx_plan_destroy", "apx_plan_constants", "apx_pla
            "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_dirs_antipodes", "apx_strerror", "apx_version"]
 PEAK_EXPORTS = ["apx_peak_name", "apx_peak_measure"]          # include/aptsig_peaks.h
 EXT_EXPORTS = ["apx_intensity_max", "apx_refine_select", "apx_refine_centres", "apx_indexer_create", "apx_indexer_destroy",
-               "apx_indexer_nodes", "apx_indexer_lut", "apx_last_cuda_error_indexer", "apx_index", "apx_so3_grid_cubic", "apx_fsp"]   # aptsig_ext.h
+               "apx_indexer_nodes", "apx_indexer_lut", "apx_last_cuda_error_indexer", "apx_index", "apx_so3_grid_cubic", "apx_fsp", "apx_fsp_set_path"]   # aptsig_ext.h
 APX_INDEX_MAX_K = 8
 
 
@@ -97,6 +97,7 @@ def _lib():
         L.apx_index.argtypes = [vp, vp, vp, i64, i32, vp, vp, vp]
         L.apx_so3_grid_cubic.argtypes = [f32, vp, C.POINTER(i64)]
         L.apx_fsp.argtypes = [vp, vp, i64, f32, i32, vp, vp, vp]
+        L.apx_fsp_set_path.argtypes = [vp, i32]
         for name in EXT_EXPORTS:
             getattr(L, name).restype = C.c_int
         L.apx_peak_name.argtypes = [C.c_int]
@@ -344,6 +345,9 @@ class Plan:
                                               self._stream(stream)), "apx_refine_centres")
 
     # ---- include/aptsig_ext.h: reciprocal space method (NEXT-3) ------------------------------------------------
+    def apx_fsp_set_path(self, path):
+        self._check(_lib().apx_fsp_set_path(self._h, int(path)), "apx_fsp_set_path")
+
     def apx_fsp(self, centres, k_max, L, out, counts=None, stream=None):
         M, dev, L = int(centres.shape[0]), self.device, int(L)
         self._check(_lib().apx_fsp(self._h, _arg(centres, "centres", np.float32, (M, 3), dev), M, float(k_max), L,

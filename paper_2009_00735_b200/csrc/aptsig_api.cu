@@ -64,7 +64,7 @@ extern "C" int apx_plan_destroy(apx_plan *p)
 {
     if (!p) return APX_OK;
     DeviceGuard guard(p->device);
-    void *bufs[] = {p->dbg_centre, p->dbg_sig, p->d_refine_off, p->d_kaxis, p->d_dirs_scaled, p->d_twiddle, p->d_mma_table, p->d_mma_zero, p->d_mma_phase, p->d_dirs_sorted, p->d_dir_perm, p->d_dir_perm_mirror, p->d_type_mask, p->d_grid, p->d_cell_start,
+    void *bufs[] = {p->dbg_centre, p->dbg_sig, p->d_refine_off, p->d_kaxis, p->d_fsp_list, p->d_dirs_scaled, p->d_twiddle, p->d_mma_table, p->d_mma_zero, p->d_mma_phase, p->d_dirs_sorted, p->d_dir_perm, p->d_dir_perm_mirror, p->d_type_mask, p->d_grid, p->d_cell_start,
                     p->d_cell_cursor, p->d_scan_tiles, p->d_cell_of_ion, p->d_sorted, p->d_deferred, p->h2d_xyz, p->h2d_types, p->h2d_centres,
                     p->d2h_sig, p->d2h_counts};
     for (void *b : bufs)

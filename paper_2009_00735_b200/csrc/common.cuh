@@ -74,6 +74,9 @@ struct Plan {
     float *d_refine_off;           // [16] sub-cell centre offsets of apx_refine_centres
     float *d_kaxis;                // [cap_kaxis] k values of one axis of apx_fsp's reciprocal-space grid
     int cap_kaxis;
+    int fsp_path;                  // 0 = tensor-core kernel (+ FP32 kernel for oversized ROIs), 1 = FP32 kernel only
+    uint32_t *d_fsp_list;          // [0] count, [1..] material points k_fsp_mma left to k_fsp
+    int64_t cap_fsp_list;
     uint32_t *d_type_mask;         // [8] words
     GridParams *d_grid;
     uint32_t *d_cell_start;        // [kMaxCells + 1]
@@ -146,6 +149,8 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
 bool mma_path_supported(const Plan *p);
 cudaError_t mma_path_prepare(Plan *p);   // builds d_mma_table
 cudaError_t mma_reserve_deferred(Plan *p, int64_t need);   // deferred list of at least `need` words
+cudaError_t launch_fsp_mma(Plan *p, const float *centres, int64_t M, int L, float dk, float *out, uint32_t *counts, uint32_t *list,
+                           cudaStream_t st);
 cudaError_t mma_reserve_for(Plan *p, int64_t M);           // ... sized for any apx_query of up to M material points
 
 }  // namespace apx

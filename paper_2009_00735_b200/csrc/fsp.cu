@@ -28,6 +28,8 @@ struct FspParams {
     const float *kaxis;       // [L] k values of one axis, fp64 on the host rounded once to fp32
     float *out;               // [M][L][L][L] amplitude
     uint32_t *counts;
+    const uint32_t *list;     // nullptr: every material point; else list[0] = count, list[1..] = the material points to serve
+                              // (those the tensor-core kernel k_fsp_mma left out: more ions than its shared buffer)
     int L, tiles;             // tiles per axis = ceil(L / 64)
     float R, R2;
 };
@@ -53,12 +55,16 @@ __global__ void __launch_bounds__(kFspThreads, 2) k_fsp(const FspParams p)
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int L = p.L;
-    int b = blockIdx.x;
-    const int tx_tile = b % p.tiles; b /= p.tiles;
-    const int ty_tile = b % p.tiles; b /= p.tiles;
-    const int iz = b % L;
-    const int64_t m = b / L;
     const GridParams g = *p.grid;
+    const int64_t per_point = (int64_t)L * p.tiles * p.tiles;
+    const int64_t n_items = p.list ? (int64_t)p.list[0] * per_point : (int64_t)gridDim.x;
+  for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+    int64_t b = item;
+    const int tx_tile = (int)(b % p.tiles); b /= p.tiles;
+    const int ty_tile = (int)(b % p.tiles); b /= p.tiles;
+    const int iz = (int)(b % L);
+    const int64_t m = p.list ? (int64_t)p.list[1 + b / L] : b / L;
+    __syncthreads();                                  // the previous item is done with the shared buffers
     const float cx = p.centres[3 * m], cy = p.centres[3 * m + 1], cz = p.centres[3 * m + 2];
     const RoiCells rc = roi_cells(g, cx, cy, cz, p.R);
     const int ny_r = rc.iy1 - rc.iy0 + 1, nz_r = rc.iz1 - rc.iz0 + 1;
@@ -175,18 +181,26 @@ __global__ void __launch_bounds__(kFspThreads, 2) k_fsp(const FspParams p)
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const int iy = iy0 + 4 * ty + i;
-        if (iy >= L) continue;
+        if (iy >= L) break;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const int ix = ix0 + 4 * tx + j;
             if (ix < L) o[(size_t)iy * L + ix] = sqrtf(cr[i][j] * cr[i][j] + ci[i][j] * ci[i][j]);
         }
     }
+  }
 }
 
 }  // namespace apx
 
 using namespace apx;
+
+extern "C" int apx_fsp_set_path(apx_plan *p, int32_t path)
+{
+    if (!p || (path != 0 && path != 1)) return APX_EINVAL;
+    p->fsp_path = path;
+    return APX_OK;
+}
 
 extern "C" int apx_fsp(apx_plan *p, const float *centres, int64_t M, float k_max, int32_t L, float *out, uint32_t *counts,
                        void *stream)
@@ -212,15 +226,35 @@ extern "C" int apx_fsp(apx_plan *p, const float *centres, int64_t M, float k_max
     for (int i = 0; i < L; ++i) kax[i] = L == 1 ? 0.0f : (float)(-(double)k_max + (double)i * (2.0 * (double)k_max / (double)(L - 1)));
     cudaError_t e = cudaMemcpyAsync(p->d_kaxis, kax, sizeof(float) * L, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cu(e);
-    FspParams q;
-    q.sorted = p->d_sorted; q.cell_start = p->d_cell_start; q.grid = p->d_grid; q.centres = centres; q.kaxis = p->d_kaxis;
-    q.out = out; q.counts = counts; q.L = L; q.tiles = (L + kFspTile - 1) / kFspTile; q.R = p->R; q.R2 = p->R2;
-    const int64_t blocks = M * L * q.tiles * q.tiles;
-    if (blocks > 0x7FFFFFFFLL) return done(APX_ERANGE);
+    const int tiles = (L + kFspTile - 1) / kFspTile;
     const size_t smem = sizeof(float) * (4 * kFspStep * kFspTile + 4 * kFspStep + 3 * kFspCap);
     e = cudaFuncSetAttribute(k_fsp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return cu(e);
-    k_fsp<<<(unsigned)blocks, kFspThreads, smem, st>>>(q);
+    FspParams q;
+    q.sorted = p->d_sorted; q.cell_start = p->d_cell_start; q.grid = p->d_grid; q.centres = centres; q.kaxis = p->d_kaxis;
+    q.out = out; q.counts = counts; q.list = nullptr; q.L = L; q.tiles = tiles; q.R = p->R; q.R2 = p->R2;
+    if (p->fsp_path == 1) {
+        // FP32 pipe only
+        const int64_t blocks = M * L * tiles * tiles;
+        if (blocks > 0x7FFFFFFFLL) return done(APX_ERANGE);
+        k_fsp<<<(unsigned)blocks, kFspThreads, smem, st>>>(q);
+    } else {
+        // tensor cores (fsp_mma.cu); the material points it leaves out (more ions than its shared buffer) are appended to a
+        // device list and served by the FP32 kernel in the same stream
+        if (M + 1 > p->cap_fsp_list) {
+            if (p->d_fsp_list) cudaFree(p->d_fsp_list);
+            p->d_fsp_list = nullptr; p->cap_fsp_list = 0;
+            e = cudaMalloc(&p->d_fsp_list, (size_t)(M + 1) * 4);
+            if (e != cudaSuccess) return cu(e);
+            p->cap_fsp_list = M + 1;
+        }
+        e = cudaMemsetAsync(p->d_fsp_list, 0, 4, st);
+        if (e != cudaSuccess) return cu(e);
+        e = launch_fsp_mma(p, centres, M, L, L == 1 ? 0.0f : (float)(2.0 * (double)k_max / (double)(L - 1)), out, counts, p->d_fsp_list, st);
+        if (e != cudaSuccess) return cu(e);
+        q.list = p->d_fsp_list;
+        k_fsp<<<(unsigned)(p->sm_count * 2), kFspThreads, smem, st>>>(q);
+    }
     e = cudaGetLastError();
     if (e != cudaSuccess) return cu(e);
     return done(APX_OK);

@@ -217,7 +217,7 @@ def test_index_many_points_chunks_and_prenormalised_input():
 
 
 # ---- NEXT-3 ------------------------------------------------------------------------------------------------------
-def _fsp_check(plan, xyz, types, centres, R, k_max, L, accepted=None):
+def _fsp_check(plan, xyz, types, centres, R, k_max, L, accepted=None, path=0):
     """|F| of apx_fsp against Eq. 2 written out in fp64 (oracle), element by element.  Tolerance:
     the fp32 phase k.d carries <= 3 roundings of relative 6e-8 on |k.d| <= sqrt3 k_max R cycles, i.e. a phase error of
     about 2 pi * 2e-7 * sqrt3 k_max R per ion, and the sum over N_w ions at most N_w times that."""
@@ -226,6 +226,7 @@ def _fsp_check(plan, xyz, types, centres, R, k_max, L, accepted=None):
     M = len(centres)
     out = torch.full((M, L, L, L), -7.0, dtype=torch.float32, device=dev)
     cnt = torch.full((M,), -1, dtype=torch.int32, device=dev)
+    plan.apx_fsp_set_path(path)                                                 # 0 = tensor cores (+ FP32 for big ROIs), 1 = FP32 pipe
     plan.apx_fsp(torch.from_numpy(centres).to(dev), k_max, L, out, cnt)
     torch.cuda.synchronize()
     got, gc = out.cpu().numpy(), cnt.cpu().numpy()
@@ -251,14 +252,16 @@ def test_fsp_against_oracle_small_grids():
     plan = apx.Plan(R, 256, O.dirs_fibonacci(8), k_lo=7, k_hi=17, device=0)
     plan.apx_ingest(torch.from_numpy(xyz).to(dev), torch.from_numpy(types).to(dev))
     centres = np.array([[0, 0, 0], [0.4, -0.3, 0.2], [2.6, 0, 0], [9, 9, 9]], np.float32)       # full, shifted, partial, empty
-    for L, k_max in ((9, 5.0), (16, 2.0 * math.pi), (33, 6.0), (1, 3.0)):
-        gc = _fsp_check(plan, xyz, types, centres, R, k_max, L)
-        assert gc[3] == 0 and gc[0] > 300
+    for path in (0, 1):
+        for L, k_max in ((9, 5.0), (16, 2.0 * math.pi), (33, 6.0), (1, 3.0)):
+            gc = _fsp_check(plan, xyz, types, centres, R, k_max, L, path=path)
+            assert gc[3] == 0 and gc[0] > 300
     plan.apx_plan_destroy()
     # with an ion-type filter (Eq. 2: "all atoms N_w of a selected atom type")
     plan = apx.Plan(R, 256, O.dirs_fibonacci(8), k_lo=7, k_hi=17, accepted_types={1}, device=0)
     plan.apx_ingest(torch.from_numpy(xyz).to(dev), torch.from_numpy(types).to(dev))
-    _fsp_check(plan, xyz, types, centres[:2], R, 5.0, 9, accepted={1})
+    for path in (0, 1):
+        _fsp_check(plan, xyz, types, centres[:2], R, 5.0, 9, accepted={1}, path=path)
     plan.apx_plan_destroy()
 
 
@@ -272,19 +275,21 @@ def test_fsp_bragg_peak_and_multi_tile_grid():
     plan = apx.Plan(R, 256, O.dirs_fibonacci(8), k_lo=7, k_hi=17, device=0)
     plan.apx_ingest(torch.from_numpy(xyz).to(dev), None)
     L, k_max = 81, 5.0
-    out = torch.empty((1, L, L, L), dtype=torch.float32, device=dev)
-    cnt = torch.empty(1, dtype=torch.int32, device=dev)
-    plan.apx_fsp(torch.zeros((1, 3), dtype=torch.float32, device=dev), k_max, L, out, cnt)
-    torch.cuda.synchronize()
-    F, n = out.cpu().numpy()[0], int(cnt.item())
-    c = L // 2
-    assert F[c, c, c] == pytest.approx(n, rel=1e-6)                               # F(0) = N_w
-    for idx in ((c, c, 0), (c, c, L - 1), (c, 0, c), (L - 1, c, c)):               # k = (+-2/a, 0, 0) etc.
-        assert F[idx] == pytest.approx(n, rel=1e-4)
     rel = O.members(xyz, None, np.zeros(3, np.float32), R)
     ref = np.abs(X.fsp(rel, k_max, L))
-    tol = 1e-4 * ref + n * (2e-6 + 2 * math.pi * 2e-7 * math.sqrt(3) * k_max * R)
-    assert (np.abs(F - ref) <= tol).all()
+    for path in (0, 1):
+        out = torch.full((1, L, L, L), -7.0, dtype=torch.float32, device=dev)
+        cnt = torch.empty(1, dtype=torch.int32, device=dev)
+        plan.apx_fsp_set_path(path)
+        plan.apx_fsp(torch.zeros((1, 3), dtype=torch.float32, device=dev), k_max, L, out, cnt)
+        torch.cuda.synchronize()
+        F, n = out.cpu().numpy()[0], int(cnt.item())
+        c = L // 2
+        assert F[c, c, c] == pytest.approx(n, rel=1e-6)                           # F(0) = N_w
+        for idx in ((c, c, 0), (c, c, L - 1), (c, 0, c), (L - 1, c, c)):           # k = (+-2/a, 0, 0) etc.
+            assert F[idx] == pytest.approx(n, rel=1e-4)
+        tol = 1e-4 * ref + n * (2e-6 + 2 * math.pi * 2e-7 * math.sqrt(3) * k_max * R)
+        assert (np.abs(F - ref) <= tol).all(), (path, np.abs(F - ref).max())
     plan.apx_plan_destroy()
 
 
@@ -293,9 +298,12 @@ def test_fsp_streams_rois_larger_than_the_shared_ion_buffer():
     dev = torch.device("cuda:0")
     xyz = np.ascontiguousarray(lattice_in_ball(0.405, fcc_basis, random_rotation(_rng(4)), (0, 0, 0), 4.0).astype(np.float32))
     types = np.zeros(len(xyz), np.uint8)
-    R = 3.3                                                                      # ~9000 ions > 6144
-    plan = apx.Plan(R, 256, O.dirs_fibonacci(8), k_lo=7, k_hi=17, device=0)
-    plan.apx_ingest(torch.from_numpy(xyz).to(dev), torch.from_numpy(types).to(dev))
-    gc = _fsp_check(plan, xyz, types, np.array([[0.1, 0.2, -0.1]], np.float32), R, 4.0, 12)
-    assert gc[0] > 6144
-    plan.apx_plan_destroy()
+    # ~9000 ions > 6144: the FP32 kernel streams the cell rows; ~5100 ions: more than the tensor-core kernel holds (4096) but
+    # within the FP32 kernel's buffer; with a small ROI riding along so that the deferred list is shorter than M
+    for R, lo, hi in ((3.3, 6144, 10 ** 6), (2.75, 4096, 6144)):
+        plan = apx.Plan(R, 256, O.dirs_fibonacci(8), k_lo=7, k_hi=17, device=0)
+        plan.apx_ingest(torch.from_numpy(xyz).to(dev), torch.from_numpy(types).to(dev))
+        for path in (0, 1):
+            gc = _fsp_check(plan, xyz, types, np.array([[0.1, 0.2, -0.1], [3.9, 0.0, 0.0]], np.float32), R, 4.0, 12, path=path)
+            assert lo < gc[0] <= hi and gc[1] < 4096
+        plan.apx_plan_destroy()

@@ -318,20 +318,36 @@ def run_fsp(args):
     out = torch.empty((M, L, L, L), dtype=torch.float32, device=dev)
     cnt = torch.empty(M, dtype=torch.int32, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    plan.apx_fsp_set_path(args.fsp_path)
     ms = _time_steps(torch, lambda: plan.apx_fsp(centres, 2.0 * np.pi, L, out, cnt), args.steps, args.warmup, flush)
     nw = float(cnt.cpu().numpy().astype(np.int64).sum())
-    flops = 8.0 * nw * L ** 3
+    flops = 8.0 * nw * L ** 3                                  # Eq. 2: one complex multiply-add per (ion, k point)
     pk = load_peaks()
-    achieved = flops / (ms * 1e-3) / 1e12
+    if args.fsp_path == 1:
+        bound, kernel, peak, unit = "alu", "k_fsp", pk["fp32_tflops"], "TFLOP/s"
+        achieved, src = flops / (ms * 1e-3) / 1e12, pk["source"]
+        model = "8 flop (one complex multiply-add) per (ion, k point) on the FP32 pipe"
+    else:
+        # tensor-core kernel: the complex contraction as one real GEMM (8 flop per (ion, k point)) executed three times
+        # (Ah Bh, Ah Bl, Al Bh of the fp16 hi + lo split): executed tensor flops = 3 x model flops
+        try:
+            peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["bf16_tflops"]
+            src = "MEASURED_PEAKS.json bf16_tflops (burst, kernel timed alone; fp16 has the same nominal rate as bf16)"
+        except Exception:
+            peak, src = 1600.0, "fallback (B200_PROFILING.md)"
+        bound, kernel, unit = "tensor", "k_fsp_mma", "TFLOP/s"
+        achieved = 3.0 * flops / (ms * 1e-3) / 1e12
+        model = "executed fp16 tensor flops = 3 GEMMs (hi*hi, hi*lo, lo*hi) x 8 flop per (ion, k point)"
     print(json.dumps({"metric": "FSP k-points/s", "value": float(M) * L ** 3 / (ms * 1e-3), "unit": "k-points/s", "n_gpus": 1,
                       "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
-                      "dtype": "f32", "data": "synthetic",
+                      "dtype": "f32" if args.fsp_path == 1 else "f16 hi+lo split operands, f32 accumulate", "data": "synthetic",
                       "config": {"workload": f"FSP (Eq. 2): {M} ROIs of config 2 (R = 2.0 nm, mean {nw / M:.0f} ions) x {L}^3 k points, "
-                                             "k_max = 2 pi / nm", "rois_per_s": M / (ms * 1e-3)},
-                      "gpu_launches": args.steps,
-                      "roofline": {"bound": "alu", "kernel": "k_fsp", "achieved": achieved, "peak": pk["fp32_tflops"],
-                                   "unit": "TFLOP/s", "frac": achieved / pk["fp32_tflops"], "traffic": None,
-                                   "peak_source": pk["source"], "model": "8 flop (one complex multiply-add) per (ion, k point)"}}))
+                                             "k_max = 2 pi / nm", "rois_per_s": M / (ms * 1e-3),
+                                 "kernel_path": "fp32" if args.fsp_path == 1 else "tensor"},
+                      "gpu_launches": (1 if args.fsp_path == 1 else 2) * args.steps,
+                      "roofline": {"bound": bound, "kernel": kernel, "achieved": achieved, "peak": peak,
+                                   "unit": unit, "frac": achieved / peak, "traffic": None, "peak_source": src, "model": model,
+                                   "model_tflops": flops / (ms * 1e-3) / 1e12}}))
     plan.apx_plan_destroy()
 
 
@@ -499,8 +515,14 @@ def run_ours(args, rank, world, local_rank):
     h2d = w.xyz.nbytes + w.types.nbytes + Me * 12
     d2h = Me * D * 8 + Me * 4
     bound_is_atom = atom_frac >= fp32_frac
+    # counters of the committed ncu capture, scaled from the material points it ran on to those of this run (DRAM traffic is
+    # the 8 B per histogram of output, shared-memory wavefronts follow the pairs: both linear in the material points)
+    cap_pts = ncu_constant(kname, cfg, "points") or M_all
+    scale = M_tot / world / cap_pts
     traffic = ncu_constant(kname, cfg, "dram_bytes")
+    traffic = traffic * scale if traffic else None
     lsu = ncu_constant(kname, cfg, "lsu_wavefronts_shared")
+    lsu = lsu * scale * world if lsu else None
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
@@ -578,6 +600,7 @@ def main():
     ap.add_argument("--fsp", action="store_true", help="time the reciprocal space method (Eq. 2, NEXT-3)")
     ap.add_argument("--fsp-points", type=int, default=1000)
     ap.add_argument("--fsp-L", type=int, default=64)
+    ap.add_argument("--fsp-path", type=int, default=0, choices=[0, 1], help="0 = tensor-core kernel, 1 = FP32-pipe kernel")
     ap.add_argument("--peaks", action="store_true", help="run the on-chip peak microbenchmarks and write --peaks-out")
     ap.add_argument("--peaks-out", default=PEAKS_JSON)
     ap.add_argument("--peak-iters", type=int, default=20000)

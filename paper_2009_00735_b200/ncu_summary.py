@@ -70,6 +70,7 @@ def main():
     ap.add_argument("--config", required=True, help="BASELINE.json config number the capture ran on")
     ap.add_argument("--command", required=True, help="the full command that produced the report")
     ap.add_argument("--note", default="")
+    ap.add_argument("--points", type=int, default=0, help="material points of the captured launch (0 = the whole config)")
     args = ap.parse_args()
     names, units, launches = read_report(args.report)
     col = {n: i for i, n in enumerate(names)}
@@ -97,6 +98,7 @@ def main():
                       "lsu_wavefronts_shared": val("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum"),
                       "lsu_wavefronts_shared_atom": val("l1tex__data_pipe_lsu_wavefronts_mem_shared_op_atom.sum"),
                       "inst_executed": val("smsp__inst_executed.sum"),
+                      "points": args.points,
                       "capture": f"profiles/{args.name}.md"}
     os.makedirs(os.path.join(ROOT, "profiles"), exist_ok=True)
     with open(os.path.join(ROOT, "profiles", args.name + ".md"), "w") as f:

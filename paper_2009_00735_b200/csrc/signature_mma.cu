@@ -311,13 +311,13 @@ __device__ __noinline__ void flag_pair(uint32_t *flag, int *nfix, uint16_t *fix,
     }
 }
 // two ions (dx0,dx1), (dy0,dy1), (dz0,dz1) for this lane's direction
-// kDetect: nonint2 (packed fp32 pair) accumulates, per component, the number of projections that are NOT exact integers:
-// RU(x + magic) - RD(x + magic) is exactly 1.0f for a non-integer x and 0.0f for an integer (adjacent floats with ulp 1), so
-// the test costs three packed FP instructions per two ions and no integer work.
+// kDetect: nonint accumulates the number of the projections that are NOT exact integers: the bit patterns of RU(x + magic)
+// and RD(x + magic) differ by exactly 1 for a non-integer x and by 0 for an integer.  (A packed-FP variant of the count --
+// FADD2.RP, packed subtract, packed add -- was measured slower: it moves work to the FMA pipe the projections already load.)
 template <bool kDetect, int BLK>
 __device__ __forceinline__ void bin_pair(float dx0, float dx1, float dy0, float dy1, float dz0, float dz1, uint64_t nx2,
                                          uint64_t ny2, uint64_t nz2, uint64_t ma2, uint64_t sc2, uint64_t mb2, uint32_t kz,
-                                         uint32_t k0, uint32_t inc, uint64_t &nonint2)
+                                         uint32_t k0, uint32_t inc, uint32_t &nonint)
 {
     uint64_t t, ua, va;
     asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(t) : "l"(nx2), "l"(pack2(dx0, dx1)));
@@ -331,24 +331,8 @@ __device__ __forceinline__ void bin_pair(float dx0, float dx1, float dy0, float 
     if (kDetect) {
         uint64_t up;
         asm("add.rp.f32x2 %0, %1, %2;" : "=l"(up) : "l"(t), "l"(ma2));
-#ifndef APX_DETECT_FP
-        // integer variant: RU - RD of the bit patterns, accumulated in the low word of nonint2
-        nonint2 += (uint64_t)(((uint32_t)up - ua0) + ((uint32_t)(up >> 32) - ua1));
-#else
-        uint64_t d;
-        asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(up), "l"(ua));              // exact: (0 or 1, 0 or 1)
-        asm("add.rn.f32x2 %0, %1, %2;" : "=l"(nonint2) : "l"(nonint2), "l"(d));
-#endif
+        nonint += ((uint32_t)up - ua0) + ((uint32_t)(up >> 32) - ua1);
     }
-}
-__device__ __forceinline__ float sum2(uint64_t v)
-{
-#ifndef APX_DETECT_FP
-    return (float)(uint32_t)v;
-#endif
-    float lo, hi;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-    return lo + hi;
 }
 
 // One direction pair of a lane: set A (low u16, increment 1) and set B (high u16, increment 65536) of the same word.
@@ -373,7 +357,7 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
             float4 q[6];
 #pragma unroll
             for (int u = 0; u < 6; ++u) q[u] = lds128(src + (uint32_t)u * 16u);
-            uint64_t na = 0ull, nb = 0ull;                    // packed (0.0f, 0.0f)
+            uint32_t na = 0u, nb = 0u;
 #pragma unroll
             for (int hh = 0; hh < 2; ++hh) {
                 const float4 X = q[3 * hh], Y = q[3 * hh + 1], Z = q[3 * hh + 2];
@@ -383,21 +367,21 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
                 bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, nb);
             }
             if (kDetect) {
-                if (__builtin_expect(sum2(na) != 8.0f, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
-                if (__builtin_expect(sum2(nb) != 8.0f, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
+                if (__builtin_expect(na != 8u, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
+                if (__builtin_expect(nb != 8u, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
             }
         }
         if (ib + 4 * NS <= i1) {                             // one quad per stream
             const uint32_t a = ions_s + (uint32_t)ib * 12u + (uint32_t)h * 48u;
             const float4 X = lds128(a), Y = lds128(a + 16u), Z = lds128(a + 32u);
-            uint64_t na = 0ull, nb = 0ull;
+            uint32_t na = 0u, nb = 0u;
             bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, na);
             bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, ax2, ay2, az2, ma2, sc2, mb2, c.kz, k0, 1u, na);
             bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, nb);
             bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, nb);
             if (kDetect) {
-                if (__builtin_expect(sum2(na) != 4.0f, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
-                if (__builtin_expect(sum2(nb) != 4.0f, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
+                if (__builtin_expect(na != 4u, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
+                if (__builtin_expect(nb != 4u, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
             }
             ib += 4 * NS;
         }

@@ -220,11 +220,11 @@ __host__ __device__ inline MmaSmem mma_smem_layout(int B, int N, int W, int cap)
 // whose register pairs are the operands of the packed fp32x2 arithmetic of the binning warps.
 template <bool kMulti>
 __device__ __forceinline__ void gather_roi3(const MmaParams &p, const GridParams &g, const RoiCells &rc,
-                                            float cx, float cy, float cz, float *ions, int *s_n, int cls)
+                                            float cx, float cy, float cz, float *ions, int *s_n, int cls, int nwarps)
 {
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;     // warps 0 .. nwarps-1 gather
     const int ny_r = rc.iy1 - rc.iy0 + 1, nz_r = rc.iz1 - rc.iz0 + 1;
-    for (int row = wid; row < ny_r * nz_r; row += kMmaWarps) {
+    for (int row = wid; row < ny_r * nz_r; row += nwarps) {
         int iy = rc.iy0 + row % ny_r, iz = rc.iz0 + row / ny_r;
         int base = (iz * g.ny + iy) * g.nx;
         uint32_t beg = p.cell_start[base + rc.ix0], end = p.cell_start[base + rc.ix1 + 1];
@@ -271,18 +271,16 @@ __device__ __forceinline__ uint64_t pack2(float lo, float hi)
     asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
     return r;
 }
-struct Detect;
-__device__ void flag_pair(uint32_t *flag, int *nfix, uint16_t *fix, uint32_t bit, uint32_t id);
 template <bool kClamp, bool kDetect, int BLK>
-__device__ __forceinline__ void bin_one(float dx, float dy, float dz, float npx, float npy, float npz, const BinConst &c,
-                                        uint32_t k0, uint32_t inc, uint32_t *flag, int *nfix, uint16_t *fix, uint32_t bit, uint32_t id)
+__device__ __forceinline__ bool bin_one(float dx, float dy, float dz, float npx, float npy, float npz, const BinConst &c,
+                                        uint32_t k0, uint32_t inc)
 {
     float x = __fmaf_rn(npz, dz, __fmaf_rn(npy, dy, __fmul_rn(npx, dx)));
     if (kClamp) x = fminf(fmaxf(x, -c.half_b), c.half_b - 0.25f);
     const uint32_t ua = __float_as_uint(__fadd_rd(x, c.magic_a));
-    if (kDetect && ua == __float_as_uint(__fadd_ru(x, c.magic_a))) flag_pair(flag, nfix, fix, bit, id);
     const uint32_t va = __float_as_uint(__fmaf_rd(x, c.scl, c.magic_b));
     red_shared_add(ua * (uint32_t)BLK + (va * c.kz + k0), inc);
+    return kDetect && ua == __float_as_uint(__fadd_ru(x, c.magic_a));      // true: x is an exact integer
 }
 // Half-grid mode (antipodally symmetric direction grids such as the geodesic mesh of the paper, L60): only one
 // direction v of every pair (v, -v) is binned.  x(-v) = -x(v) bit for bit (every product and sum is negated exactly), so
@@ -296,18 +294,30 @@ __device__ __forceinline__ void bin_one(float dx, float dy, float dz, float npx,
 constexpr int kFlagSlots = 8;
 constexpr int kFixCap = 512;             // flagged pairs per sub-range of kSubGroups groups
 constexpr int kSubGroups = 128;
-struct Detect {
-    uint32_t *flag;                      // bit s = slot s of this group has met an exact-integer projection
-    int *nfix;
-    uint16_t *fix;                       // flagged pairs: (group within the sub-range) * 32 + slot
-    uint32_t bit, id;
+// Shared state of the flagging: one struct so that the rarely-taken path needs one base address.
+struct FixShared {
+    uint32_t flag[kFlagSlots];           // flag word per group in flight: bit s = slot s has met an exact-integer projection
+    int nfix;                            // number of listed pairs of the sub-range
+    uint16_t fix[kFixCap];               // flagged pairs: (group within the sub-range) * G + slot
 };
-__device__ __noinline__ void flag_pair(uint32_t *flag, int *nfix, uint16_t *fix, uint32_t bit, uint32_t id)
+// What a binning lane needs to flag one of its two pairs -- two registers, opaque to the compiler (it would otherwise
+// re-derive the addresses from the thread id and the shared-memory window inside the hot loop):
+//   base_s = shared-space address of the FixShared; ctx = flag slot | lane word l << 4 | (group within sub-range * G) << 16
+struct Detect {
+    uint32_t base_s, ctx;
+};
+// set = 0: the lane's set-A direction (slot l), 1: its set-B direction (slot LW + l)
+template <int LW>
+__device__ __noinline__ void flag_pair(uint32_t base_s, uint32_t ctx, uint32_t set)
 {
-    const uint32_t old = atomicOr(flag, bit);
+    const uint32_t slot = ((ctx >> 4) & 0xFFFu) + set * (uint32_t)LW, bit = 1u << slot, id = (ctx >> 16) + slot;
+    uint32_t old;
+    asm volatile("atom.shared.or.b32 %0, [%1], %2;" : "=r"(old) : "r"(base_s + 4u * (ctx & 15u)), "r"(bit) : "memory");
     if (!(old & bit)) {
-        const int i = atomicAdd(nfix, 1);
-        if (i < kFixCap) fix[i] = (uint16_t)id;
+        uint32_t i;
+        asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(i) : "r"(base_s + (uint32_t)offsetof(FixShared, nfix)) : "memory");
+        if (i < (uint32_t)kFixCap)
+            asm volatile("st.shared.u16 [%0], %1;" ::"r"(base_s + (uint32_t)offsetof(FixShared, fix) + 2u * i), "h"((uint16_t)id) : "memory");
     }
 }
 // two ions (dx0,dx1), (dy0,dy1), (dz0,dz1) for this lane's direction
@@ -344,7 +354,7 @@ struct LaneDirs {
 // so one ion load serves two (ion, direction) pairs.
 template <bool kClamp, bool kDetect, int NB>
 __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const LaneDirs &n, const BinConst &c, uint32_t k0,
-                                         int h, const Detect &da, const Detect &db)
+                                         int h, const Detect &dt)
 {
     constexpr int NS = Lay<NB>::NS, BLK = Lay<NB>::BLK;
     int ib = i0;
@@ -367,8 +377,8 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
                 bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, nb);
             }
             if (kDetect) {
-                if (__builtin_expect(na != 8u, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
-                if (__builtin_expect(nb != 8u, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
+                if (__builtin_expect(na != 8u, 0)) flag_pair<Lay<NB>::LW>(dt.base_s, dt.ctx, 0u);
+                if (__builtin_expect(nb != 8u, 0)) flag_pair<Lay<NB>::LW>(dt.base_s, dt.ctx, 1u);
             }
         }
         if (ib + 4 * NS <= i1) {                             // one quad per stream
@@ -380,8 +390,8 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
             bin_pair<kDetect, BLK>(X.x, X.y, Y.x, Y.y, Z.x, Z.y, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, nb);
             bin_pair<kDetect, BLK>(X.z, X.w, Y.z, Y.w, Z.z, Z.w, bx2, by2, bz2, ma2, sc2, mb2, c.kz, k0, 65536u, nb);
             if (kDetect) {
-                if (__builtin_expect(na != 4u, 0)) flag_pair(da.flag, da.nfix, da.fix, da.bit, da.id);
-                if (__builtin_expect(nb != 4u, 0)) flag_pair(db.flag, db.nfix, db.fix, db.bit, db.id);
+                if (__builtin_expect(na != 4u, 0)) flag_pair<Lay<NB>::LW>(dt.base_s, dt.ctx, 0u);
+                if (__builtin_expect(nb != 4u, 0)) flag_pair<Lay<NB>::LW>(dt.base_s, dt.ctx, 1u);
             }
             ib += 4 * NS;
         }
@@ -392,8 +402,8 @@ __device__ __forceinline__ void bin_ions(uint32_t ions_s, int i0, int i1, const 
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dx) : "r"(a));
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dy) : "r"(a + 16u));
         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(dz) : "r"(a + 32u));
-        bin_one<kClamp, kDetect, BLK>(dx, dy, dz, n.ax, n.ay, n.az, c, k0, 1u, da.flag, da.nfix, da.fix, da.bit, da.id);
-        bin_one<kClamp, kDetect, BLK>(dx, dy, dz, n.bx, n.by, n.bz, c, k0, 65536u, db.flag, db.nfix, db.fix, db.bit, db.id);
+        if (bin_one<kClamp, kDetect, BLK>(dx, dy, dz, n.ax, n.ay, n.az, c, k0, 1u)) flag_pair<Lay<NB>::LW>(dt.base_s, dt.ctx, 0u);
+        if (bin_one<kClamp, kDetect, BLK>(dx, dy, dz, n.bx, n.by, n.bz, c, k0, 65536u)) flag_pair<Lay<NB>::LW>(dt.base_s, dt.ctx, 1u);
     }
 }
 
@@ -570,14 +580,15 @@ struct Seq {
 };
 struct PipeShared {
     uint64_t *full, *done, *doneq, *free_, *epi, *tfree;    // doneq[buf * 3 + q]: first three quarters of a buffer's MMAs complete
+    FixShared *fs;
     uint32_t *flag;
-    int *nfix;
+    int *n, *nfix;
     uint16_t *fix;
 };
 
 // The warp-specialised pipeline of one (material point, chunk).  kBig: the ROI's ions have spilled into the second
 // histogram buffer, so only buffer 0 is used and bin -> transform -> clear are serial per item.
-template <int KS, int NB, bool kBig, bool kHalf, bool kMulti>
+template <int KS, int NB, bool kBig, bool kHalf, bool kMulti, int kRole>
 __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &L, unsigned char *smem, uint32_t tmem, int n_ions,
                                              const Seq &sq, int64_t m, const float *ions, const float2 *phase,
                                              float2 *exch, float2 *cand, const PipeShared &ps, int cls)
@@ -600,7 +611,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
 #ifdef APX_TRACE
     int trace_n = sq.grp_base == 0 && sq.mode == 0 && cls == 0 ? 0 : (1 << 30);      // the CTA's first sequence only
 #endif
-    if (warp < kBinWarps) {
+    if (kRole == 0) {                                            // (the binning warps; every other warp runs the kRole = 1 copy)
         BinConst c;
         c.half_b = (float)(p.B / 2); c.magic_a = magic_for(p.B); c.magic_b = 12582912.0f + 4.0f;
         c.scl = __int_as_float((127 - p.nl) << 23);                       // 2^-nl
@@ -648,18 +659,23 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                 const int nq = (a1 - a0 + 3) >> 2;                                   // quads of this pass, split evenly
                 i0 = a0 + 4 * ((warp * nq) / kBinWarps); i1 = min(a1, a0 + 4 * (((warp + 1) * nq) / kBinWarps));
             }
-            const uint32_t k0 = k0base + (uint32_t)buf * (L.hist1 - L.hist0);
-            Detect dta, dtb;
+            uint32_t k0 = k0base + (uint32_t)buf * (L.hist1 - L.hist0);
+            // opaque to the compiler: it would otherwise re-derive k0 and kz from the thread id and the shared-memory base
+            // (S2R, shifts, multiplies: ~20 of 146 instructions) in every iteration of the binning loop
+            asm volatile("mov.b32 %0, %0;" : "+r"(k0));
+            asm volatile("mov.b32 %0, %0;" : "+r"(c.kz));
+            Detect dt;
+            dt.base_s = dt.ctx = 0u;
             if (detect) {
-                dta.flag = dtb.flag = &ps.flag[(sq.grp_base + gl) & (kFlagSlots - 1)];
-                dta.nfix = dtb.nfix = ps.nfix; dta.fix = dtb.fix = ps.fix;
-                dta.bit = 1u << l; dtb.bit = 1u << (LW + l);
-                dta.id = (uint32_t)(gl * G + l); dtb.id = dta.id + (uint32_t)LW;
-                bin_ions<false, true, NB>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
+                dt.base_s = smem_u32(ps.fs);
+                dt.ctx = (uint32_t)((sq.grp_base + gl) & (kFlagSlots - 1)) | ((uint32_t)l << 4) | ((uint32_t)(gl * G) << 16);
+                asm volatile("mov.b32 %0, %0;" : "+r"(dt.base_s));
+                asm volatile("mov.b32 %0, %0;" : "+r"(dt.ctx));
+                bin_ions<false, true, NB>(ions_s, i0, i1, n, c, k0, h, dt);
             } else if (p.clamp) {
-                bin_ions<true, false, NB>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
+                bin_ions<true, false, NB>(ions_s, i0, i1, n, c, k0, h, dt);
             } else {
-                bin_ions<false, false, NB>(ions_s, i0, i1, n, c, k0, h, dta, dtb);
+                bin_ions<false, false, NB>(ions_s, i0, i1, n, c, k0, h, dt);
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // histogram writes -> async proxy
             __syncwarp();
@@ -668,7 +684,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             APX_TRACE_EVENT(p, 9, sq.grp_base + gl);                                 // arrived
             if (++pass == npass) { pass = 0; ++gl; }
         }
-    } else if (warp == kMmaWarp) {
+    } else if (kRole != 0 && warp == kMmaWarp) {
         // ---- MMA warp: descriptors advance by adding to the 14-bit start-address field ---------------
         const uint32_t idesc = (1u << 4) | (1u << 15) | ((uint32_t)(p.N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
         const uint32_t tb = smem_u32(smem + L.table), hb = smem_u32(smem + L.hist0);
@@ -713,7 +729,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             __syncwarp();
             if (++pass == npass) { pass = 0; ++gl; }
         }
-    } else if (warp == kClrWarp) {
+    } else if (kRole != 0 && warp == kClrWarp) {
         // ---- clear warp: once the tensor core has read a buffer, clear it with bulk copies of zeros (TMA engine, no
         //      LSU work); free(buf) completes when all bytes have landed
         for (int it = 0; it < (kBig ? 0 : nitems); ++it) {           // (single-buffered: the binning warps clear)
@@ -741,7 +757,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             }
             __syncwarp();
         }
-    } else {
+    } else if (kRole != 0) {
         // ---- service warps: set s runs the epilogue of the groups with (group number & 1) == s ----------
         const int q = warp & 3, set = (warp - kSvcWarp0) >> 2;
         for (int gl = (set ^ sq.grp_base) & 1; gl < sq.ngrp; gl += 2) {
@@ -764,99 +780,56 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
 
 // one sequence, in the double-buffered pipeline or -- the ROI's ions have spilled into the second buffer, or B = 2048 -- the
 // single-buffered one
-template <int KS, int NB, bool kHalf, bool kMulti>
+template <int KS, int NB, bool kHalf, bool kMulti, int kRole>
 __device__ __forceinline__ void run_seq(const MmaParams &p, const MmaSmem &L, unsigned char *smem, uint32_t tmem, int n, const Seq &sq,
                                         int64_t m, const float *ions, const float2 *phase, float2 *exch, float2 *cand,
                                         const PipeShared &ps, int cls)
 {
-    if (NB == 8 || n > p.cap) run_pipeline<KS, NB, true, kHalf, kMulti>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
-    else run_pipeline<KS, NB, false, kHalf, kMulti>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
+    if (NB == 8 || n > p.cap) run_pipeline<KS, NB, true, kHalf, kMulti, kRole>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
+    else run_pipeline<KS, NB, false, kHalf, kMulti, kRole>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
 }
 
-// KS = K/16 k-steps per group, NB = bin parts (layout), kHalf = half-grid mode, kMulti = several signatures per plan
-template <int KS, int NB, bool kHalf, bool kMulti>
-__global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_constant__ MmaParams p)
+// (Re-)initialise the pipeline's barriers and counters; one thread.  again: a new class of signatures restarts the phase counts.
+__device__ __forceinline__ void init_barriers(const PipeShared &ps, bool again)
 {
-    extern __shared__ unsigned char smem_raw[];
-    unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned, still shared-space
-    const MmaSmem L = mma_smem_layout(p.B, p.N, p.W, p.cap);
-    // per histogram buffer: full (binned), done (transformed), free (cleared); per accumulator: tfree (read out)
-    __shared__ uint64_t s_full[2], s_done[2], s_doneq[6], s_free[2], s_epi[4], s_tfree[4];      // per histogram buffer / per accumulator
-    __shared__ uint32_t s_tmem;
-    __shared__ int s_n, s_nfix;
-    __shared__ uint32_t s_flag[kFlagSlots];
-    __shared__ uint16_t s_fix[kFixCap];
+    auto reinit = [&](uint64_t *b, uint32_t cnt) {
+        if (again) asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(b)) : "memory");
+        mbar_init(b, cnt);
+    };
+    for (int i = 0; i < 2; ++i) { reinit(&ps.full[i], kBinWarps); reinit(&ps.done[i], 1); reinit(&ps.free_[i], 1); }
+    for (int i = 0; i < 6; ++i) reinit(&ps.doneq[i], 1);
+    for (int i = 0; i < 4; ++i) { reinit(&ps.epi[i], 1); reinit(&ps.tfree[i], 4); }
+    asm volatile("fence.mbarrier_init.release.cluster;");
+    *ps.n = 0; *ps.nfix = 0;
+    for (int i = 0; i < kFlagSlots; ++i) ps.flag[i] = 0u;
+}
 
+// Work of one CTA = (material point m, chunk of direction groups [g_begin, g_end)) after the setup: one pass per class of
+// signatures (specs with the same type mask): gather, then the group pipeline.  Compiled twice: kRole 0 is the copy the
+// 16 binning warps run (they also gather), kRole 1 the copy of the MMA, clear and service warps.  Both copies execute the
+// same sequence of CTA-wide barriers.  The split keeps the other roles' code (and their live registers) out of the binning
+// warps' copy, so that the constants of the binning loop stay in registers.
+struct CtaWork {
+    int chunk, g_begin, g_end;
+    int64_t m;
+    float cx, cy, cz;
+};
+template <int KS, int NB, bool kHalf, bool kMulti, int kRole>
+__device__ __forceinline__ void cta_body(const MmaParams &p, const MmaSmem &L, unsigned char *smem, const PipeShared &ps,
+                                         const uint32_t *s_tmem, const CtaWork &w, uint32_t &tmem)
+{
     const int tid = threadIdx.x, warp = tid >> 5;
-    // CTAs are ordered chunk-major; with up to 6 chunks per material point the chunks shrink geometrically (weights
-    // 2^(nchunks-1-c)), so the last waves of the grid consist of the smallest work items
-    const int chunk = blockIdx.x / p.M;
-    const int64_t m = blockIdx.x % p.M;
-    int g_begin, g_end;
-    if (p.nchunks <= 6) {
-        const int wtot = (1 << p.nchunks) - 1, wlo = wtot - ((1 << (p.nchunks - chunk)) - 1);
-        g_begin = (int)((int64_t)wlo * p.ngroups / wtot);
-        g_end = (int)((int64_t)(wlo + (1 << (p.nchunks - 1 - chunk))) * p.ngroups / wtot);
-    } else {                                                   // few material points: many equal chunks
-        g_begin = (int)((int64_t)chunk * p.ngroups / p.nchunks);
-        g_end = (int)((int64_t)(chunk + 1) * p.ngroups / p.nchunks);
-    }
-    const GridParams g = *p.grid;
-    const float cx = p.centres[3 * m], cy = p.centres[3 * m + 1], cz = p.centres[3 * m + 2];
-    const RoiCells rc = roi_cells(g, cx, cy, cz, p.R);
+    const int chunk = w.chunk, g_begin = w.g_begin, g_end = w.g_end;
+    const int64_t m = w.m;
     float *ions = reinterpret_cast<float *>(smem + L.ions);
     float2 *exch = reinterpret_cast<float2 *>(smem + L.exch);
     float2 *cand = reinterpret_cast<float2 *>(smem + L.cand);
     float2 *phase = reinterpret_cast<float2 *>(smem + L.phase);
-    constexpr int K = KS * 16;
-
-    // ---- setup: barriers, TMEM, twiddle table ----------------------------------------------------------
-    auto init_barriers = [&](bool again) {
-        for (int i = 0; i < 2; ++i) {
-            if (again) {                                   // a new class of signatures restarts the pipeline's phase counts
-                uint64_t *bars[3] = {&s_full[i], &s_done[i], &s_free[i]};
-                for (uint64_t *b : bars) asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(b)) : "memory");
-            }
-            mbar_init(&s_full[i], kBinWarps);
-            mbar_init(&s_done[i], 1);
-            mbar_init(&s_free[i], 1);
-        }
-        for (int i = 0; i < 6; ++i) {
-            if (again) asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&s_doneq[i])) : "memory");
-            mbar_init(&s_doneq[i], 1);
-        }
-        for (int i = 0; i < 4; ++i) {
-            if (again) {
-                asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&s_epi[i])) : "memory");
-                asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&s_tfree[i])) : "memory");
-            }
-            mbar_init(&s_epi[i], 1);
-            mbar_init(&s_tfree[i], 4);
-        }
-        asm volatile("fence.mbarrier_init.release.cluster;");
-        s_n = 0; s_nfix = 0;
-        for (int i = 0; i < kFlagSlots; ++i) s_flag[i] = 0u;
-    };
-    if (tid == 0) init_barriers(false);
-    if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "r"(p.tmem_cols));
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
-    }
-    {
-        uint4 *t = reinterpret_cast<uint4 *>(smem + L.table);
-        for (int i = tid; i < K * p.N / 8; i += kMmaThreads) t[i] = p.table[i];
-        for (int i = tid; i < NB * p.W; i += kMmaThreads) phase[i] = p.phase[i];
-    }
-    PipeShared ps;
-    ps.full = s_full; ps.done = s_done; ps.doneq = s_doneq; ps.free_ = s_free; ps.epi = s_epi; ps.tfree = s_tfree;
-    ps.flag = s_flag; ps.nfix = &s_nfix; ps.fix = s_fix;
-    uint32_t tmem = 0;
-    // ---- one pass per class of signatures (specs with the same type mask): gather, then the group pipeline ---------
     const int n_classes = kMulti ? p.ss.n_classes : 1;
     for (int cls = 0; cls < n_classes; ++cls) {
         if (cls > 0) {
             __syncthreads();                               // the previous class has drained (epilogues done, clears landed)
-            if (tid == 0) init_barriers(true);
+            if (tid == 0) init_barriers(ps, true);
         }
         {
             uint4 *h0 = reinterpret_cast<uint4 *>(smem + L.hist0), *h1 = reinterpret_cast<uint4 *>(smem + L.hist1);
@@ -869,10 +842,16 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
         asm volatile("tcgen05.fence::before_thread_sync;");
         __syncthreads();
         asm volatile("tcgen05.fence::after_thread_sync;");
-        tmem = s_tmem;
-        if (g.n_accepted) gather_roi3<kMulti>(p, g, rc, cx, cy, cz, ions, &s_n, cls);
+        tmem = *s_tmem;
+        if (kRole == 0) {                                  // (the binning warps gather)
+            const GridParams g = *p.grid;
+            if (g.n_accepted) {
+                const RoiCells rc = roi_cells(g, w.cx, w.cy, w.cz, p.R);
+                gather_roi3<kMulti>(p, g, rc, w.cx, w.cy, w.cz, ions, ps.n, cls, kBinWarps);
+            }
+        }
         __syncthreads();
-        const int n = s_n;
+        const int n = *ps.n;
         if (chunk == 0 && tid == 0 && p.counts) {
             if (!kMulti) p.counts[m] = (uint32_t)n;
             else
@@ -891,16 +870,16 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
             for (int sg = g_begin; sg < g_end; sg += sub) {
                 Seq sq;
                 sq.mode = 0; sq.g0 = sg; sq.ngrp = min(sub, g_end - sg); sq.grp_base = grp_total; sq.nfix = 0;
-                run_seq<KS, NB, kHalf, kMulti>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
+                run_seq<KS, NB, kHalf, kMulti, kRole>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
                 grp_total += sq.ngrp;
                 if (kHalf) {
                     __syncthreads();                           // every epilogue of the sub-range is done, the list is complete
-                    const int nf = s_nfix;
+                    const int nf = *ps.nfix;
                     __syncthreads();
-                    if (tid == 0) s_nfix = 0;
+                    if (tid == 0) *ps.nfix = 0;
                     if (nf > kFixCap) overflow = true;         // pathological input: the FFT kernel redoes this material point
                     sq.mode = 1; sq.nfix = min(nf, kFixCap); sq.ngrp = (sq.nfix + Lay<NB>::G - 1) / Lay<NB>::G; sq.grp_base = grp_total;
-                    if (sq.ngrp) run_seq<KS, NB, kHalf, kMulti>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
+                    if (sq.ngrp) run_seq<KS, NB, kHalf, kMulti, kRole>(p, L, smem, tmem, n, sq, m, ions, phase, exch, cand, ps, cls);
                     grp_total += sq.ngrp;
                     __syncthreads();                           // the list is consumed before the next sub-range appends
                 }
@@ -908,18 +887,68 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
             if (overflow && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
             // the bulk copies that clear the buffers after their last use must land before the CTA gives up its shared memory
             // (or re-initialises the barriers for the next class)
-            if (warp == kClrWarp && grp_total > 0) {
+            if (kRole != 0 && warp == kClrWarp && grp_total > 0) {
                 const int npass = n > 2048 ? (n + 2047) / 2048 : 1, items = grp_total * npass;
                 if (NB == 8 || n > p.cap) {
                     // single-buffered: cleared with plain stores by the binning warps, nothing in flight
                 } else {
                     const int u0 = (items + 1) >> 1, u1 = items >> 1;
-                    if (u0) mbar_wait(&s_free[0], (uint32_t)((u0 - 1) & 1));
-                    if (u1) mbar_wait(&s_free[1], (uint32_t)((u1 - 1) & 1));
+                    if (u0) mbar_wait(&ps.free_[0], (uint32_t)((u0 - 1) & 1));
+                    if (u1) mbar_wait(&ps.free_[1], (uint32_t)((u1 - 1) & 1));
                 }
             }
         }
     }
+}
+
+// KS = K/16 k-steps per group, NB = bin parts (layout), kHalf = half-grid mode, kMulti = several signatures per plan
+template <int KS, int NB, bool kHalf, bool kMulti>
+__global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_constant__ MmaParams p)
+{
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned, still shared-space
+    const MmaSmem L = mma_smem_layout(p.B, p.N, p.W, p.cap);
+    // per histogram buffer: full (binned), done (transformed), free (cleared); per accumulator: tfree (read out)
+    __shared__ uint64_t s_full[2], s_done[2], s_doneq[6], s_free[2], s_epi[4], s_tfree[4];      // per histogram buffer / per accumulator
+    __shared__ uint32_t s_tmem;
+    __shared__ int s_n;
+    __shared__ FixShared s_fs;
+
+    const int tid = threadIdx.x, warp = tid >> 5;
+    // CTAs are ordered chunk-major; with up to 6 chunks per material point the chunks shrink geometrically (weights
+    // 2^(nchunks-1-c)), so the last waves of the grid consist of the smallest work items
+    CtaWork w;
+    w.chunk = blockIdx.x / p.M;
+    w.m = blockIdx.x % p.M;
+    if (p.nchunks <= 6) {
+        const int wtot = (1 << p.nchunks) - 1, wlo = wtot - ((1 << (p.nchunks - w.chunk)) - 1);
+        w.g_begin = (int)((int64_t)wlo * p.ngroups / wtot);
+        w.g_end = (int)((int64_t)(wlo + (1 << (p.nchunks - 1 - w.chunk))) * p.ngroups / wtot);
+    } else {                                                   // few material points: many equal chunks
+        w.g_begin = (int)((int64_t)w.chunk * p.ngroups / p.nchunks);
+        w.g_end = (int)((int64_t)(w.chunk + 1) * p.ngroups / p.nchunks);
+    }
+    w.cx = p.centres[3 * w.m]; w.cy = p.centres[3 * w.m + 1]; w.cz = p.centres[3 * w.m + 2];
+    constexpr int K = KS * 16;
+
+    // ---- setup: barriers, TMEM, twiddle table ----------------------------------------------------------
+    PipeShared ps;
+    ps.full = s_full; ps.done = s_done; ps.doneq = s_doneq; ps.free_ = s_free; ps.epi = s_epi; ps.tfree = s_tfree;
+    ps.fs = &s_fs; ps.flag = s_fs.flag; ps.n = &s_n; ps.nfix = &s_fs.nfix; ps.fix = s_fs.fix;
+    if (tid == 0) init_barriers(ps, false);
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "r"(p.tmem_cols));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    {
+        uint4 *t = reinterpret_cast<uint4 *>(smem + L.table);
+        float2 *phase = reinterpret_cast<float2 *>(smem + L.phase);
+        for (int i = tid; i < K * p.N / 8; i += kMmaThreads) t[i] = p.table[i];
+        for (int i = tid; i < NB * p.W; i += kMmaThreads) phase[i] = p.phase[i];
+    }
+    uint32_t tmem = 0;
+    if (warp < kBinWarps) cta_body<KS, NB, kHalf, kMulti, 0>(p, L, smem, ps, &s_tmem, w, tmem);
+    else cta_body<KS, NB, kHalf, kMulti, 1>(p, L, smem, ps, &s_tmem, w, tmem);
     // ---- teardown ---------------------------------------------------------------------------------
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();

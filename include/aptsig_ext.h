@@ -94,6 +94,29 @@ int apx_fsp(apx_plan *plan, const float *centres, int64_t M, float k_max, int32_
  * 1 = the FP32-pipe kernel for everything.  Results agree within the tolerance derived in DESIGN.md section 2. */
 int apx_fsp_set_path(apx_plan *plan, int32_t path);
 
+/* apx_fsp for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the same operation (Eq. 2), the same kernels, arguments, layout and results as apx_fsp with the
+ * plan's current apx_fsp_set_path choice, but the scratch apx_fsp keeps in lazily (re)allocated plan buffers -- the k axis
+ * (float32[L]) and the device list of ROIs the tensor-core kernel hands to the FP32 kernel (uint32[1 + M]) -- lives in ONE
+ * file-scope `static __device__` array of APX_FSP_NOALLOC_SCRATCH_BYTES inside the library (held by every GPU that loads
+ * the library until the process exits).  The call performs no cudaMalloc / cudaFree / allocating library routine and no
+ * host-to-device copy: the k axis is computed on the device (same fp64 formula, rounded once) and the list count is
+ * cleared by a small kernel in `cuda_stream` ahead of the FSP kernels.
+ *   Limits: M <= APX_FSP_NOALLOC_MAX_M and L <= APX_FSP_NOALLOC_MAX_L, else APX_ERANGE and nothing is launched
+ *   (apx_fsp_noalloc_limits reports the numbers); all other argument rules and status codes are apx_fsp's.
+ *   Sharing: every call on a device uses the same array, which keeps the last call's contents.  Calls in one stream are
+ *   ordered and safe; calls that overlap on the GPU (different streams, or several plans on one device) RACE on it --
+ *   serialise them, or use apx_fsp.
+ *   The first call on a device resolves the array's device address (cudaGetSymbolAddress, once per device); make that
+ *   first call outside stream capture. */
+#define APX_FSP_NOALLOC_MAX_M 16384
+#define APX_FSP_NOALLOC_MAX_L 1024
+#define APX_FSP_NOALLOC_SCRATCH_BYTES 69888   /* 4096 (k axis) + 65792 (list: 1 + 16384 words, padded to 256 B) */
+int apx_fsp_noalloc(apx_plan *plan, const float *centres, int64_t M, float k_max, int32_t L, float *out, uint32_t *counts,
+                    void *cuda_stream);
+/* The limits above, for bindings: any pointer may be NULL.  Returns APX_OK. */
+int apx_fsp_noalloc_limits(int64_t *max_M, int32_t *max_L, int64_t *scratch_bytes);
+
 #ifdef __cplusplus
 }
 #endif

@@ -21,7 +21,7 @@ EXPORTS = ["apx_plan_create", "apx_plan_destroy", "apx_plan_constants", "apx_pla
            "apx_dirs_fibonacci", "apx_dirs_geodesic", "apx_dirs_antipodes", "apx_strerror", "apx_version"]
 PEAK_EXPORTS = ["apx_peak_name", "apx_peak_measure"]          # include/aptsig_peaks.h
 EXT_EXPORTS = ["apx_intensity_max", "apx_refine_select", "apx_refine_centres", "apx_indexer_create", "apx_indexer_destroy",
-               "apx_indexer_nodes", "apx_indexer_lut", "apx_last_cuda_error_indexer", "apx_index", "apx_so3_grid_cubic", "apx_fsp", "apx_fsp_set_path"]   # aptsig_ext.h
+               "apx_indexer_nodes", "apx_indexer_lut", "apx_last_cuda_error_indexer", "apx_index", "apx_so3_grid_cubic", "apx_fsp", "apx_fsp_set_path", "apx_fsp_noalloc", "apx_fsp_noalloc_limits"]   # aptsig_ext.h
 APX_INDEX_MAX_K = 8
 
 
@@ -98,6 +98,8 @@ def _lib():
         L.apx_so3_grid_cubic.argtypes = [f32, vp, C.POINTER(i64)]
         L.apx_fsp.argtypes = [vp, vp, i64, f32, i32, vp, vp, vp]
         L.apx_fsp_set_path.argtypes = [vp, i32]
+        L.apx_fsp_noalloc.argtypes = [vp, vp, i64, f32, i32, vp, vp, vp]
+        L.apx_fsp_noalloc_limits.argtypes = [C.POINTER(i64), C.POINTER(i32), C.POINTER(i64)]
         for name in EXT_EXPORTS:
             getattr(L, name).restype = C.c_int
         L.apx_peak_name.argtypes = [C.c_int]
@@ -354,6 +356,18 @@ class Plan:
                                    _arg(out, "out", np.float32, (M, L, L, L), dev),
                                    _arg(counts, "counts", np.uint32, (M,), dev, optional=True), self._stream(stream)), "apx_fsp")
 
+    def apx_fsp_noalloc(self, centres, k_max, L, out, counts=None, stream=None):
+        """apx_fsp without any allocation: scratch in the library's static device array (limits: apx_fsp_noalloc_limits)."""
+        M, dev, L = int(centres.shape[0]), self.device, int(L)
+        rc = _lib().apx_fsp_noalloc(self._h, _arg(centres, "centres", np.float32, (M, 3), dev), M, float(k_max), L,
+                                    _arg(out, "out", np.float32, (M, L, L, L), dev),
+                                    _arg(counts, "counts", np.uint32, (M,), dev, optional=True), self._stream(stream))
+        where = "apx_fsp_noalloc"
+        if rc == APX_ERANGE:
+            max_m, max_l, nbytes = apx_fsp_noalloc_limits()
+            where += f" (M = {M}, L = {L}; the static scratch of {nbytes} bytes serves M <= {max_m}, L <= {max_l}: use apx_fsp)"
+        self._check(rc, where)
+
     def apx_plan_destroy(self):
         if self._h:
             _lib().apx_plan_destroy(self._h)
@@ -364,6 +378,13 @@ class Plan:
             self.apx_plan_destroy()
         except Exception:
             pass
+
+
+def apx_fsp_noalloc_limits():
+    """(max M, max L, bytes of the static device scratch array) of apx_fsp_noalloc."""
+    m, l, b = C.c_int64(), C.c_int32(), C.c_int64()
+    _lib().apx_fsp_noalloc_limits(C.byref(m), C.byref(l), C.byref(b))
+    return m.value, l.value, b.value
 
 
 class Indexer:

@@ -151,6 +151,8 @@ cudaError_t mma_path_prepare(Plan *p);   // builds d_mma_table
 cudaError_t mma_reserve_deferred(Plan *p, int64_t need);   // deferred list of at least `need` words
 cudaError_t launch_fsp_mma(Plan *p, const float *centres, int64_t M, int L, float dk, float *out, uint32_t *counts, uint32_t *list,
                            cudaStream_t st);
+cudaError_t launch_fsp_mma_at(Plan *p, const float *kaxis, const float *centres, int64_t M, int L, float dk, float *out,
+                              uint32_t *counts, uint32_t *list, cudaStream_t st);   // k axis at a given device address
 cudaError_t mma_reserve_for(Plan *p, int64_t M);           // ... sized for any apx_query of up to M material points
 
 }  // namespace apx

@@ -10,6 +10,7 @@
 // sorted cloud, exact fp32 ball test) is the one of the signature kernels.  ROIs with more ions than the shared buffer
 // are handled by streaming the candidate ions of their cell rows through the same loop with non-members masked to zero.
 #include <cmath>
+#include <mutex>
 #include "common.cuh"
 #include "../../include/aptsig_ext.h"
 
@@ -253,6 +254,107 @@ extern "C" int apx_fsp(apx_plan *p, const float *centres, int64_t M, float k_max
         e = launch_fsp_mma(p, centres, M, L, L == 1 ? 0.0f : (float)(2.0 * (double)k_max / (double)(L - 1)), out, counts, p->d_fsp_list, st);
         if (e != cudaSuccess) return cu(e);
         q.list = p->d_fsp_list;
+        k_fsp<<<(unsigned)(p->sm_count * 2), kFspThreads, smem, st>>>(q);
+    }
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cu(e);
+    return done(APX_OK);
+}
+
+// ---- apx_fsp_noalloc: the same kernels with their scratch in a static device array (include/aptsig_ext.h) ------------------
+//
+// Layout of the array: [0, 4096) the k axis float32[<= 1024]; [4096, 4096 + 65792) the list uint32[1 + 16384] of the material
+// points k_fsp_mma leaves to k_fsp (word 0 = count).  Every GPU that loads the library holds the array until exit.  In HOST
+// code the name g_fsp_scratch is only a stand-in for the symbol, never a device address: the address each device uses is taken
+// once per device with cudaGetSymbolAddress (below, with that device current) and handed to the kernels as an argument.
+namespace apx {
+constexpr int kNoAllocMaxM = APX_FSP_NOALLOC_MAX_M, kNoAllocMaxL = APX_FSP_NOALLOC_MAX_L;
+constexpr size_t kNoAllocKaxisBytes = sizeof(float) * kNoAllocMaxL;                                     // 4096
+constexpr size_t kNoAllocListBytes = ((sizeof(uint32_t) * (size_t)(1 + kNoAllocMaxM) + 255) / 256) * 256;      // 65792
+static_assert(kNoAllocKaxisBytes % 256 == 0, "the list must start 256-byte aligned");
+static_assert(kNoAllocKaxisBytes + kNoAllocListBytes == APX_FSP_NOALLOC_SCRATCH_BYTES, "header and layout disagree");
+static __device__ __align__(256) unsigned char g_fsp_scratch[APX_FSP_NOALLOC_SCRATCH_BYTES];
+
+// k axis (reading #25) exactly as apx_fsp computes it on the host -- fp64, every operation rounded on its own (no fused
+// multiply-add), one final rounding to fp32 -- and the list count back to zero (the array keeps the previous call's contents).
+__global__ void __launch_bounds__(1024) k_fsp_noalloc_prepare(unsigned char *scratch, float k_max, int L)
+{
+    float *kaxis = reinterpret_cast<float *>(scratch);
+    uint32_t *list = reinterpret_cast<uint32_t *>(scratch + kNoAllocKaxisBytes);
+    const int i = threadIdx.x;
+    if (i < L) {
+        const double step = L == 1 ? 0.0 : __ddiv_rn(__dmul_rn(2.0, (double)k_max), (double)(L - 1));
+        kaxis[i] = L == 1 ? 0.0f : (float)__dadd_rn(-(double)k_max, __dmul_rn((double)i, step));
+    }
+    if (i == 0) list[0] = 0u;
+}
+}  // namespace apx
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_scratch_mu;
+unsigned char *g_scratch_addr[kMaxDevices];      // device address of g_fsp_scratch on device d, nullptr = not resolved yet
+
+// Device address of the scratch array on `device`, which must be the CURRENT device.  Resolved once per device.
+cudaError_t scratch_address(int device, unsigned char **out)
+{
+    if (device < 0 || device >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_scratch_mu);
+    if (!g_scratch_addr[device]) {
+        void *ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&ptr, apx::g_fsp_scratch);
+        if (e != cudaSuccess) return e;
+        if (!ptr) return cudaErrorInvalidSymbol;
+        g_scratch_addr[device] = static_cast<unsigned char *>(ptr);
+    }
+    *out = g_scratch_addr[device];
+    return cudaSuccess;
+}
+}  // namespace
+
+extern "C" int apx_fsp_noalloc_limits(int64_t *max_M, int32_t *max_L, int64_t *scratch_bytes)
+{
+    if (max_M) *max_M = kNoAllocMaxM;
+    if (max_L) *max_L = kNoAllocMaxL;
+    if (scratch_bytes) *scratch_bytes = APX_FSP_NOALLOC_SCRATCH_BYTES;
+    return APX_OK;
+}
+
+extern "C" int apx_fsp_noalloc(apx_plan *p, const float *centres, int64_t M, float k_max, int32_t L, float *out, uint32_t *counts,
+                               void *stream)
+{
+    if (!p || M < 0 || L < 1 || !(k_max >= 0.0f) || !std::isfinite(k_max) || (M > 0 && (!centres || !out))) return APX_EINVAL;
+    if (M > kNoAllocMaxM || L > kNoAllocMaxL) return APX_ERANGE;          // beyond the static scratch: nothing is launched
+    if (!p->ingested) return APX_ESTATE;
+    if (M == 0) return APX_OK;
+    int prev = -1;
+    cudaGetDevice(&prev);
+    if (prev != p->device) cudaSetDevice(p->device);
+    auto done = [&](int code) { if (prev >= 0 && prev != p->device) cudaSetDevice(prev); return code; };
+    auto cu = [&](cudaError_t e) { p->last_cuda = (int)e; return done(APX_ECUDA); };
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned char *scratch = nullptr;
+    cudaError_t e = scratch_address(p->device, &scratch);                  // the plan's device is current here
+    if (e != cudaSuccess) return cu(e);
+    const float *kaxis = reinterpret_cast<const float *>(scratch);
+    uint32_t *list = reinterpret_cast<uint32_t *>(scratch + kNoAllocKaxisBytes);
+    const int tiles = (L + kFspTile - 1) / kFspTile;
+    const size_t smem = sizeof(float) * (4 * kFspStep * kFspTile + 4 * kFspStep + 3 * kFspCap);
+    e = cudaFuncSetAttribute(k_fsp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return cu(e);
+    const int64_t blocks = p->fsp_path == 1 ? M * L * tiles * tiles : M * ((L + 1) / 2) * tiles * tiles;
+    if (blocks > 0x7FFFFFFFLL) return done(APX_ERANGE);
+    k_fsp_noalloc_prepare<<<1, 1024, 0, st>>>(scratch, k_max, L);
+    FspParams q;
+    q.sorted = p->d_sorted; q.cell_start = p->d_cell_start; q.grid = p->d_grid; q.centres = centres; q.kaxis = kaxis;
+    q.out = out; q.counts = counts; q.list = nullptr; q.L = L; q.tiles = tiles; q.R = p->R; q.R2 = p->R2;
+    if (p->fsp_path == 1) {
+        k_fsp<<<(unsigned)blocks, kFspThreads, smem, st>>>(q);
+    } else {
+        e = launch_fsp_mma_at(p, kaxis, centres, M, L, L == 1 ? 0.0f : (float)(2.0 * (double)k_max / (double)(L - 1)), out, counts,
+                              list, st);
+        if (e != cudaSuccess) return cu(e);
+        q.list = list;
         k_fsp<<<(unsigned)(p->sm_count * 2), kFspThreads, smem, st>>>(q);
     }
     e = cudaGetLastError();

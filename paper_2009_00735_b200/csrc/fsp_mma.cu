@@ -296,4 +296,21 @@ cudaError_t launch_fsp_mma(Plan *p, const float *centres, int64_t M, int L, floa
     return cudaGetLastError();
 }
 
+// The same launch with the k axis at a caller-given device address instead of the plan's d_kaxis: used by apx_fsp_noalloc
+// (fsp.cu), whose k axis and deferred list live in the library's static scratch array.
+cudaError_t launch_fsp_mma_at(Plan *p, const float *kaxis, const float *centres, int64_t M, int L, float dk, float *out,
+                              uint32_t *counts, uint32_t *list, cudaStream_t st)
+{
+    FspMmaParams q;
+    q.sorted = p->d_sorted; q.cell_start = p->d_cell_start; q.grid = p->d_grid; q.centres = centres; q.kaxis = kaxis;
+    q.out = out; q.counts = counts; q.list = list; q.L = L; q.tiles = (L + 63) / 64; q.cap = 4096; q.R = p->R; q.R2 = p->R2; q.dk = dk;
+    const int64_t blocks = M * ((L + 1) / 2) * q.tiles * q.tiles;
+    if (blocks > 0x7FFFFFFFLL) return cudaErrorInvalidConfiguration;
+    const size_t smem = 2 * (size_t)kFmStageBytes + (size_t)q.cap * 12 + 1024;
+    cudaError_t e = cudaFuncSetAttribute(k_fsp_mma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_fsp_mma<<<(unsigned)blocks, kFmThreads, smem, st>>>(q);
+    return cudaGetLastError();
+}
+
 }  // namespace apx

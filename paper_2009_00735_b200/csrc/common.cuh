@@ -61,7 +61,7 @@ struct Plan {
     int *d_dir_perm_mirror;        // [Dp] half-grid mode: index of the direction opposite to the slot's
     int Dp;                        // D rounded up to a multiple of 32
     int mma_paired;                // 1 = half-grid mode: the grid is antipodally symmetric, one direction per pair is binned
-    int tune_unit_split, tune_nacc;   // k_signature_mma scheduling knobs (see mma_path_prepare)
+    int tune_unit_split, tune_nacc, tune_dc;   // k_signature_mma scheduling knobs (see mma_path_prepare)
     int need_clamp;                // 1 = the bin clamp of Eq. 1 can trigger and must stay in the kernels' inner loops
     uint32_t *d_deferred;          // [0] count, [1..] material points the MMA kernel left to the FFT kernel
     int64_t cap_deferred;

@@ -159,6 +159,13 @@ __device__ __forceinline__ void tmem_ld16(uint32_t addr, uint32_t (&v)[16])
                  : "r"(addr));
 }
 
+__device__ __forceinline__ uint32_t tmem_ld1(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+
 struct MmaParams {
     const float4 *sorted;
     const uint32_t *cell_start;
@@ -185,6 +192,10 @@ struct MmaParams {
     SpecSet ss;                // signatures of the plan: classes (type masks), per-spec sub-windows of [k_lo, k_lo + W)
     int nacc, nacc_log2;       // TMEM accumulators (2 or 4): group gq uses accumulator gq & (nacc - 1), so the MMAs of a group
                                // wait for the epilogue of group gq - nacc only
+    int dc_col;                // >= 0: spare accumulator column 4 W whose twiddle is 1 for every bin: it receives the sum of the
+                               // counters AS THE TENSOR CORE READ THEM, = N_c exactly unless a counter exceeded 2048 (see pass_ions)
+    int pass_ions;             // ions binned per pass: 2048 (no counter can leave the exactly aliased range), or, with dc_col,
+                               // the whole ROI in one pass, checked after the fact by the DC column
     int unit_split;            // 1 = ions are dealt to the binning warps in whole blocks of 4 * NS (no ragged tails)
     uint32_t tmem_cols;
     float R, R2;
@@ -418,6 +429,7 @@ struct EpiOut {
     int mode, gi, g0, f, nfix;           // g0 = first group of the sub-range, f = fix-up group, nfix = listed pairs
     uint32_t *flag;                      // mode 0, half-grid: flag word of this group (read, then reset)
     const uint16_t *fix;
+    int *ovf;                            // set to 1 when a slot's DC sum is not N_c: a counter left the exact fp16 range
 };
 template <bool kHalf, int NB, bool kMulti>
 __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc, const EpiOut &eo, int64_t m, const float2 *phase,
@@ -436,6 +448,7 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
 #pragma unroll
     for (int sp = 0; sp < NSP; ++sp) { best[sp] = -1.0f; kbest[sp] = !kMulti ? p.k_lo : (sp < n_specs ? p.ss.k_lo[sp] : 0); }
     const bool one_spec = !kMulti || n_specs == 1;
+    float dcsum = 0.f;
 #pragma unroll 1
     for (int r0 = 0; r0 < p.W; r0 += kEpiRound) {
         uint32_t v[16];
@@ -458,7 +471,17 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
                 else exch[(j * 4 + q) * 32 + lane] = P;
             }
         }
+        if (p.dc_col >= 0 && r0 == 0) {
+            // DC check: the sum of this part's counters as the tensor core read them travels in the exchange slot (j = q) that
+            // the reduce-scatter never uses; warp q = 0 adds the parts behind the barrier
+            float dcv = __uint_as_float(tmem_ld1(acc0 + (uint32_t)p.dc_col));
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (NB == 8) dcv += __shfl_xor_sync(0xffffffffu, dcv, 16);
+            exch[(q * 4 + q) * 32 + lane].x = dcv;
+        }
         if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
+        if (p.dc_col >= 0 && r0 == 0 && q == 0)
+            dcsum = (exch[0 * 32 + lane].x + exch[5 * 32 + lane].x) + (exch[10 * 32 + lane].x + exch[15 * 32 + lane].x);
         const int w = r0 + q;
         if (w < p.W) {
             float xr = keep.x, xi = keep.y;
@@ -482,6 +505,7 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
         if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
     }
     if (kHalf && mode == 0 && q == 0 && lane == 0) *eo.flag = 0u;     // every thread of the set has read it (barriers above)
+    bool dc_pending = p.dc_col >= 0;
 #pragma unroll 1
     for (int sp = 0; sp < n_specs; ++sp) {
         if (kMulti && p.ss.cls_of[sp] != eo.cls) continue;
@@ -494,6 +518,14 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
         if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
         if (q == 0 && lane < Lay<NB>::G) {                   // (NB = 8: lanes 16..31 carry copies of lanes 0..15)
             constexpr int G = Lay<NB>::G;
+            if (dc_pending) {
+                // all parts of the slot: 2^-24 * (sum of the counters as fp16 numbers), exact in fp32.  It equals N_c unless
+                // some counter went beyond 2048, where the u16 bit pattern stops being the fp16 number of the same value
+                const float dc = dcsum;
+                const int slot0 = (lane & 1) * (G / 2) + ((lane >> 3) << 2) + ((lane & 7) >> 1);
+                const bool live = mode == 0 ? p.perm[eo.gi * G + slot0] >= 0 : eo.f * G + slot0 < eo.nfix;
+                if (live && dc * 16777216.0f != (float)eo.n) *eo.ovf = 1;
+            }
             float bb = -1.0f;
             int kb = kMulti ? p.ss.k_lo[sp] : p.k_lo;
 #pragma unroll
@@ -523,6 +555,7 @@ __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc,
                 }
             }
         }
+        dc_pending = false;
         if (!one_spec) {                                     // cand is reused by the next spec of the class
             if (set == 0) asm volatile("bar.sync 3, 128;" ::: "memory"); else asm volatile("bar.sync 4, 128;" ::: "memory");
         }
@@ -584,6 +617,7 @@ struct PipeShared {
     uint32_t *flag;
     int *n, *nfix;
     uint16_t *fix;
+    int *ovf;                                               // 1: this CTA's material point goes to the deferred list
 };
 
 // The warp-specialised pipeline of one (material point, chunk).  kBig: the ROI's ions have spilled into the second
@@ -604,7 +638,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
     // A ROI with more than `cap` ions has spilled into the second histogram buffer: it runs with buffer 0 only
     // (bin -> transform -> clear serial per item); `use` counts the uses of a buffer.
     const int n = n_ions;
-    const int npass = n > 2048 ? (n + 2047) / 2048 : 1;          // fp16 counters are exact up to 2048
+    const int npass = n > p.pass_ions ? (n + p.pass_ions - 1) / p.pass_ions : 1;     // (fp16 counters are exact up to 2048)
     const int nitems = sq.ngrp * npass;
     const int mode = kHalf ? sq.mode : 0;
     const int it_base = sq.grp_base * npass;
@@ -649,7 +683,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
                 mbar_wait_lean(&ps.free_[buf], (uint32_t)((use - 1) & 1));             // cleared after its previous use
             }
             APX_TRACE_EVENT(p, 1, sq.grp_base + gl);                                 // bin start (buffer free)
-            const int a0 = pass * 2048, a1 = min(n_ions, a0 + 2048);
+            const int a0 = pass * p.pass_ions, a1 = min(n_ions, a0 + p.pass_ions);
             int i0, i1;
             if (p.unit_split) {                                                      // whole blocks of 4 * NS ions per warp: no ragged tails
                 constexpr int U = 4 * Lay<NB>::NS;
@@ -768,7 +802,7 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             EpiOut eo;
             eo.cls = cls; eo.n = n;
             eo.mode = mode; eo.gi = sq.g0 + gl; eo.g0 = sq.g0; eo.f = gl; eo.nfix = sq.nfix;
-            eo.flag = kHalf ? &ps.flag[gq & (kFlagSlots - 1)] : nullptr; eo.fix = ps.fix;
+            eo.flag = kHalf ? &ps.flag[gq & (kFlagSlots - 1)] : nullptr; eo.fix = ps.fix; eo.ovf = ps.ovf;
             epilogue_group<kHalf, NB, kMulti>(p, tmem + (uint32_t)((gq & (p.nacc - 1)) * p.N), eo, m, phase, exch, cand, set, q, lane);
             asm volatile("tcgen05.fence::before_thread_sync;");
             __syncwarp();
@@ -800,8 +834,18 @@ __device__ __forceinline__ void init_barriers(const PipeShared &ps, bool again)
     for (int i = 0; i < 6; ++i) reinit(&ps.doneq[i], 1);
     for (int i = 0; i < 4; ++i) { reinit(&ps.epi[i], 1); reinit(&ps.tfree[i], 4); }
     asm volatile("fence.mbarrier_init.release.cluster;");
-    *ps.n = 0; *ps.nfix = 0;
+    *ps.n = 0; *ps.nfix = 0; *ps.ovf = 0;
     for (int i = 0; i < kFlagSlots; ++i) ps.flag[i] = 0u;
+}
+
+// A fix-list overflow or a failed DC check (a counter beyond 2048 in a single-pass ROI) sends the material point to the FFT
+// kernel: at most one entry per CTA and class.  Thread 0, behind a CTA barrier that follows the last epilogue of the class.
+__device__ __forceinline__ void flush_overflow(const MmaParams &p, const PipeShared &ps, int64_t m)
+{
+    if (*ps.ovf) {
+        p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
+        *ps.ovf = 0;
+    }
 }
 
 // Work of one CTA = (material point m, chunk of direction groups [g_begin, g_end)) after the setup: one pass per class of
@@ -829,7 +873,10 @@ __device__ __forceinline__ void cta_body(const MmaParams &p, const MmaSmem &L, u
     for (int cls = 0; cls < n_classes; ++cls) {
         if (cls > 0) {
             __syncthreads();                               // the previous class has drained (epilogues done, clears landed)
-            if (tid == 0) init_barriers(ps, true);
+            if (tid == 0) {
+                flush_overflow(p, ps, m);
+                init_barriers(ps, true);
+            }
         }
         {
             uint4 *h0 = reinterpret_cast<uint4 *>(smem + L.hist0), *h1 = reinterpret_cast<uint4 *>(smem + L.hist1);
@@ -884,11 +931,11 @@ __device__ __forceinline__ void cta_body(const MmaParams &p, const MmaSmem &L, u
                     __syncthreads();                           // the list is consumed before the next sub-range appends
                 }
             }
-            if (overflow && tid == 0) p.deferred[1 + atomicAdd(&p.deferred[0], 1u)] = (uint32_t)m;
+            if (overflow && tid == 0) *ps.ovf = 1;
             // the bulk copies that clear the buffers after their last use must land before the CTA gives up its shared memory
             // (or re-initialises the barriers for the next class)
             if (kRole != 0 && warp == kClrWarp && grp_total > 0) {
-                const int npass = n > 2048 ? (n + 2047) / 2048 : 1, items = grp_total * npass;
+                const int npass = n > p.pass_ions ? (n + p.pass_ions - 1) / p.pass_ions : 1, items = grp_total * npass;
                 if (NB == 8 || n > p.cap) {
                     // single-buffered: cleared with plain stores by the binning warps, nothing in flight
                 } else {
@@ -911,7 +958,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
     // per histogram buffer: full (binned), done (transformed), free (cleared); per accumulator: tfree (read out)
     __shared__ uint64_t s_full[2], s_done[2], s_doneq[6], s_free[2], s_epi[4], s_tfree[4];      // per histogram buffer / per accumulator
     __shared__ uint32_t s_tmem;
-    __shared__ int s_n;
+    __shared__ int s_n, s_ovf;
     __shared__ FixShared s_fs;
 
     const int tid = threadIdx.x, warp = tid >> 5;
@@ -934,7 +981,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
     // ---- setup: barriers, TMEM, twiddle table ----------------------------------------------------------
     PipeShared ps;
     ps.full = s_full; ps.done = s_done; ps.doneq = s_doneq; ps.free_ = s_free; ps.epi = s_epi; ps.tfree = s_tfree;
-    ps.fs = &s_fs; ps.flag = s_fs.flag; ps.n = &s_n; ps.nfix = &s_fs.nfix; ps.fix = s_fs.fix;
+    ps.fs = &s_fs; ps.flag = s_fs.flag; ps.n = &s_n; ps.nfix = &s_fs.nfix; ps.fix = s_fs.fix; ps.ovf = &s_ovf;
     if (tid == 0) init_barriers(ps, false);
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "r"(p.tmem_cols));
@@ -952,6 +999,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_signature_mma(const __grid_c
     // ---- teardown ---------------------------------------------------------------------------------
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
+    if (tid == 0) flush_overflow(p, ps, w.m);
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(p.tmem_cols));
 }
 
@@ -1060,6 +1108,7 @@ cudaError_t mma_path_prepare(Plan *p)
         for (int n = 0; n < N; ++n) {
             const int w = n / 4, c = n % 4;
             __half val = __float2half(0.0f);
+            if (n == 4 * W) val = __float2half(1.0f);    // spare column (if N > 4 W): "k = 0" twiddle, the DC check of MmaParams::dc_col
             if (w < W) {
                 const int64_t binpart = (int64_t)(r & 7) * (B / 8) + nb * (r >> 3);
                 const double th = 2.0 * M_PI * (double)((binpart * (p->k_lo + w)) % B) / (double)B;
@@ -1148,6 +1197,8 @@ cudaError_t mma_path_prepare(Plan *p)
     // scheduling knobs: defaults chosen from measurements, overridable from the environment for A/B runs
     p->tune_unit_split = 1; p->tune_nacc = 4;
     if (const char *ev = std::getenv("APX_TUNE_UNITS")) p->tune_unit_split = std::atoi(ev);
+    p->tune_dc = 1;
+    if (const char *ev = std::getenv("APX_TUNE_DC")) p->tune_dc = std::atoi(ev);
     if (const char *ev = std::getenv("APX_TUNE_NACC")) p->tune_nacc = std::atoi(ev);
     const int Dp = (int)perm.size();
     p->mma_paired = sym ? 1 : 0;
@@ -1235,6 +1286,9 @@ cudaError_t launch_signature_mma(Plan *p, const float *centres, int64_t M, float
     q.clamp = p->need_clamp;
     q.half = p->mma_paired;
     q.unit_split = p->tune_unit_split;
+    // a spare accumulator column (N > 4 W) carries the DC check, which lets a ROI of more than 2048 ions be binned in ONE pass
+    q.dc_col = (q.N > 4 * q.W && p->tune_dc) ? 4 * q.W : -1;
+    q.pass_ions = q.dc_col >= 0 ? (1 << 20) : 2048;
     q.nacc = (p->tune_nacc == 4 && 4 * q.N <= 512) ? 4 : 2;
     q.nacc_log2 = q.nacc == 4 ? 2 : 1;
     uint32_t cols = 32;

@@ -275,6 +275,30 @@ def test_b2048_tensor_path_multipass_and_deferred(flags):
     assert path == 1 and cnt.min() > 4096
 
 
+def test_single_pass_roi_with_a_counter_beyond_2048_is_caught_by_the_dc_column():
+    """With a spare accumulator column (N > 4 W) the tensor-core kernel bins a ROI of more than 2048 ions in ONE pass and checks
+    afterwards, through a "k = 0" twiddle column, that the counters the tensor core read sum to N_c -- they do unless some
+    counter exceeded 2048, where a u16 bit pattern stops being the fp16 number of the same value.  Here 2600 ions sit within
+    1e-4 nm of one point, so for almost every direction one bin holds more than 2048 of them: the material point must come
+    out right all the same (it is handed to the general kernel).  The second centre is an ordinary two-pass-sized ROI that
+    stays on the single-pass route."""
+    rng = np.random.Generator(np.random.PCG64(5))
+    xyz, types = _ball(3.0)
+    blob = (np.array([0.31, -0.12, 0.2]) + rng.uniform(-1e-4, 1e-4, (2600, 3))).astype(np.float32)
+    far = xyz[np.linalg.norm(xyz - np.array([0.31, -0.12, 0.2]), axis=1) > 1.2]      # thin the lattice around the blob
+    xyz = np.ascontiguousarray(np.concatenate([far, blob]).astype(np.float32))
+    rng.shuffle(xyz)
+    types = np.zeros(len(xyz), np.uint8)
+    for B, window, dirs in ((256, (12, 40), O.dirs_fibonacci(96)), (2048, (23, 51), apx.apx_dirs_geodesic(2))):
+        w = _case(xyz, types, 2.2, B)
+        centres = np.array([[0, 0, 0], [-0.6, 0.3, -0.2]], np.float32)
+        plan = apx.Plan(2.2, B, dirs, k_lo=window[0], k_hi=window[1], device=0)
+        assert plan.apx_plan_path() == 1
+        plan.apx_plan_destroy()
+        path, cnt = _check(w, dirs, centres, window, 0)
+        assert path == 1 and cnt.min() > 2600
+
+
 def test_large_roi_deferred_from_tensor_path_b1024():
     """B = 1024 on the auto path: more than 8192 ions exceed even the spill mode of the tensor-core kernel, the material
     point goes to the deferred list and the general kernel (streaming its cell rows) serves it in the same stream."""

@@ -504,7 +504,7 @@ def run_ours(args, rank, world, local_rank):
     pk = load_peaks()
     fp32_tflops = PAIR_FLOP * pairs / q_s / 1e12
     if path == "fft":
-        fp32_tflops += 2.5 * B * np.log2(B) * M_tot * D / q_s / 1e12        # unpruned real FFT, SURVEY 8(d)
+        fp32_tflops += 2.5 * B * np.log2(B) * M_tot * d_exec / q_s / 1e12   # unpruned real FFT of the EXECUTED histograms
     fp32_frac = fp32_tflops / pk["fp32_tflops"]
     atom_rate = pairs / 32.0 / q_s                             # one 32-lane shared atomic per 32 pairs
     atom_frac = atom_rate / pk["atom_warp_inst_per_s"]

@@ -40,7 +40,7 @@ typedef enum {
                                   windowed-DFT kernel cannot serve the plan (window too wide) */
 #define APX_FLAG_NORMALISE 8   /* apx_plan_create: write A / N_c instead of A (apx_sig_spec.normalise of the one signature) */
 #define APX_FLAG_LOCAL_MAX 16  /* apx_plan_create: APX_PEAK_LOCAL_MAX for the one signature (general FFT kernel) */
-#define APX_FLAG_NO_PAIRING 4  /* tensor-core kernel: no half-grid mode even when the grid is antipodally
+#define APX_FLAG_NO_PAIRING 4  /* either kernel: no half-grid mode even when the grid is antipodally
                                   symmetric (test hook; results are identical either way) */
 
 /* peak modes (L75 "particular bins"; L149-151 "second strongest peak") */
@@ -97,7 +97,7 @@ int apx_plan_destroy(apx_plan *plan);
 int apx_plan_constants(const apx_plan *plan, float *R2, float *s, float *freq_per_bin);
 /* 0 = general FFT kernel, 1 = tensor-core windowed-DFT kernel (chosen at create time from the window). */
 int apx_plan_path(const apx_plan *plan);
-/* 1 = half-grid mode of the tensor-core kernel: the direction grid is antipodally symmetric (every n has its exact
+/* 1 = half-grid mode of the plan's kernel (both kernels have one): the direction grid is antipodally symmetric (every n has its exact
  * negative in the grid, e.g. the paper's geodesic mesh, L60), so one member of every pair (n, -n) is binned and its
  * peak serves both (the histogram of -n is the mirror image: same amplitude spectrum); pairs with an ion whose
  * projection is an exact integer, where the mirror symmetry of Eq. 1's floor fails, are redone on their own.

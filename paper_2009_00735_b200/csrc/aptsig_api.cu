@@ -64,7 +64,7 @@ extern "C" int apx_plan_destroy(apx_plan *p)
 {
     if (!p) return APX_OK;
     DeviceGuard guard(p->device);
-    void *bufs[] = {p->dbg_centre, p->dbg_sig, p->d_refine_off, p->d_kaxis, p->d_fsp_list, p->d_dirs_scaled, p->d_twiddle, p->d_mma_table, p->d_mma_zero, p->d_mma_phase, p->d_dirs_sorted, p->d_dir_perm, p->d_dir_perm_mirror, p->d_type_mask, p->d_grid, p->d_cell_start,
+    void *bufs[] = {p->dbg_centre, p->dbg_sig, p->d_refine_off, p->d_kaxis, p->d_fsp_list, p->d_dirs_scaled, p->d_twiddle, p->d_mma_table, p->d_mma_zero, p->d_mma_phase, p->d_dirs_sorted, p->d_dir_perm, p->d_dir_perm_mirror, p->d_fft_half, p->d_fft_partner, p->d_type_mask, p->d_grid, p->d_cell_start,
                     p->d_cell_cursor, p->d_scan_tiles, p->d_cell_of_ion, p->d_sorted, p->d_deferred, p->h2d_xyz, p->h2d_types, p->h2d_centres,
                     p->d2h_sig, p->d2h_counts};
     for (void *b : bufs)
@@ -178,6 +178,27 @@ static int create_plan(const apx_plan_desc *desc, const apx_sig_spec *specs_in, 
         }
         p->need_clamp = unit ? 0 : 1;
     }
+    // Half-grid mode of the general kernel (antipodally symmetric grids, e.g. the paper's geodesic mesh, L60): it bins the
+    // lower-numbered member of every pair (n, -n) and writes the peak to both (signature_fft.cu).  Used whenever that kernel
+    // runs: plans on the FFT path and the material points the tensor-core kernel defers.
+    {
+        const int D = p->D;
+        std::vector<int32_t> partner((size_t)D, -1);
+        if (!p->need_clamp && !(desc->flags & APX_FLAG_NO_PAIRING) && D >= 2 && D % 2 == 0 &&
+            apx_dirs_antipodes(nps.data(), D, partner.data()) == 1) {
+            std::vector<int32_t> half;
+            half.reserve((size_t)D / 2);
+            for (int d = 0; d < D; ++d)
+                if (d < partner[d]) half.push_back(d);
+            if ((int)half.size() == D / 2) {
+                CUF(cudaMalloc(&p->d_fft_half, half.size() * 4));
+                CUF(cudaMalloc(&p->d_fft_partner, partner.size() * 4));
+                CUF(cudaMemcpy(p->d_fft_half, half.data(), half.size() * 4, cudaMemcpyHostToDevice));
+                CUF(cudaMemcpy(p->d_fft_partner, partner.data(), partner.size() * 4, cudaMemcpyHostToDevice));
+                p->fft_paired = 1;
+            }
+        }
+    }
     p->path = 0;
     if (!(desc->flags & APX_FLAG_FORCE_FFT) && !any_local && mma_path_supported(p)) {
         CUF(mma_path_prepare(p));
@@ -220,7 +241,7 @@ extern "C" int apx_plan_constants(const apx_plan *p, float *R2, float *s, float 
 }
 
 extern "C" int apx_plan_path(const apx_plan *p) { return p ? p->path : APX_EINVAL; }
-extern "C" int apx_plan_paired(const apx_plan *p) { return p ? (p->path == 1 ? p->mma_paired : 0) : APX_EINVAL; }
+extern "C" int apx_plan_paired(const apx_plan *p) { return p ? (p->path == 1 ? p->mma_paired : p->fft_paired) : APX_EINVAL; }
 extern "C" int apx_last_cuda_error(const apx_plan *p) { return p ? p->last_cuda : (int)cudaErrorInvalidValue; }
 
 extern "C" int apx_ingest(apx_plan *p, const float *xyz, const uint8_t *types, int64_t N, void *stream)

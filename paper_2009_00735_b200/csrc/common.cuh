@@ -60,6 +60,8 @@ struct Plan {
     int *d_dir_perm;               // [Dp] original index of each sorted slot, -1 = padding
     int *d_dir_perm_mirror;        // [Dp] half-grid mode: index of the direction opposite to the slot's
     int Dp;                        // D rounded up to a multiple of 32
+    int *d_fft_half, *d_fft_partner;   // general kernel's half-grid mode: binned member of each pair, partner of each direction
+    int fft_paired;                // 1 = the general (FFT) kernel runs in half-grid mode on this plan's symmetric grid
     int mma_paired;                // 1 = half-grid mode: the grid is antipodally symmetric, one direction per pair is binned
     int tune_unit_split, tune_nacc, tune_dc;   // k_signature_mma scheduling knobs (see mma_path_prepare)
     int need_clamp;                // 1 = the bin clamp of Eq. 1 can trigger and must stay in the kernels' inner loops

@@ -34,6 +34,10 @@ struct FftParams {
     const uint32_t *list;      // nullptr = direct mode; else list[0] = count, list[1..] = material point ids
     uint32_t *hist_out;        // test hook (apx_debug_histograms, M = 1): uint32[hist_nd][B] histograms of the directions
     int hist_d0, hist_nd;      // [hist_d0, hist_d0 + hist_nd), copied from the shared counters the FFT is about to read
+    // half-grid mode (antipodally symmetric grids, see the kernel): half[u] = the member of pair u that is binned,
+    // partner[d] = index of -d; nullptr = every direction on its own
+    const int *half, *partner;
+    int Dh;                    // pairs (D / 2)
     int D, k_lo, k_hi, cap, nchunks, ngroups, clamp;
     float R, R2;
     SpecSet ss;                // signatures of the plan: classes (type masks) and per-spec windows / modes
@@ -159,7 +163,7 @@ __device__ __forceinline__ void gather_roi(const FftParams &p, const GridParams 
     }
 }
 
-template <int B>
+template <int B, bool kHalf>
 __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const __grid_constant__ FftParams p)
 {
     constexpr int G = (B <= 1024) ? 32 : 32768 / B;            // directions per group
@@ -171,7 +175,17 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const __grid_c
     float2 *s_tw = reinterpret_cast<float2 *>(buf + (size_t)B * G);                // [B/2]
     float2 *cand = s_tw + B / 2;                                                   // [T][G]
     float *ions = reinterpret_cast<float *>(cand + T * G);                         // [cap][3]
-    __shared__ int s_n;
+    __shared__ int s_n, s_nfix;
+    __shared__ uint32_t s_mask;
+    __shared__ int s_fix[2 * G];
+    // Half-grid mode.  For -n every product and sum of Eq. 1's projection is negated exactly, so b(-n) = B - 1 - b(n) unless
+    // the projection is an exact integer: the histogram of -n is the mirror image of that of n and has the same amplitude
+    // spectrum.  A group then holds one member of G pairs and writes each peak to both directions.  Pairs that met an
+    // exact-integer projection (RD(x + magic) = RU(x + magic)) are flagged in s_mask; their -n members are collected in
+    // s_fix and binned on their own, G at a time, in fix-up groups between the ordinary ones (the list never holds more than
+    // 2G - 1 entries).  Results are identical to the full grid.
+    constexpr bool halfmode = kHalf;                            // (p.half != nullptr)
+    const int units = halfmode ? p.Dh : p.D;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int d = lane % G, t = warp * LPD + lane / G;                             // direction slot, thread index within it
@@ -192,7 +206,7 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const __grid_c
 
       for (int cls = 0; cls < p.ss.n_classes; ++cls) {     // specs with the same type mask share gather, binning and FFT
         __syncthreads();                 // previous item done with the shared buffers; s_tw loaded
-        if (tid == 0) s_n = 0;
+        if (tid == 0) { s_n = 0; s_nfix = 0; }
         __syncthreads();
         if (g.n_accepted) gather_roi(p, g, rc, cx, cy, cz, ions, &s_n, cls);
         __syncthreads();
@@ -202,17 +216,42 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const __grid_c
                 if (p.ss.cls_of[sp] == cls) p.counts[(size_t)sp * p.M + m] = (uint32_t)n;
         const bool stream = n > p.cap;
 
-        for (int gi = g_begin; gi < g_end; ++gi) {
+        for (int gi = g_begin;;) {
+            // ordinary group gi, or -- half-grid mode -- a fix-up group as soon as G flagged partners wait (all of them once the
+            // ordinary groups are done).  s_nfix was last written before the barrier that ended the previous iteration.
+            const int nf = halfmode ? s_nfix : 0;
+            const bool fix = nf >= G || (gi >= g_end && nf > 0);
+            if (!fix && gi >= g_end) break;
+            const int fcnt = fix ? min(nf, G) : 0;
+            int dsel = -1, dpart = -1;                          // direction of this lane's slot, its partner (written too)
+            if (!fix) {
+                const int u = gi * G + d;
+                if (u < units) { dsel = halfmode ? p.half[u] : u; dpart = halfmode ? p.partner[dsel] : -1; }
+            } else if (d < fcnt) {
+                dsel = s_fix[nf - fcnt + d];
+            }
+            const bool detect = halfmode && !fix;
+            if (tid == 0) s_mask = 0u;                          // (the previous iteration's readers are behind its last barrier)
             // ---- clear the counters -----------------------------------------------------------------
             {
                 uint4 *h = reinterpret_cast<uint4 *>(buf);
                 for (int i = tid; i < B * G / 4; i += kFftThreads) h[i] = make_uint4(0, 0, 0, 0);
             }
             __syncthreads();
+            if (tid == 0 && fix) s_nfix = nf - fcnt;            // (every thread has read nf and its list entry)
             // ---- project-and-bin (step a4): lane = direction, the T threads of a direction split the ions --
             {
-                const int dg = min(gi * G + d, p.D - 1);
+                const int dg = max(dsel, 0);
+                bool flagged = false;                           // this thread met an exact-integer projection
                 const float npx = p.dirs_scaled[3 * dg], npy = p.dirs_scaled[3 * dg + 1], npz = p.dirs_scaled[3 * dg + 2];
+                // bin of one ion (Eq. 1, clamped like bin_of); notes an exact-integer projection in half-grid mode
+                auto bin_x = [&](float dx, float dy, float dz) -> int {
+                    float x = __fmaf_rn(npz, dz, __fmaf_rn(npy, dy, __fmul_rn(npx, dx)));
+                    x = fminf(fmaxf(x, -half_b), half_b - 0.25f);
+                    const uint32_t ua = __float_as_uint(__fadd_rd(x, magic));
+                    if (detect) flagged |= ua == __float_as_uint(__fadd_ru(x, magic));
+                    return (int)(ua - 0x4B400000u);
+                };
                 uint32_t *cnt = reinterpret_cast<uint32_t *>(buf) + d;
                 if (!stream) {
                     // thread t takes ions t, t+T, ...; four independent chains per iteration
@@ -227,11 +266,12 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const __grid_c
                             float x = __fmaf_rn(npz, q[u].z, __fmaf_rn(npy, q[u].y, __fmul_rn(npx, q[u].x)));
                             if (p.clamp) x = fminf(fmaxf(x, -half_b), half_b - 0.25f);
                             const uint32_t ua = __float_as_uint(__fadd_rd(x, magic));
+                            if (detect) flagged |= ua == __float_as_uint(__fadd_ru(x, magic));
                             asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(ua * (uint32_t)(4 * G) + cb), "r"(1u) : "memory");
                         }
                     }
                     for (; i < n; i += T)
-                        atomicAdd(cnt + bin_of(npx, npy, npz, ions[3 * i], ions[3 * i + 1], ions[3 * i + 2], half_b, magic) * G, 1u);
+                        atomicAdd(cnt + bin_x(ions[3 * i], ions[3 * i + 1], ions[3 * i + 2]) * G, 1u);
                 } else {
                     // ROI larger than the shared ion buffer: walk the cell rows again, one ion per (warp, lane / G)
                     const int ny_r = rc.iy1 - rc.iy0 + 1, nz_r = rc.iz1 - rc.iz0 + 1;
@@ -243,10 +283,11 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const __grid_c
                             const float4 q = p.sorted[i];
                             const float dx = __fsub_rn(q.x, cx), dy = __fsub_rn(q.y, cy), dz = __fsub_rn(q.z, cz);
                             if (inside(dx, dy, dz, p.R2) && (p.ss.n_classes == 1 || type_in_class(p.ss, cls, __float_as_uint(q.w))))
-                                atomicAdd(cnt + bin_of(npx, npy, npz, dx, dy, dz, half_b, magic) * G, 1u);
+                                atomicAdd(cnt + bin_x(dx, dy, dz) * G, 1u);
                         }
                     }
                 }
+                if (flagged) atomicOr(&s_mask, 1u << d);
             }
             __syncthreads();
             if (p.hist_out && cls == 0) {                        // test hook (first class): counters complete, FFT not started
@@ -286,6 +327,8 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const __grid_c
                 const float xi = ei + (w.y * oi - w.x * orr);
                 return xr * xr + xi * xi;
             };
+            // flagged pairs: the -n member goes to the fix-up list (published by the barriers of the spec loop below)
+            if (detect && tid < G && dpart >= 0 && ((s_mask >> tid) & 1u)) s_fix[atomicAdd(&s_nfix, 1)] = dpart;
             for (int sp = 0; sp < p.ss.n_specs; ++sp) {
                 if (p.ss.cls_of[sp] != cls) continue;
                 const int s_lo = p.ss.k_lo[sp], s_hi = p.ss.k_hi[sp];
@@ -308,15 +351,18 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const __grid_c
                         const int ck = __float_as_int(c.y);
                         if (c.x > bb || (c.x == bb && ck < kb)) { bb = c.x; kb = ck; }
                     }
-                    const int dg = gi * G + tid;
                     float amp = 0.5f * sqrtf(fmaxf(bb, 0.0f));
                     if (p.ss.norm[sp]) amp = n ? __fdiv_rn(amp, (float)n) : 0.0f;
-                    if (dg < p.D) p.sig[(size_t)sp * p.M * p.D + (size_t)m * p.D + dg] = make_float2(amp, (float)kb);
+                    float2 *out = p.sig + (size_t)sp * p.M * p.D + (size_t)m * p.D;
+                    if (dsel >= 0) out[dsel] = make_float2(amp, (float)kb);           // (tid < G: this thread's slot is d = tid)
+                    // the mirrored histogram has the same amplitude spectrum
+                    if (dpart >= 0 && !((s_mask >> tid) & 1u)) out[dpart] = make_float2(amp, (float)kb);
                 }
                 __syncthreads();                                          // cand is reused by the next spec
             }
             // the next group's clear of buf is ordered after this group's reads by the barrier above; cand is
             // rewritten only after three more barriers
+            if (!fix) ++gi;
         }
       }
     }
@@ -330,7 +376,7 @@ static size_t fft_smem_for(int B, int cap)
 }
 static int fft_cap_for(int B)
 {
-    const size_t budget = 232448 - 256;
+    const size_t budget = 232448 - 1024;           // minus static shared (fix-up list, flags)
     return (int)(((budget - fft_smem_for(B, 0)) / 12) & ~(size_t)63);
 }
 
@@ -345,7 +391,10 @@ static cudaError_t launch_fft_common(Plan *p, const float *centres, int64_t M, c
     q.hist_out = p->dbg_hist_out; q.hist_d0 = p->dbg_d0; q.hist_nd = p->dbg_nd;
     q.ss = p->specs; q.M = M;
     q.list = list; q.D = p->D; q.k_lo = p->k_lo; q.k_hi = p->k_hi; q.cap = fft_cap_for(B);
-    q.ngroups = (p->D + G - 1) / G;
+    // half-grid mode on antipodally symmetric grids (not under the histogram export hook, which indexes groups by direction)
+    const bool halfmode = p->fft_paired && !p->dbg_hist_out;
+    q.half = halfmode ? p->d_fft_half : nullptr; q.partner = halfmode ? p->d_fft_partner : nullptr; q.Dh = p->D / 2;
+    q.ngroups = ((halfmode ? q.Dh : p->D) + G - 1) / G;
     // enough CTAs to fill the machine a few times over, but at least a handful of groups per CTA (one gather each)
     int nchunks = 1;
     const int64_t want = (int64_t)p->sm_count * 4;
@@ -366,11 +415,11 @@ static cudaError_t launch_fft_common(Plan *p, const float *centres, int64_t M, c
         return cudaGetLastError();
     };
     switch (B) {
-        case 256: return launch(k_signature_fft<256>);
-        case 512: return launch(k_signature_fft<512>);
-        case 1024: return launch(k_signature_fft<1024>);
-        case 2048: return launch(k_signature_fft<2048>);
-        case 4096: return launch(k_signature_fft<4096>);
+        case 256: return halfmode ? launch(k_signature_fft<256, true>) : launch(k_signature_fft<256, false>);
+        case 512: return halfmode ? launch(k_signature_fft<512, true>) : launch(k_signature_fft<512, false>);
+        case 1024: return halfmode ? launch(k_signature_fft<1024, true>) : launch(k_signature_fft<1024, false>);
+        case 2048: return halfmode ? launch(k_signature_fft<2048, true>) : launch(k_signature_fft<2048, false>);
+        case 4096: return halfmode ? launch(k_signature_fft<4096, true>) : launch(k_signature_fft<4096, false>);
         default: return cudaErrorInvalidValue;
     }
 }

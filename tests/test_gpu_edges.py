@@ -250,6 +250,43 @@ def test_half_grid_mode_with_exact_integer_projections(flags, centre_ions, B):
     _check(w, dirs, centres, (15, 34), flags)
 
 
+@pytest.mark.parametrize("B", [1024, 4096])
+@pytest.mark.parametrize("centre_ions", [False, True], ids=["some_flagged", "all_flagged"])
+@pytest.mark.parametrize("flags", [pytest.param(apx.APX_FLAG_FORCE_FFT, id="half"),
+                                   pytest.param(apx.APX_FLAG_FORCE_FFT | apx.APX_FLAG_NO_PAIRING, id="full")])
+def test_general_kernel_half_grid_mode_with_exact_integer_projections(flags, centre_ions, B):
+    """The same construction as above for the general (FFT) kernel, which has a half-grid mode of its own: one member of
+    every pair (n, -n) is binned and transformed, the peak is written to both, pairs that met an exact-integer projection
+    are flagged and their -n members are binned on their own in fix-up groups.  With an ion exactly on each centre EVERY
+    pair is flagged (all of -n goes through fix-up groups); B = 4096 runs 8 directions per group.  A second pass with a
+    wide window and the local-maximum peak mode covers the other epilogue."""
+    rng = np.random.Generator(np.random.PCG64(12))
+    R = (B / 2 - 1) / (B / 4)
+    c2 = np.array([0.25, 0.5, -0.25])
+    g = np.arange(-10, 11) / 4.0
+    grid = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+    grid = grid[(grid ** 2).sum(1) <= 2.6 ** 2]
+    on_centre = ((grid == 0).all(1)) | ((grid == c2).all(1))
+    grid = grid[(rng.random(len(grid)) < 0.25) & ~on_centre]
+    if centre_ions:
+        grid = np.concatenate([grid, np.zeros((1, 3)), c2[None]])
+    rnd = rng.uniform(-2.6, 2.6, size=(900, 3))
+    xyz = np.concatenate([grid, rnd]).astype(np.float32)
+    rng.shuffle(xyz)
+    dirs = apx.apx_dirs_geodesic(2 if B == 4096 else 3)
+    centres = np.array([[0, 0, 0], c2], np.float32)
+    w = _case(xyz, np.zeros(len(xyz), np.uint8), R, B)
+    plan = apx.Plan(R, B, dirs, k_lo=15, k_hi=34, device=0, flags=flags)
+    assert plan.apx_plan_path() == 0 and plan.apx_plan_paired() == (0 if flags & apx.APX_FLAG_NO_PAIRING else 1)
+    # the histogram export runs the same kernel with the pairing switched off: every direction's own counters
+    import torch
+    plan.apx_ingest(torch.from_numpy(w.xyz).cuda(), torch.from_numpy(w.types).cuda())
+    _hist_check(plan, w, dirs, centres[1], 0, min(len(dirs), 64))
+    plan.apx_plan_destroy()
+    _check(w, dirs, centres, (15, 34), flags)
+    _check(w, dirs, centres, (1, B // 2), flags)
+
+
 def test_half_grid_mode_is_off_for_asymmetric_grids():
     plan = apx.Plan(2.0, 1024, O.dirs_fibonacci(1000), k_lo=15, k_hi=34, device=0)
     assert plan.apx_plan_path() == 1 and plan.apx_plan_paired() == 0

@@ -404,8 +404,9 @@ def test_binding_rejects_wrong_dtype_shape_device():
     plan.apx_plan_destroy()
 
 
-def test_half_grid_full_machine_runs_are_bitwise_repeatable():
-    """Every SM busy with back-to-back groups (the regime where the warp-specialised pipeline of the tensor-core kernel runs
+@pytest.mark.parametrize("flags", PATHS)
+def test_half_grid_full_machine_runs_are_bitwise_repeatable(flags):
+    """(Both kernels, each in its half-grid mode.)  Every SM busy with back-to-back groups (the regime where the warp-specialised pipeline of the tensor-core kernel runs
     furthest ahead of its epilogues): 1200 single-pass ROIs on the symmetric geodesic grid, five runs, bit-identical outputs
     (counts are integers and every ROI is binned in one pass, so nothing may differ), and a sample against the oracle."""
     import torch
@@ -417,8 +418,8 @@ def test_half_grid_full_machine_runs_are_bitwise_repeatable():
     dirs = apx.apx_dirs_geodesic(4)
     centres = rng.uniform(1.0, 11.0, (1200, 3)).astype(np.float32)
     dev = torch.device("cuda:0")
-    plan = apx.Plan(2.0, 1024, dirs, k_lo=15, k_hi=34, device=0)
-    assert plan.apx_plan_paired() == 1
+    plan = apx.Plan(2.0, 1024, dirs, k_lo=15, k_hi=34, device=0, flags=flags)
+    assert plan.apx_plan_paired() == 1 and plan.apx_plan_path() == (0 if flags else 1)
     X, T, C_ = torch.from_numpy(xyz).to(dev), torch.from_numpy(types).to(dev), torch.from_numpy(centres).to(dev)
     ref_sig = None
     for _ in range(5):

@@ -226,7 +226,7 @@ def run_ingest(args):
     ms = sum(a.elapsed_time(b) for a, b in ev) / args.steps
     # algorithmic bytes per ion: xyz + type read by k_bounds and k_count (2 x 13), cell id written and read (2 x 4),
     # xyz read again and the 16-byte record written by k_scatter (12 + 16)
-    bytes_per_ion = 2 * 13 + 2 * 4 + 12 + 16
+    bytes_per_ion = 3 * 13 + 16                     # xyz + type read by the bounds, count and scatter passes; one 16-byte record written
     try:
         peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
         src = "MEASURED_PEAKS.json hbm_gbs"

@@ -41,11 +41,9 @@ static int ensure_capacity(apx_plan *p, int64_t N)
 {
     if (N <= p->capacity) return APX_OK;
     if (p->d_sorted) cudaFree(p->d_sorted);
-    if (p->d_cell_of_ion) cudaFree(p->d_cell_of_ion);
-    p->d_sorted = nullptr; p->d_cell_of_ion = nullptr; p->capacity = 0;
+    p->d_sorted = nullptr; p->capacity = 0;
     int64_t cap = N + N / 8 + 1024;
     CU(p, cudaMalloc(&p->d_sorted, (size_t)cap * sizeof(float4)));
-    CU(p, cudaMalloc(&p->d_cell_of_ion, (size_t)cap * sizeof(uint32_t)));
     p->capacity = cap;
     return APX_OK;
 }
@@ -65,7 +63,7 @@ extern "C" int apx_plan_destroy(apx_plan *p)
     if (!p) return APX_OK;
     DeviceGuard guard(p->device);
     void *bufs[] = {p->dbg_centre, p->dbg_sig, p->d_refine_off, p->d_kaxis, p->d_fsp_list, p->d_dirs_scaled, p->d_twiddle, p->d_mma_table, p->d_mma_zero, p->d_mma_phase, p->d_dirs_sorted, p->d_dir_perm, p->d_dir_perm_mirror, p->d_fft_half, p->d_fft_partner, p->d_type_mask, p->d_grid, p->d_cell_start,
-                    p->d_cell_cursor, p->d_scan_tiles, p->d_cell_of_ion, p->d_sorted, p->d_deferred, p->h2d_xyz, p->h2d_types, p->h2d_centres,
+                    p->d_cell_cursor, p->d_scan_tiles, p->d_sorted, p->d_deferred, p->h2d_xyz, p->h2d_types, p->h2d_centres,
                     p->d2h_sig, p->d2h_counts};
     for (void *b : bufs)
         if (b) cudaFree(b);

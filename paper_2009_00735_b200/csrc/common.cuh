@@ -84,7 +84,6 @@ struct Plan {
     uint32_t *d_cell_start;        // [kMaxCells + 1]
     uint32_t *d_cell_cursor;       // [kMaxCells]
     uint32_t *d_scan_tiles;        // [kMaxCells / 8192] tile totals of the cell scan
-    uint32_t *d_cell_of_ion;       // [capacity]
     float4 *d_sorted;              // [capacity]  (x, y, z, ion type bits)
     int64_t capacity;              // ions the sorted buffers can hold
     // host staging for apx_run_host

@@ -79,6 +79,35 @@ def test_multipass_binning_mma_b256():
     assert path == 1 and cnt.min() > 2048
 
 
+@pytest.mark.parametrize("off", [0, 1, 2, 3])
+def test_ingest_with_unaligned_inputs_and_ragged_tails(off):
+    """Ingest reads four ions per thread with 16-byte loads when the caller's arrays allow it: views that start 12 * off bytes
+    (coordinates) and off bytes (types) into an allocation, with ion counts of every residue mod 4, must give the same result
+    through the scalar loads; an ion-type filter and a few non-finite ions ride along."""
+    import torch
+    dev = torch.device("cuda:0")
+    rng = np.random.Generator(np.random.PCG64(3 + off))
+    xyz, _ = _ball(2.6, eta=0.6, sigma=0.03)
+    xyz = np.ascontiguousarray(xyz[: len(xyz) - off].astype(np.float32))
+    types = (rng.random(len(xyz)) < 0.3).astype(np.uint8)
+    xyz[5] = (np.nan, 0, 0); xyz[11] = (0, np.inf, 0)
+    dirs = O.dirs_fibonacci(40)
+    centres = np.array([[0, 0, 0], [1.0, -0.5, 0.3]], np.float32)
+    xt = torch.from_numpy(xyz).to(dev); tt = torch.from_numpy(types).to(dev)
+    plan = apx.Plan(1.5, 256, dirs, k_lo=7, k_hi=17, accepted_types={0}, device=0)
+    xv, tv = xt[off:], tt[off:]                                   # contiguous views, data pointers moved by 12 * off / off bytes
+    assert xv.data_ptr() % 16 == (12 * off) % 16 and xv.is_contiguous()
+    sig = torch.full((2, len(dirs), 2), -7.0, dtype=torch.float32, device=dev)
+    cnt = torch.full((2,), -1, dtype=torch.int32, device=dev)
+    plan.apx_run(xv, tv, torch.from_numpy(centres).to(dev), sig, cnt)
+    torch.cuda.synchronize()
+    plan.apx_plan_destroy()
+    with np.errstate(invalid="ignore"):
+        ref, rc, win = O.signatures(xyz[off:], types[off:], centres, dirs, 1.5, 256, k_lo=7, k_hi=17, accepted={0}, want_window=True)
+    assert_parity(sig.cpu().numpy(), cnt.cpu().numpy().astype(np.uint32), ref, rc, win, 7)
+    assert rc[0] > 300
+
+
 def test_streaming_fallback_fft():
     """ROI larger than the FFT kernel's shared ion buffer (~6900 ions at B = 1024): cell rows are streamed again
     for every direction group."""

@@ -376,7 +376,7 @@ def run_ours(args, rank, world, local_rank):
     from workloads import make_config
 
     dist = None
-    if world > 1:
+    if world > 1 or os.environ.get("APX_BENCH_DIST") == "1":   # (the variable: exercise the NCCL plumbing with a single rank under torchrun)
         import torch.distributed as dist_mod
         dist = dist_mod
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))

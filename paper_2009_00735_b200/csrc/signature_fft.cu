@@ -215,6 +215,21 @@ __global__ void __launch_bounds__(kFftThreads, 1) k_signature_fft(const __grid_c
             for (int sp = 0; sp < p.ss.n_specs; ++sp)
                 if (p.ss.cls_of[sp] == cls) p.counts[(size_t)sp * p.M + m] = (uint32_t)n;
         const bool stream = n > p.cap;
+        if (n == 0 && !p.hist_out) {
+            // empty ROI: all counters stay zero -> amplitude 0, lowest bin of each window (also for the local-maximum mode: no bin
+            // is a local maximum, the initial candidate k_lo stands); written without binning or transforming anything
+            for (int u = g_begin * G + tid; u < min(g_end * G, units); u += kFftThreads) {
+                const int dsel = halfmode ? p.half[u] : u, dpart = halfmode ? p.partner[dsel] : -1;
+                for (int sp = 0; sp < p.ss.n_specs; ++sp) {
+                    if (p.ss.cls_of[sp] != cls) continue;
+                    float2 *out = p.sig + (size_t)sp * p.M * p.D + (size_t)m * p.D;
+                    const float2 res = make_float2(0.0f, (float)p.ss.k_lo[sp]);
+                    out[dsel] = res;
+                    if (dpart >= 0) out[dpart] = res;
+                }
+            }
+            continue;
+        }
 
         for (int gi = g_begin;;) {
             // ordinary group gi, or -- half-grid mode -- a fix-up group as soon as G flagged partners wait (all of them once the

@@ -906,6 +906,23 @@ __device__ __forceinline__ void cta_body(const MmaParams &p, const MmaSmem &L, u
                     if (p.ss.cls_of[sp] == cls) p.counts[(size_t)sp * p.M + m] = (uint32_t)n;
         }
 
+        if (n == 0 && !p.hist_out) {
+            // empty ROI (e.g. a material point in the other phase of a filtered run): every histogram is zero, so every
+            // amplitude is 0 and the arg-max keeps the lowest bin of the window -- written without running the pipeline
+            constexpr int G = Lay<NB>::G;
+            for (int sl = g_begin * G + tid; sl < g_end * G; sl += kMmaThreads) {
+                const int d = p.perm[sl], d2 = kHalf ? p.perm_mirror[sl] : -1;
+                const int n_specs = kMulti ? p.ss.n_specs : 1;
+                for (int sp = 0; sp < n_specs; ++sp) {
+                    if (kMulti && p.ss.cls_of[sp] != cls) continue;
+                    float2 *out = p.sig + (kMulti ? (size_t)sp * (size_t)p.M * p.D : (size_t)0) + (size_t)m * p.D;
+                    const float2 res = make_float2(0.0f, (float)(kMulti ? p.ss.k_lo[sp] : p.k_lo));
+                    if (d >= 0) out[d] = res;
+                    if (d2 >= 0) out[d2] = res;
+                }
+            }
+            continue;
+        }
         int grp_total = 0;                                     // groups run by this CTA for this class (ordinary + fix-up)
         if (n > p.cap_big) {
             // too many ions even for ion buffer + second histogram buffer: leave this material point to the FFT kernel

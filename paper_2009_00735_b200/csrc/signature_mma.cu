@@ -431,10 +431,13 @@ struct EpiOut {
     const uint16_t *fix;
     int *ovf;                            // set to 1 when a slot's DC sum is not N_c: a counter left the exact fp16 range
 };
-template <bool kHalf, int NB, bool kMulti>
+// (Q = the warp's TMEM lane quarter as a compile-time constant: which of the four partial sums of a round stays in the warp and
+// which three go to the partners is then fixed in the code instead of being selected at run time)
+template <bool kHalf, int NB, bool kMulti, int Q>
 __device__ __forceinline__ void epilogue_group(const MmaParams &p, uint32_t acc, const EpiOut &eo, int64_t m, const float2 *phase,
-                                               float2 *exch_all, float2 *cand_all, int set, int q, int lane)
+                                            float2 *exch_all, float2 *cand_all, int set, int lane)
 {
+    constexpr int q = Q;
     const int mode = kHalf ? eo.mode : 0;
     const uint32_t mask = (kHalf && mode == 0) ? *eo.flag : 0u;         // complete: every binning warp has arrived
     const uint32_t acc0 = acc + ((uint32_t)(q * 32) << 16);
@@ -803,7 +806,13 @@ __device__ __forceinline__ void run_pipeline(const MmaParams &p, const MmaSmem &
             eo.cls = cls; eo.n = n;
             eo.mode = mode; eo.gi = sq.g0 + gl; eo.g0 = sq.g0; eo.f = gl; eo.nfix = sq.nfix;
             eo.flag = kHalf ? &ps.flag[gq & (kFlagSlots - 1)] : nullptr; eo.fix = ps.fix; eo.ovf = ps.ovf;
-            epilogue_group<kHalf, NB, kMulti>(p, tmem + (uint32_t)((gq & (p.nacc - 1)) * p.N), eo, m, phase, exch, cand, set, q, lane);
+            const uint32_t acc_g = tmem + (uint32_t)((gq & (p.nacc - 1)) * p.N);
+            switch (q) {                                                            // (warp-uniform)
+                case 0: epilogue_group<kHalf, NB, kMulti, 0>(p, acc_g, eo, m, phase, exch, cand, set, lane); break;
+                case 1: epilogue_group<kHalf, NB, kMulti, 1>(p, acc_g, eo, m, phase, exch, cand, set, lane); break;
+                case 2: epilogue_group<kHalf, NB, kMulti, 2>(p, acc_g, eo, m, phase, exch, cand, set, lane); break;
+                default: epilogue_group<kHalf, NB, kMulti, 3>(p, acc_g, eo, m, phase, exch, cand, set, lane); break;
+            }
             asm volatile("tcgen05.fence::before_thread_sync;");
             __syncwarp();
             APX_TRACE_EVENT(p, 8, gq);                                                // epilogue end

@@ -88,6 +88,46 @@ __device__ __forceinline__ float2 fm_phase(float k, float d)
     return make_float2(c, s);
 }
 
+// Operand tiles of one chunk (see the kernel).  off[u] = byte offset of (row kFmPer * seg + u, K pair j) in a tile, computed
+// once per CTA: the rows 64 further down (second z-slice of A, imaginary block of B) sit exactly 8192 bytes behind, because
+// the swizzle only looks at the row index modulo 8.
+template <bool kFull>
+__device__ __forceinline__ void fm_build_tiles(const FspMmaParams &p, unsigned char *Ah, unsigned char *Al, unsigned char *Bh,
+                                               unsigned char *Bl, const float *ions, const float2 (*s_ion)[kFmChunk],
+                                               const uint32_t (&off)[kFmPer], int w0, int n, int iy0, int ix0, int L, int tid)
+{
+    const int j = tid & 31, seg = tid >> 5;
+    const bool ion_ok = kFull || w0 + j < n;
+    const float dx = ion_ok ? ions[3 * (w0 + j)] : 0.f, dy = ion_ok ? ions[3 * (w0 + j) + 1] : 0.f;
+    const float2 ez0 = s_ion[0][j], ez1 = s_ion[1][j], ry = s_ion[2][j], rx = s_ion[3][j];
+    float2 ey = fm_phase(p.kaxis[min(iy0 + kFmPer * seg, L - 1)], dy), ex = fm_phase(p.kaxis[min(ix0 + kFmPer * seg, L - 1)], dx);
+#pragma unroll
+    for (int u = 0; u < kFmPer; ++u) {
+        const int t64 = kFmPer * seg + u;
+        const bool y_ok = kFull || (ion_ok && iy0 + t64 < L), x_ok = kFull || (ion_ok && ix0 + t64 < L);
+#pragma unroll
+        for (int zl = 0; zl < 2; ++zl) {
+            const float2 ez = zl ? ez1 : ez0;                      // (zero for a missing ion / slice)
+            const float ar = y_ok ? ez.x * ey.x - ez.y * ey.y : 0.f, ai = y_ok ? ez.x * ey.y + ez.y * ey.x : 0.f;
+            uint32_t hi, lo;
+            fm_split2(ar, ai, hi, lo);
+            *reinterpret_cast<uint32_t *>(Ah + off[u] + zl * 8192u) = hi;
+            *reinterpret_cast<uint32_t *>(Al + off[u] + zl * 8192u) = lo;
+        }
+        {
+            uint32_t hi, lo;                                       // (Re e, Im e) in (low, high) halves
+            fm_split2(x_ok ? ex.x : 0.f, x_ok ? ex.y : 0.f, hi, lo);
+            *reinterpret_cast<uint32_t *>(Bh + off[u]) = hi ^ 0x80000000u;                    // (Re e, -Im e)
+            *reinterpret_cast<uint32_t *>(Bl + off[u]) = lo ^ 0x80000000u;
+            *reinterpret_cast<uint32_t *>(Bh + off[u] + 8192u) = __byte_perm(hi, 0, 0x1032);    // (Im e,  Re e)
+            *reinterpret_cast<uint32_t *>(Bl + off[u] + 8192u) = __byte_perm(lo, 0, 0x1032);
+        }
+        const float2 ny = make_float2(ey.x * ry.x - ey.y * ry.y, ey.x * ry.y + ey.y * ry.x);
+        const float2 nx = make_float2(ex.x * rx.x - ex.y * rx.y, ex.x * rx.y + ex.y * rx.x);
+        ey = ny; ex = nx;
+    }
+}
+
 __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant__ FspMmaParams p)
 {
     extern __shared__ unsigned char fm_raw[];
@@ -165,6 +205,9 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
     const float kz0 = p.kaxis[min(iz0, L - 1)], kz1 = p.kaxis[min(iz0 + 1, L - 1)];
     const bool z1_valid = iz0 + 1 < L;
 
+    uint32_t tile_off[kFmPer];
+#pragma unroll
+    for (int u = 0; u < kFmPer; ++u) tile_off[u] = fm_off(kFmPer * (tid >> 5) + u, tid & 31);
     for (int c = 0; c < nchunks; ++c) {
         const int s = c & 1, use = c >> 1;
         if (use >= 1) fm_mbar_wait(&s_done[s], (uint32_t)((use - 1) & 1));        // the MMAs that read this stage have completed
@@ -187,40 +230,12 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
         // thread = (ion j of the chunk, kFmPer consecutive iy and ix): the phase factor of the first one comes from sincospif,
         // the next ones by multiplying with the step factor -- a few fp32 complex products add < 4e-7 to the phase, inside the
         // tolerance budget of DESIGN.md section 2.  A warp writes one 128-byte operand row per store (32 consecutive K pairs):
-        // conflict-free.  Splits x = hi + lo / 2048 are taken two values at a time (cvt.rn.f16x2.f32).
+        // conflict-free.  Splits x = hi + lo / 2048 are taken two values at a time (cvt.rn.f16x2.f32).  A chunk of 32 ions in a
+        // tile that lies inside the k grid (the common case) takes the copy without the validity selects.
         {
-            const int j = tid & 31, seg = tid >> 5;
-            const bool ion_ok = w0 + j < n;
-            const float dx = ion_ok ? ions[3 * (w0 + j)] : 0.f, dy = ion_ok ? ions[3 * (w0 + j) + 1] : 0.f;
-            const float2 ez0 = s_ion[0][j], ez1 = s_ion[1][j], ry = s_ion[2][j], rx = s_ion[3][j];
-            float2 ey = fm_phase(p.kaxis[min(iy0 + kFmPer * seg, L - 1)], dy), ex = fm_phase(p.kaxis[min(ix0 + kFmPer * seg, L - 1)], dx);
-#pragma unroll
-            for (int u = 0; u < kFmPer; ++u) {
-                const int t64 = kFmPer * seg + u;
-                const bool y_ok = ion_ok && iy0 + t64 < L, x_ok = ion_ok && ix0 + t64 < L;
-#pragma unroll
-                for (int zl = 0; zl < 2; ++zl) {
-                    const float2 ez = zl ? ez1 : ez0;                      // (zero for a missing ion / slice)
-                    const float ar = y_ok ? ez.x * ey.x - ez.y * ey.y : 0.f, ai = y_ok ? ez.x * ey.y + ez.y * ey.x : 0.f;
-                    uint32_t hi, lo;
-                    fm_split2(ar, ai, hi, lo);
-                    const uint32_t off = fm_off(zl * 64 + t64, j);
-                    *reinterpret_cast<uint32_t *>(Ah + off) = hi;
-                    *reinterpret_cast<uint32_t *>(Al + off) = lo;
-                }
-                {
-                    uint32_t hi, lo;                                       // (Re e, Im e) in (low, high) halves
-                    fm_split2(x_ok ? ex.x : 0.f, x_ok ? ex.y : 0.f, hi, lo);
-                    const uint32_t o_re = fm_off(t64, j), o_im = fm_off(64 + t64, j);
-                    *reinterpret_cast<uint32_t *>(Bh + o_re) = hi ^ 0x80000000u;                  // (Re e, -Im e)
-                    *reinterpret_cast<uint32_t *>(Bl + o_re) = lo ^ 0x80000000u;
-                    *reinterpret_cast<uint32_t *>(Bh + o_im) = __byte_perm(hi, 0, 0x1032);          // (Im e,  Re e)
-                    *reinterpret_cast<uint32_t *>(Bl + o_im) = __byte_perm(lo, 0, 0x1032);
-                }
-                const float2 ny = make_float2(ey.x * ry.x - ey.y * ry.y, ey.x * ry.y + ey.y * ry.x);
-                const float2 nx = make_float2(ex.x * rx.x - ex.y * rx.y, ex.x * rx.y + ex.y * rx.x);
-                ey = ny; ex = nx;
-            }
+            const bool full = w0 + kFmChunk <= n && iy0 + 64 <= L && ix0 + 64 <= L && z1_valid;
+            if (full) fm_build_tiles<true>(p, Ah, Al, Bh, Bl, ions, s_ion, tile_off, w0, n, iy0, ix0, L, tid);
+            else fm_build_tiles<false>(p, Ah, Al, Bh, Bl, ions, s_ion, tile_off, w0, n, iy0, ix0, L, tid);
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");       // operand tiles -> async proxy (tensor core)
         asm volatile("tcgen05.fence::before_thread_sync;");

@@ -342,7 +342,7 @@ extern "C" int apx_fsp_noalloc(apx_plan *p, const float *centres, int64_t M, flo
     const size_t smem = sizeof(float) * (4 * kFspStep * kFspTile + 4 * kFspStep + 3 * kFspCap);
     e = cudaFuncSetAttribute(k_fsp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return cu(e);
-    const int64_t blocks = p->fsp_path == 1 ? M * L * tiles * tiles : M * ((L + 1) / 2) * tiles * tiles;
+    const int64_t blocks = p->fsp_path == 1 ? M * L * tiles * tiles : M * ((L + 3) / 4) * tiles * tiles     /* k_fsp_mma: four z-slices per CTA */;
     if (blocks > 0x7FFFFFFFLL) return done(APX_ERANGE);
     k_fsp_noalloc_prepare<<<1, 1024, 0, st>>>(scratch, k_max, L);
     FspParams q;

@@ -9,9 +9,10 @@
 // so that C'[m][(re,ix)] = Re C and C'[m][(im,ix)] = Im C.  Operands are fp16; to keep fp32-level accuracy every operand is
 // split x = hi + 2^-11 lo (both fp16) and three products are accumulated in fp32 in TMEM:
 //     D0 += Ah Bh,   D1 += Ah Bl + Al Bh,   C' = D0 + D1 / 2048        (the lo*lo term, 2^-22 relative, is dropped).
-// CTA = (material point, pair of z-slices, 64 x 64 tile of (iy, ix)); ions in chunks of 32 (K' = 64 = one 128-byte swizzle
-// row).  All 512 threads build the four operand tiles of a chunk (phase factors by sincospif, exact argument reduction) in
-// one of two shared-memory stages, one thread issues the 12 tcgen05.mma of the chunk and commits to the stage's mbarrier;
+// CTA = (material point, TWO pairs of z-slices, 64 x 64 tile of (iy, ix)): the B' tiles and the ey / ex factors of a chunk are
+// built once and feed both pairs (each pair has its own A tiles and its own D0 / D1 accumulators: 4 x 128 = all 512 TMEM
+// columns); ions in chunks of 32 (K' = 64 = one 128-byte swizzle row).  All 512 threads build the four operand tiles of a chunk (phase factors by sincospif, exact argument reduction) in
+// one of two shared-memory stages, one thread issues the 24 tcgen05.mma of the chunk and commits to the stage's mbarrier;
 // building chunk c+1 overlaps the MMAs of chunk c.  ROIs with more ions than the shared buffer are left to k_fsp (fsp.cu).
 #include <cuda_fp16.h>
 #include "common.cuh"
@@ -23,7 +24,10 @@ constexpr int kFmThreads = 512;
 constexpr int kFmPer = 64 / (kFmThreads / 32);   // consecutive iy / ix per thread when the operand tiles are built
 constexpr int kFmChunk = 32;                  // ions per chunk
 constexpr int kFmTileBytes = 128 * 128;       // 128 rows x 64 fp16 (K-major, SWIZZLE_128B)
-constexpr int kFmStageBytes = 4 * kFmTileBytes;   // Ah, Al, Bh, Bl
+constexpr int kFmPairs = 2;                   // z-slice pairs per CTA: one B' tile and one set of ey / ex factors feed all of them
+constexpr int kFmSlices = 2 * kFmPairs;
+constexpr int kFmStageBytes = (2 * kFmPairs + 2) * kFmTileBytes;   // (Ah, Al) per slice pair, Bh, Bl
+constexpr int kFmCap = 2752;                  // ions held in shared memory beside the two stages
 
 struct FspMmaParams {
     const float4 *sorted;
@@ -92,27 +96,30 @@ __device__ __forceinline__ float2 fm_phase(float k, float d)
 // once per CTA: the rows 64 further down (second z-slice of A, imaginary block of B) sit exactly 8192 bytes behind, because
 // the swizzle only looks at the row index modulo 8.
 template <bool kFull>
-__device__ __forceinline__ void fm_build_tiles(const FspMmaParams &p, unsigned char *Ah, unsigned char *Al, unsigned char *Bh,
+__device__ __forceinline__ void fm_build_tiles(const FspMmaParams &p, unsigned char *A, unsigned char *Bh,
                                                unsigned char *Bl, const float *ions, const float2 (*s_ion)[kFmChunk],
                                                const uint32_t (&off)[kFmPer], int w0, int n, int iy0, int ix0, int L, int tid)
 {
     const int j = tid & 31, seg = tid >> 5;
     const bool ion_ok = kFull || w0 + j < n;
     const float dx = ion_ok ? ions[3 * (w0 + j)] : 0.f, dy = ion_ok ? ions[3 * (w0 + j) + 1] : 0.f;
-    const float2 ez0 = s_ion[0][j], ez1 = s_ion[1][j], ry = s_ion[2][j], rx = s_ion[3][j];
+    float2 ez[kFmSlices];
+#pragma unroll
+    for (int zl = 0; zl < kFmSlices; ++zl) ez[zl] = s_ion[zl][j];                 // (zero for a missing ion / slice)
+    const float2 ry = s_ion[kFmSlices][j], rx = s_ion[kFmSlices + 1][j];
     float2 ey = fm_phase(p.kaxis[min(iy0 + kFmPer * seg, L - 1)], dy), ex = fm_phase(p.kaxis[min(ix0 + kFmPer * seg, L - 1)], dx);
 #pragma unroll
     for (int u = 0; u < kFmPer; ++u) {
         const int t64 = kFmPer * seg + u;
         const bool y_ok = kFull || (ion_ok && iy0 + t64 < L), x_ok = kFull || (ion_ok && ix0 + t64 < L);
 #pragma unroll
-        for (int zl = 0; zl < 2; ++zl) {
-            const float2 ez = zl ? ez1 : ez0;                      // (zero for a missing ion / slice)
-            const float ar = y_ok ? ez.x * ey.x - ez.y * ey.y : 0.f, ai = y_ok ? ez.x * ey.y + ez.y * ey.x : 0.f;
+        for (int zl = 0; zl < kFmSlices; ++zl) {
+            const float ar = y_ok ? ez[zl].x * ey.x - ez[zl].y * ey.y : 0.f, ai = y_ok ? ez[zl].x * ey.y + ez[zl].y * ey.x : 0.f;
             uint32_t hi, lo;
             fm_split2(ar, ai, hi, lo);
-            *reinterpret_cast<uint32_t *>(Ah + off[u] + zl * 8192u) = hi;
-            *reinterpret_cast<uint32_t *>(Al + off[u] + zl * 8192u) = lo;
+            unsigned char *Ah = A + (zl >> 1) * (2 * kFmTileBytes), *Al = Ah + kFmTileBytes;      // tiles of slice pair zl / 2
+            *reinterpret_cast<uint32_t *>(Ah + off[u] + (zl & 1) * 8192u) = hi;
+            *reinterpret_cast<uint32_t *>(Al + off[u] + (zl & 1) * 8192u) = lo;
         }
         {
             uint32_t hi, lo;                                       // (Re e, Im e) in (low, high) halves
@@ -137,17 +144,17 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
     __shared__ uint64_t s_done[2], s_final;
     __shared__ uint32_t s_tmem;
     __shared__ int s_n;
-    __shared__ float2 s_ion[4][kFmChunk];         // per ion of the chunk: ez (slice 0), ez (slice 1), step factors along y, x
+    __shared__ float2 s_ion[kFmSlices + 2][kFmChunk];   // per ion of the chunk: ez of the CTA's slices, step factors along y, x
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int L = p.L;
     int b = blockIdx.x;
     const int tx_tile = b % p.tiles; b /= p.tiles;
     const int ty_tile = b % p.tiles; b /= p.tiles;
-    const int nzp = (L + 1) / 2;
+    const int nzp = (L + kFmSlices - 1) / kFmSlices;         // groups of kFmSlices z-slices
     const int izp = b % nzp;
     const int64_t m = b / nzp;
-    const int iz0 = 2 * izp, iy0 = ty_tile * 64, ix0 = tx_tile * 64;
+    const int iz0 = kFmSlices * izp, iy0 = ty_tile * 64, ix0 = tx_tile * 64;
     const GridParams g = *p.grid;
     const float cx = p.centres[3 * m], cy = p.centres[3 * m + 1], cz = p.centres[3 * m + 2];
     const RoiCells rc = roi_cells(g, cx, cy, cz, p.R);
@@ -159,7 +166,7 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
         s_n = 0;
     }
     if (wid == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(fm_smem_u32(&s_tmem)), "r"(256u));
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(fm_smem_u32(&s_tmem)), "r"(256u * kFmPairs));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
@@ -202,8 +209,7 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
     const uint32_t idesc = (1u << 4) | ((uint32_t)(128 >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
     const uint32_t d_hi = (uint32_t)(1024 >> 4) | (1u << 14) | (2u << 29);                  // SBO = 1024 B, version 1, SWIZZLE_128B
     const int nchunks = skip ? 0 : (n + kFmChunk - 1) / kFmChunk;
-    const float kz0 = p.kaxis[min(iz0, L - 1)], kz1 = p.kaxis[min(iz0 + 1, L - 1)];
-    const bool z1_valid = iz0 + 1 < L;
+    const bool z_all_valid = iz0 + kFmSlices <= L;
 
     uint32_t tile_off[kFmPer];
 #pragma unroll
@@ -211,17 +217,16 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
     for (int c = 0; c < nchunks; ++c) {
         const int s = c & 1, use = c >> 1;
         if (use >= 1) fm_mbar_wait(&s_done[s], (uint32_t)((use - 1) & 1));        // the MMAs that read this stage have completed
-        unsigned char *Ah = stage0 + s * kFmStageBytes, *Al = Ah + kFmTileBytes, *Bh = Al + kFmTileBytes, *Bl = Bh + kFmTileBytes;
+        unsigned char *A = stage0 + s * kFmStageBytes, *Bh = A + 2 * kFmPairs * kFmTileBytes, *Bl = Bh + kFmTileBytes;
         const int w0 = c * kFmChunk;
         // per-ion factors of the chunk, computed once: phases along z for the two slices and the step factors exp(-2 pi i dk d)
         // along y and x (sincospif: exact argument reduction)
-        if (tid < 4 * kFmChunk) {
+        if (tid < (kFmSlices + 2) * kFmChunk) {
             const int j = tid & (kFmChunk - 1), which = tid / kFmChunk;
             float2 e = make_float2(0.f, 0.f);
             if (w0 + j < n) {
-                if (which == 0) e = fm_phase(kz0, ions[3 * (w0 + j) + 2]);
-                else if (which == 1) e = z1_valid ? fm_phase(kz1, ions[3 * (w0 + j) + 2]) : e;
-                else if (which == 2) e = fm_phase(p.dk, ions[3 * (w0 + j) + 1]);
+                if (which < kFmSlices) e = iz0 + which < L ? fm_phase(p.kaxis[min(iz0 + which, L - 1)], ions[3 * (w0 + j) + 2]) : e;
+                else if (which == kFmSlices) e = fm_phase(p.dk, ions[3 * (w0 + j) + 1]);
                 else e = fm_phase(p.dk, ions[3 * (w0 + j)]);
             }
             s_ion[which][j] = e;
@@ -233,26 +238,30 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
         // conflict-free.  Splits x = hi + lo / 2048 are taken two values at a time (cvt.rn.f16x2.f32).  A chunk of 32 ions in a
         // tile that lies inside the k grid (the common case) takes the copy without the validity selects.
         {
-            const bool full = w0 + kFmChunk <= n && iy0 + 64 <= L && ix0 + 64 <= L && z1_valid;
-            if (full) fm_build_tiles<true>(p, Ah, Al, Bh, Bl, ions, s_ion, tile_off, w0, n, iy0, ix0, L, tid);
-            else fm_build_tiles<false>(p, Ah, Al, Bh, Bl, ions, s_ion, tile_off, w0, n, iy0, ix0, L, tid);
+            const bool full = w0 + kFmChunk <= n && iy0 + 64 <= L && ix0 + 64 <= L && z_all_valid;
+            if (full) fm_build_tiles<true>(p, A, Bh, Bl, ions, s_ion, tile_off, w0, n, iy0, ix0, L, tid);
+            else fm_build_tiles<false>(p, A, Bh, Bl, ions, s_ion, tile_off, w0, n, iy0, ix0, L, tid);
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");       // operand tiles -> async proxy (tensor core)
         asm volatile("tcgen05.fence::before_thread_sync;");
         __syncthreads();
         if (tid == 0) {
             asm volatile("tcgen05.fence::after_thread_sync;");
-            const uint32_t ah = (fm_smem_u32(Ah) >> 4) & 0x3FFFu, al = (fm_smem_u32(Al) >> 4) & 0x3FFFu;
             const uint32_t bh = (fm_smem_u32(Bh) >> 4) & 0x3FFFu, bl = (fm_smem_u32(Bl) >> 4) & 0x3FFFu;
 #pragma unroll
-            for (int ks = 0; ks < 4; ++ks) {                    // K = 16 per MMA: +32 bytes inside the 128-byte swizzle row
-                const uint32_t adv = (uint32_t)ks * 2u;
-                const uint64_t dAh = ((uint64_t)d_hi << 32) | ((ah + adv) | (1u << 16)), dAl = ((uint64_t)d_hi << 32) | ((al + adv) | (1u << 16));
-                const uint64_t dBh = ((uint64_t)d_hi << 32) | ((bh + adv) | (1u << 16)), dBl = ((uint64_t)d_hi << 32) | ((bl + adv) | (1u << 16));
-                const uint32_t first = (c == 0 && ks == 0) ? 0u : 1u;
-                fm_mma(tmem, dAh, dBh, idesc, first);            // D0 += Ah Bh
-                fm_mma(tmem + 128u, dAh, dBl, idesc, first);     // D1 += Ah Bl
-                fm_mma(tmem + 128u, dAl, dBh, idesc, 1u);        // D1 += Al Bh
+            for (int pr = 0; pr < kFmPairs; ++pr) {             // slice pair pr: its own A tiles and accumulators, the shared B' tiles
+                const uint32_t ah = (fm_smem_u32(A + pr * 2 * kFmTileBytes) >> 4) & 0x3FFFu, al = ah + (uint32_t)(kFmTileBytes >> 4);
+                const uint32_t acc = tmem + 256u * (uint32_t)pr;
+#pragma unroll
+                for (int ks = 0; ks < 4; ++ks) {                // K = 16 per MMA: +32 bytes inside the 128-byte swizzle row
+                    const uint32_t adv = (uint32_t)ks * 2u;
+                    const uint64_t dAh = ((uint64_t)d_hi << 32) | ((ah + adv) | (1u << 16)), dAl = ((uint64_t)d_hi << 32) | ((al + adv) | (1u << 16));
+                    const uint64_t dBh = ((uint64_t)d_hi << 32) | ((bh + adv) | (1u << 16)), dBl = ((uint64_t)d_hi << 32) | ((bl + adv) | (1u << 16));
+                    const uint32_t first = (c == 0 && ks == 0) ? 0u : 1u;
+                    fm_mma(acc, dAh, dBh, idesc, first);            // D0 += Ah Bh
+                    fm_mma(acc + 128u, dAh, dBl, idesc, first);     // D1 += Ah Bl
+                    fm_mma(acc + 128u, dAl, dBh, idesc, 1u);        // D1 += Al Bh
+                }
             }
             asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(fm_smem_u32(&s_done[s])) : "memory");
             if (c == nchunks - 1)
@@ -261,38 +270,44 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
     }
 
     // ---- epilogue: |C'| -> out[m][iz][iy][ix]; warps 0..3 own TMEM lane quarters = rows (iz_local = q / 2, iy = 32 (q & 1) + lane)
+    //      of every slice pair; pair pr has its accumulators at columns 256 pr
     if (!skip && wid < 4) {
-        const int zl = wid >> 1, iy = iy0 + 32 * (wid & 1) + lane, iz = iz0 + zl;
-        const bool row_ok = iz < L && iy < L;
-        float *o = p.out + (((size_t)m * L + min(iz, L - 1)) * L + min(iy, L - 1)) * (size_t)L + ix0;
         if (nchunks > 0) {
             fm_mbar_wait(&s_final, 0u);
             asm volatile("tcgen05.fence::after_thread_sync;");
-            const uint32_t row_addr = tmem + ((uint32_t)(wid * 32) << 16);
+        }
 #pragma unroll 1
-            for (int cb = 0; cb < 4; ++cb) {                      // 16 ix per step: Re at columns ix, Im at 64 + ix, D1 at +128
-                uint32_t r0[16], r1[16], i0[16], i1[16];
-                fm_tmem_ld16(row_addr + (uint32_t)(16 * cb), r0);
-                fm_tmem_ld16(row_addr + (uint32_t)(128 + 16 * cb), r1);
-                fm_tmem_ld16(row_addr + (uint32_t)(64 + 16 * cb), i0);
-                fm_tmem_ld16(row_addr + (uint32_t)(192 + 16 * cb), i1);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        for (int pr = 0; pr < kFmPairs; ++pr) {
+            const int zl = 2 * pr + (wid >> 1), iy = iy0 + 32 * (wid & 1) + lane, iz = iz0 + zl;
+            const bool row_ok = iz < L && iy < L;
+            float *o = p.out + (((size_t)m * L + min(iz, L - 1)) * L + min(iy, L - 1)) * (size_t)L + ix0;
+            if (nchunks > 0) {
+                const uint32_t row_addr = tmem + 256u * (uint32_t)pr + ((uint32_t)(wid * 32) << 16);
+#pragma unroll 1
+                for (int cb = 0; cb < 4; ++cb) {                  // 16 ix per step: Re at columns ix, Im at 64 + ix, D1 at +128
+                    uint32_t r0[16], r1[16], i0[16], i1[16];
+                    fm_tmem_ld16(row_addr + (uint32_t)(16 * cb), r0);
+                    fm_tmem_ld16(row_addr + (uint32_t)(128 + 16 * cb), r1);
+                    fm_tmem_ld16(row_addr + (uint32_t)(64 + 16 * cb), i0);
+                    fm_tmem_ld16(row_addr + (uint32_t)(192 + 16 * cb), i1);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-                for (int e = 0; e < 16; ++e) {
-                    const float re = __uint_as_float(r0[e]) + __uint_as_float(r1[e]) * (1.0f / 2048.0f);
-                    const float im = __uint_as_float(i0[e]) + __uint_as_float(i1[e]) * (1.0f / 2048.0f);
-                    const int ix = ix0 + 16 * cb + e;
-                    if (row_ok && ix < L) o[16 * cb + e] = sqrtf(re * re + im * im);
+                    for (int e = 0; e < 16; ++e) {
+                        const float re = __uint_as_float(r0[e]) + __uint_as_float(r1[e]) * (1.0f / 2048.0f);
+                        const float im = __uint_as_float(i0[e]) + __uint_as_float(i1[e]) * (1.0f / 2048.0f);
+                        const int ix = ix0 + 16 * cb + e;
+                        if (row_ok && ix < L) o[16 * cb + e] = sqrtf(re * re + im * im);
+                    }
                 }
+            } else if (row_ok) {                                 // empty ROI: F = 0
+                for (int e = 0; e < 64; ++e)
+                    if (ix0 + e < L) o[e] = 0.f;
             }
-        } else if (row_ok) {                                     // empty ROI: F = 0
-            for (int e = 0; e < 64; ++e)
-                if (ix0 + e < L) o[e] = 0.f;
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
-    if (wid == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(256u));
+    if (wid == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(256u * kFmPairs));
 }
 
 // launcher (called by apx_fsp)
@@ -301,8 +316,8 @@ cudaError_t launch_fsp_mma(Plan *p, const float *centres, int64_t M, int L, floa
 {
     FspMmaParams q;
     q.sorted = p->d_sorted; q.cell_start = p->d_cell_start; q.grid = p->d_grid; q.centres = centres; q.kaxis = p->d_kaxis;
-    q.out = out; q.counts = counts; q.list = list; q.L = L; q.tiles = (L + 63) / 64; q.cap = 4096; q.R = p->R; q.R2 = p->R2; q.dk = dk;
-    const int64_t blocks = M * ((L + 1) / 2) * q.tiles * q.tiles;
+    q.out = out; q.counts = counts; q.list = list; q.L = L; q.tiles = (L + 63) / 64; q.cap = kFmCap; q.R = p->R; q.R2 = p->R2; q.dk = dk;
+    const int64_t blocks = M * ((L + kFmSlices - 1) / kFmSlices) * q.tiles * q.tiles;
     if (blocks > 0x7FFFFFFFLL) return cudaErrorInvalidConfiguration;
     const size_t smem = 2 * (size_t)kFmStageBytes + (size_t)q.cap * 12 + 1024;
     cudaError_t e = cudaFuncSetAttribute(k_fsp_mma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -318,8 +333,8 @@ cudaError_t launch_fsp_mma_at(Plan *p, const float *kaxis, const float *centres,
 {
     FspMmaParams q;
     q.sorted = p->d_sorted; q.cell_start = p->d_cell_start; q.grid = p->d_grid; q.centres = centres; q.kaxis = kaxis;
-    q.out = out; q.counts = counts; q.list = list; q.L = L; q.tiles = (L + 63) / 64; q.cap = 4096; q.R = p->R; q.R2 = p->R2; q.dk = dk;
-    const int64_t blocks = M * ((L + 1) / 2) * q.tiles * q.tiles;
+    q.out = out; q.counts = counts; q.list = list; q.L = L; q.tiles = (L + 63) / 64; q.cap = kFmCap; q.R = p->R; q.R2 = p->R2; q.dk = dk;
+    const int64_t blocks = M * ((L + kFmSlices - 1) / kFmSlices) * q.tiles * q.tiles;
     if (blocks > 0x7FFFFFFFLL) return cudaErrorInvalidConfiguration;
     const size_t smem = 2 * (size_t)kFmStageBytes + (size_t)q.cap * 12 + 1024;
     cudaError_t e = cudaFuncSetAttribute(k_fsp_mma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

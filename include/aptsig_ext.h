@@ -90,7 +90,7 @@ int apx_so3_grid_cubic(float spacing_deg, float *quats, int64_t *Ng);
 int apx_fsp(apx_plan *plan, const float *centres, int64_t M, float k_max, int32_t L, float *out, uint32_t *counts,
             void *cuda_stream);
 /* Kernel choice of apx_fsp: 0 (default) = the tensor-core kernel (Eq. 2 per z-slice pair as one real GEMM of fp16 hi + lo
- * split operands, fp32 accumulation in TMEM), with the FP32 kernel serving ROIs of more than 2752 ions in the same stream;
+ * split operands, fp32 accumulation in TMEM), with the FP32 kernel serving ROIs of more than 2560 ions in the same stream;
  * 1 = the FP32-pipe kernel for everything.  Results agree within the tolerance derived in DESIGN.md section 2. */
 int apx_fsp_set_path(apx_plan *plan, int32_t path);
 

@@ -27,7 +27,7 @@ constexpr int kFmTileBytes = 128 * 128;       // 128 rows x 64 fp16 (K-major, SW
 constexpr int kFmPairs = 2;                   // z-slice pairs per CTA: one B' tile and one set of ey / ex factors feed all of them
 constexpr int kFmSlices = 2 * kFmPairs;
 constexpr int kFmStageBytes = (2 * kFmPairs + 2) * kFmTileBytes;   // (Ah, Al) per slice pair, Bh, Bl
-constexpr int kFmCap = 2752;                  // ions held in shared memory beside the two stages
+constexpr int kFmCap = 2560;                  // ions held in shared memory beside the two stages
 
 struct FspMmaParams {
     const float4 *sorted;
@@ -144,7 +144,8 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
     __shared__ uint64_t s_done[2], s_final;
     __shared__ uint32_t s_tmem;
     __shared__ int s_n;
-    __shared__ float2 s_ion[kFmSlices + 2][kFmChunk];   // per ion of the chunk: ez of the CTA's slices, step factors along y, x
+    __shared__ float2 s_ion[2][kFmSlices + 2][kFmChunk];   // per ion of a chunk: ez of the CTA's slices, step factors along y, x;
+                                                            // [c & 1]: chunk c's are computed while chunk c - 1 is built
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int L = p.L;
@@ -214,24 +215,30 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
     uint32_t tile_off[kFmPer];
 #pragma unroll
     for (int u = 0; u < kFmPer; ++u) tile_off[u] = fm_off(kFmPer * (tid >> 5) + u, tid & 31);
-    for (int c = 0; c < nchunks; ++c) {
-        const int s = c & 1, use = c >> 1;
-        if (use >= 1) fm_mbar_wait(&s_done[s], (uint32_t)((use - 1) & 1));        // the MMAs that read this stage have completed
-        unsigned char *A = stage0 + s * kFmStageBytes, *Bh = A + 2 * kFmPairs * kFmTileBytes, *Bl = Bh + kFmTileBytes;
-        const int w0 = c * kFmChunk;
-        // per-ion factors of the chunk, computed once: phases along z for the two slices and the step factors exp(-2 pi i dk d)
-        // along y and x (sincospif: exact argument reduction)
+    // per-ion factors of chunk c, computed once: phases along z for the CTA's slices and the step factors exp(-2 pi i dk d)
+    // along y and x (sincospif: exact argument reduction).  One factor per thread (the first 192 threads); chunk c + 1's are
+    // computed behind the tile build of chunk c and published by its barrier.
+    auto ion_factors = [&](int c) {
         if (tid < (kFmSlices + 2) * kFmChunk) {
-            const int j = tid & (kFmChunk - 1), which = tid / kFmChunk;
+            const int j = tid & (kFmChunk - 1), which = tid / kFmChunk, w0 = c * kFmChunk;
             float2 e = make_float2(0.f, 0.f);
             if (w0 + j < n) {
                 if (which < kFmSlices) e = iz0 + which < L ? fm_phase(p.kaxis[min(iz0 + which, L - 1)], ions[3 * (w0 + j) + 2]) : e;
                 else if (which == kFmSlices) e = fm_phase(p.dk, ions[3 * (w0 + j) + 1]);
                 else e = fm_phase(p.dk, ions[3 * (w0 + j)]);
             }
-            s_ion[which][j] = e;
+            s_ion[c & 1][which][j] = e;
         }
-        __syncthreads();
+    };
+    for (int c = 0; c < nchunks; ++c) {
+        const int s = c & 1, use = c >> 1;
+        if (use >= 1) fm_mbar_wait(&s_done[s], (uint32_t)((use - 1) & 1));        // the MMAs that read this stage have completed
+        unsigned char *A = stage0 + s * kFmStageBytes, *Bh = A + 2 * kFmPairs * kFmTileBytes, *Bl = Bh + kFmTileBytes;
+        const int w0 = c * kFmChunk;
+        if (c == 0) {
+            ion_factors(0);
+            __syncthreads();
+        }
         // thread = (ion j of the chunk, kFmPer consecutive iy and ix): the phase factor of the first one comes from sincospif,
         // the next ones by multiplying with the step factor -- a few fp32 complex products add < 4e-7 to the phase, inside the
         // tolerance budget of DESIGN.md section 2.  A warp writes one 128-byte operand row per store (32 consecutive K pairs):
@@ -239,8 +246,9 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
         // tile that lies inside the k grid (the common case) takes the copy without the validity selects.
         {
             const bool full = w0 + kFmChunk <= n && iy0 + 64 <= L && ix0 + 64 <= L && z_all_valid;
-            if (full) fm_build_tiles<true>(p, A, Bh, Bl, ions, s_ion, tile_off, w0, n, iy0, ix0, L, tid);
-            else fm_build_tiles<false>(p, A, Bh, Bl, ions, s_ion, tile_off, w0, n, iy0, ix0, L, tid);
+            if (full) fm_build_tiles<true>(p, A, Bh, Bl, ions, s_ion[c & 1], tile_off, w0, n, iy0, ix0, L, tid);
+            else fm_build_tiles<false>(p, A, Bh, Bl, ions, s_ion[c & 1], tile_off, w0, n, iy0, ix0, L, tid);
+            if (c + 1 < nchunks) ion_factors(c + 1);
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");       // operand tiles -> async proxy (tensor core)
         asm volatile("tcgen05.fence::before_thread_sync;");

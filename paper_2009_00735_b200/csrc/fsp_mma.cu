@@ -20,7 +20,9 @@
 
 namespace apx {
 
-constexpr int kFmThreads = 512;
+constexpr int kFmThreads = 512;                // threads that build the operand tiles (16 warps)
+constexpr int kFmAll = kFmThreads + 32;         // + one warp that only issues the MMAs, so that no builder arrives late at the
+                                                // chunk barrier because it had the tensor-core instructions to issue
 constexpr int kFmPer = 64 / (kFmThreads / 32);   // consecutive iy / ix per thread when the operand tiles are built
 constexpr int kFmChunk = 32;                  // ions per chunk
 constexpr int kFmTileBytes = 128 * 128;       // 128 rows x 64 fp16 (K-major, SWIZZLE_128B)
@@ -135,7 +137,7 @@ __device__ __forceinline__ void fm_build_tiles(const FspMmaParams &p, unsigned c
     }
 }
 
-__global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant__ FspMmaParams p)
+__global__ void __launch_bounds__(kFmAll, 1) k_fsp_mma(const __grid_constant__ FspMmaParams p)
 {
     extern __shared__ unsigned char fm_raw[];
     unsigned char *smem = fm_raw + ((1024u - (fm_smem_u32(fm_raw) & 1023u)) & 1023u);      // 1024-byte aligned (swizzle atoms)
@@ -176,7 +178,8 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
     const uint32_t tmem = s_tmem;
 
     // ---- gather (as in fsp.cu) ------------------------------------------------------------------------------------
-    if (g.n_accepted) {
+    const bool builder = wid < kFmThreads / 32;
+    if (g.n_accepted && builder) {
         const int ny_r = rc.iy1 - rc.iy0 + 1, nz_r = rc.iz1 - rc.iz0 + 1;
         for (int row = wid; row < ny_r * nz_r; row += kFmThreads / 32) {
             const int iy = rc.iy0 + row % ny_r, izc = rc.iz0 + row / ny_r;
@@ -232,11 +235,11 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
     };
     for (int c = 0; c < nchunks; ++c) {
         const int s = c & 1, use = c >> 1;
-        if (use >= 1) fm_mbar_wait(&s_done[s], (uint32_t)((use - 1) & 1));        // the MMAs that read this stage have completed
+        if (builder && use >= 1) fm_mbar_wait(&s_done[s], (uint32_t)((use - 1) & 1));   // the MMAs that read this stage have completed
         unsigned char *A = stage0 + s * kFmStageBytes, *Bh = A + 2 * kFmPairs * kFmTileBytes, *Bl = Bh + kFmTileBytes;
         const int w0 = c * kFmChunk;
         if (c == 0) {
-            ion_factors(0);
+            if (builder) ion_factors(0);
             __syncthreads();
         }
         // thread = (ion j of the chunk, kFmPer consecutive iy and ix): the phase factor of the first one comes from sincospif,
@@ -244,7 +247,7 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
         // tolerance budget of DESIGN.md section 2.  A warp writes one 128-byte operand row per store (32 consecutive K pairs):
         // conflict-free.  Splits x = hi + lo / 2048 are taken two values at a time (cvt.rn.f16x2.f32).  A chunk of 32 ions in a
         // tile that lies inside the k grid (the common case) takes the copy without the validity selects.
-        {
+        if (builder) {
             const bool full = w0 + kFmChunk <= n && iy0 + 64 <= L && ix0 + 64 <= L && z_all_valid;
             if (full) fm_build_tiles<true>(p, A, Bh, Bl, ions, s_ion[c & 1], tile_off, w0, n, iy0, ix0, L, tid);
             else fm_build_tiles<false>(p, A, Bh, Bl, ions, s_ion[c & 1], tile_off, w0, n, iy0, ix0, L, tid);
@@ -253,7 +256,7 @@ __global__ void __launch_bounds__(kFmThreads, 1) k_fsp_mma(const __grid_constant
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");       // operand tiles -> async proxy (tensor core)
         asm volatile("tcgen05.fence::before_thread_sync;");
         __syncthreads();
-        if (tid == 0) {
+        if (tid == kFmThreads) {                                           // (first lane of the issuing warp)
             asm volatile("tcgen05.fence::after_thread_sync;");
             const uint32_t bh = (fm_smem_u32(Bh) >> 4) & 0x3FFFu, bl = (fm_smem_u32(Bl) >> 4) & 0x3FFFu;
 #pragma unroll
@@ -330,7 +333,7 @@ cudaError_t launch_fsp_mma(Plan *p, const float *centres, int64_t M, int L, floa
     const size_t smem = 2 * (size_t)kFmStageBytes + (size_t)q.cap * 12 + 1024;
     cudaError_t e = cudaFuncSetAttribute(k_fsp_mma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_fsp_mma<<<(unsigned)blocks, kFmThreads, smem, st>>>(q);
+    k_fsp_mma<<<(unsigned)blocks, kFmAll, smem, st>>>(q);
     return cudaGetLastError();
 }
 
@@ -347,7 +350,7 @@ cudaError_t launch_fsp_mma_at(Plan *p, const float *kaxis, const float *centres,
     const size_t smem = 2 * (size_t)kFmStageBytes + (size_t)q.cap * 12 + 1024;
     cudaError_t e = cudaFuncSetAttribute(k_fsp_mma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_fsp_mma<<<(unsigned)blocks, kFmThreads, smem, st>>>(q);
+    k_fsp_mma<<<(unsigned)blocks, kFmAll, smem, st>>>(q);
     return cudaGetLastError();
 }
 

@@ -19,6 +19,7 @@
 //     orientation index among equals).
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <numeric>
@@ -31,7 +32,7 @@ namespace {
 constexpr int kMaxK = APX_INDEX_MAX_K;
 constexpr int kIdxWarps = 8;                    // material-point blocks per CTA
 constexpr int kGBatch = 4;                      // table rows staged per batch
-constexpr int64_t kChunkPoints = 8192;          // material points transposed and indexed per pass
+constexpr int64_t kChunkPoints = 2048;          // material points transposed and indexed per pass
 
 struct Indexer {
     int device, D, n_hat, n_hat_pad, sm_count;
@@ -356,9 +357,12 @@ extern "C" int apx_index(apx_indexer *ix, const float *sig, const uint32_t *coun
     DevGuard guard(ix->device);
     cudaStream_t st = (cudaStream_t)stream;
     const int64_t chunk = std::min<int64_t>(M, kChunkPoints);
-    // orientation ranges: about two CTAs per SM along the fastest grid axis, so that the CTAs resident at one time share
-    // the image blocks of one or two CTA rows in L2 (8 blocks x D x 128 B each)
-    int nranges = (int)std::min<int64_t>(ix->Ng, (int64_t)ix->sm_count * 2);
+    // orientation ranges: as many CTAs along the fastest grid axis as the machine holds at a time (six per SM: shared memory),
+    // so that the resident CTAs all work on ONE row of 8 image blocks (8 x D x 128 B = 42 MB at D = 40 962) and the gathers hit
+    // in L2; with two ranges per SM three rows (126 MB) were resident at once and 39 % of the sectors came from DRAM
+    int per_sm = 6;
+    if (const char *ev = std::getenv("APX_TUNE_INDEX_RANGES")) per_sm = std::max(1, std::atoi(ev));
+    int nranges = (int)std::min<int64_t>(ix->Ng, (int64_t)ix->sm_count * per_sm);
     if (chunk > ix->cap_img_points) {
         if (ix->d_imgT) cudaFree(ix->d_imgT);
         ix->d_imgT = nullptr; ix->cap_img_points = 0;

@@ -627,4 +627,13 @@ def main():
 
 
 if __name__ == "__main__":
-    main()
+    # The contract is ONE JSON line on stdout.  Libraries write there too (NCCL prints its version banner to fd 1 when a
+    # communicator is created): everything that is not the result line goes to stderr, the line itself to the real stdout.
+    sys.stdout.flush()
+    _real_stdout = os.fdopen(os.dup(1), "w")
+    os.dup2(2, 1)
+    sys.stdout = _real_stdout
+    try:
+        main()
+    finally:
+        _real_stdout.flush()

@@ -562,6 +562,24 @@ def run_ours(args, rank, world, local_rank):
                      "ncu_capture": ncu_constant(kname, cfg, "capture"),
                      "tensor_tflops": tensor_flops / q_s / 1e12 if path == "mma" else None},
     }
+    if path == "mma" and lsu:
+        # What the kernel actually keeps busy: the shared-memory arrays, 128 B = one wavefront per clock and
+        # SM.  LSU wavefronts from the committed ncu capture (scaled by material points); the tensor core's operand reads and the
+        # TMA clears go through the same arrays and are counted from the layout (B <= 1024: double-buffered, TMA clears; B = 2048:
+        # the clears are plain stores and already in the LSU figure).  Reported beside the algorithmic fraction.
+        K, N = B // nb, (4 * W + 15) // 16 * 16
+        sbo = 160 if nb == 4 else 192
+        hist_bytes = (K // 8) * 16 * sbo
+        n_groups = groups * M_tot
+        operand = n_groups * (K // 16) * (128 * 16 * 2 + N * 16 * 2) / 128.0
+        clear = n_groups * hist_bytes / 128.0 if nb == 4 else 0.0
+        clk = q_s * clocks["sm_mhz"] * 1e6 * SM_COUNT * world
+        out["roofline"]["shared_memory_pipe"] = {
+            "lsu_busy_frac": lsu / clk, "with_tensor_operands_and_tma_clears_est": (lsu + operand + clear) / clk,
+            "lsu_wavefronts": lsu, "tensor_operand_wavefronts": operand, "tma_clear_wavefronts": clear, "sm_clocks": clk,
+            "note": "executed shared-memory wavefronts / SM clocks: the resource this design saturates.  The second figure counts "
+                    "the tensor core's operand reads and the TMA clears against the same 128 B/clk; it can exceed 1, so they have "
+                    "some bandwidth of their own"}
     if not args.no_cpu_baseline:
         # bounded samples of the same workload: all cores until >= 10 s of CPU work, then one core on 2 points
         odirs = np.ascontiguousarray(dirs)

@@ -253,7 +253,7 @@ def test_fsp_against_oracle_small_grids():
     plan.apx_ingest(torch.from_numpy(xyz).to(dev), torch.from_numpy(types).to(dev))
     centres = np.array([[0, 0, 0], [0.4, -0.3, 0.2], [2.6, 0, 0], [9, 9, 9]], np.float32)       # full, shifted, partial, empty
     for path in (0, 1):
-        for L, k_max in ((9, 5.0), (16, 2.0 * math.pi), (33, 6.0), (1, 3.0)):
+        for L, k_max in ((9, 5.0), (16, 2.0 * math.pi), (33, 6.0), (1, 3.0), (6, 3.0), (7, 4.5)):      # every L mod 4: four z-slices per CTA
             gc = _fsp_check(plan, xyz, types, centres, R, k_max, L, path=path)
             assert gc[3] == 0 and gc[0] > 300
     plan.apx_plan_destroy()

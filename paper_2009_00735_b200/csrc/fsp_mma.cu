@@ -77,9 +77,11 @@ __device__ __forceinline__ void fm_split(float x, uint16_t &hi, uint16_t &lo)
 // two values at once: (a, b) -> hi = half2(a, b), lo = half2((a - hi.a) * 2048, (b - hi.b) * 2048), a in the low half
 __device__ __forceinline__ void fm_split2(float a, float b, uint32_t &hi, uint32_t &lo)
 {
+    // lo = rn16((a - hi) * 2048): a - hi is exact in fp32 and so is the scaling, hence fma(a, 2048, -2048 * hi) -- with
+    // -2048 * hi formed exactly on the packed halves -- is the same number in one rounding-free step less per value
     const __half2 h = __floats2half2_rn(a, b);
-    const float2 hf = __half22float2(h);
-    const __half2 l = __floats2half2_rn((a - hf.x) * 2048.0f, (b - hf.y) * 2048.0f);
+    const float2 hs = __half22float2(__hmul2(h, __floats2half2_rn(-2048.0f, -2048.0f)));
+    const __half2 l = __floats2half2_rn(__fmaf_rn(a, 2048.0f, hs.x), __fmaf_rn(b, 2048.0f, hs.y));
     hi = *reinterpret_cast<const uint32_t *>(&h);
     lo = *reinterpret_cast<const uint32_t *>(&l);
 }
